@@ -1,0 +1,253 @@
+"""ORACLE (test infrastructure, NOT the product): ctypes binding of
+``pic_oracle.c`` plus ``OracleSim``, the explicit EM-PIC cycle composed stage
+by stage in the order of SURVEY.md section 8(c.1) (section II:
+"explicit algorithms, which iterate forward in time").
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
+/ ``--impl reference`` legs may import this module.  It imports nothing from
+``paper_2303_12873_b200`` and shares no code with the CUDA path.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pic_oracle.c")
+_HDR = os.path.join(_HERE, "pic_oracle.h")
+_LIB = os.path.join(_HERE, "libpic_oracle.so")
+
+_dp = C.POINTER(C.c_double)
+_lp = C.POINTER(C.c_longlong)
+
+
+class OraGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+                ("xmin", C.c_double), ("ymin", C.c_double), ("zmin", C.c_double)]
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (no FMA contraction).  Returns the .so path."""
+    stale = (not os.path.exists(_LIB)
+             or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_HDR)))
+    if force or stale:
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-std=c11", "-Wall", "-shared",
+                               "-fPIC", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        G = C.POINTER(OraGrid)
+        L.ora_const_c.restype = C.c_double
+        L.ora_const_eps0.restype = C.c_double
+        L.ora_shape.restype = C.c_double
+        L.ora_shape.argtypes = [C.c_int, C.c_double]
+        L.ora_courant_dt.restype = C.c_double
+        L.ora_courant_dt.argtypes = [G]
+        L.ora_gather.argtypes = [G, C.c_int, C.c_longlong] + [_dp] * 15
+        L.ora_boris.argtypes = [C.c_longlong, C.c_double, C.c_double, C.c_double] + [_dp] * 9
+        L.ora_move.argtypes = [C.c_longlong, C.c_double] + [_dp] * 9
+        L.ora_deposit_esirkepov.argtypes = [G, C.c_int, C.c_longlong, C.c_double, C.c_double] + [_dp] * 10
+        L.ora_wrap.argtypes = [G, C.c_longlong] + [_dp] * 3
+        L.ora_yee_push_B.argtypes = [G, C.c_double] + [_dp] * 6
+        L.ora_yee_push_E.argtypes = [G, C.c_double] + [_dp] * 9
+        L.ora_deposit_rho.argtypes = [G, C.c_int, C.c_longlong, C.c_double] + [_dp] * 5
+        L.ora_cell_keys.argtypes = [G, C.c_longlong] + [_dp] * 3 + [_lp]
+        L.ora_counting_sort.argtypes = [C.c_longlong, C.c_longlong, _lp, _lp, _lp]
+        _lib = L
+    return _lib
+
+
+def _d(a: np.ndarray):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"], "need contiguous float64"
+    return a.ctypes.data_as(_dp)
+
+
+def _l(a: np.ndarray):
+    assert a.dtype == np.int64 and a.flags["C_CONTIGUOUS"], "need contiguous int64"
+    return a.ctypes.data_as(_lp)
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise RuntimeError("oracle %s failed with code %d" % (what, rc))
+
+
+C_LIGHT = 299792458.0
+EPS0 = 8.8541878128e-12
+
+
+def make_grid(nx, ny, nz, dx, dy, dz, xmin=0.0, ymin=0.0, zmin=0.0) -> OraGrid:
+    return OraGrid(int(nx), int(ny), int(nz), float(dx), float(dy), float(dz),
+                   float(xmin), float(ymin), float(zmin))
+
+
+def shape(n: int, r: float) -> float:
+    return lib().ora_shape(int(n), float(r))
+
+
+def courant_dt(g: OraGrid) -> float:
+    return lib().ora_courant_dt(C.byref(g))
+
+
+def gather(g: OraGrid, order: int, x, y, z, E, B):
+    """E, B: 3-tuples of flat nx*ny*nz arrays.  Returns (Exp,Eyp,Ezp,Bxp,Byp,Bzp)."""
+    x, y, z = _f64(x), _f64(y), _f64(z)
+    n = x.size
+    F = [_f64(a) for a in (*E, *B)]
+    out = [np.empty(n) for _ in range(6)]
+    _check(lib().ora_gather(C.byref(g), order, n, _d(x), _d(y), _d(z), *[_d(a) for a in F],
+                            *[_d(a) for a in out]), "gather")
+    return tuple(out)
+
+
+def boris(q, m, dt, ux, uy, uz, Ep, Bp):
+    """In place on ux,uy,uz (contiguous float64)."""
+    n = ux.size
+    _check(lib().ora_boris(n, q, m, dt, _d(ux), _d(uy), _d(uz), *[_d(_f64(a)) for a in (*Ep, *Bp)]),
+           "boris")
+
+
+def move(dt, x, y, z, ux, uy, uz):
+    n = x.size
+    out = [np.empty(n) for _ in range(3)]
+    _check(lib().ora_move(n, dt, _d(x), _d(y), _d(z), _d(ux), _d(uy), _d(uz), *[_d(a) for a in out]),
+           "move")
+    return tuple(out)
+
+
+def deposit_esirkepov(g, order, q, dt, w, p0, p1, J):
+    """Accumulates into J = (Jx,Jy,Jz), flat contiguous float64 arrays."""
+    n = p0[0].size
+    rc = lib().ora_deposit_esirkepov(C.byref(g), order, n, q, dt, _d(_f64(w)),
+                                     *[_d(_f64(a)) for a in p0], *[_d(_f64(a)) for a in p1],
+                                     *[_d(a) for a in J])
+    _check(rc, "deposit_esirkepov")
+
+
+def wrap(g, x, y, z):
+    _check(lib().ora_wrap(C.byref(g), x.size, _d(x), _d(y), _d(z)), "wrap")
+
+
+def yee_push_B(g, dth, E, B):
+    _check(lib().ora_yee_push_B(C.byref(g), dth, *[_d(a) for a in E], *[_d(a) for a in B]), "yee_push_B")
+
+
+def yee_push_E(g, dt, E, B, J):
+    _check(lib().ora_yee_push_E(C.byref(g), dt, *[_d(a) for a in E], *[_d(a) for a in B],
+                                *[_d(a) for a in J]), "yee_push_E")
+
+
+def deposit_rho(g, order, q, w, x, y, z, rho):
+    _check(lib().ora_deposit_rho(C.byref(g), order, x.size, q, _d(_f64(w)), _d(_f64(x)), _d(_f64(y)),
+                                 _d(_f64(z)), _d(rho)), "deposit_rho")
+
+
+def cell_keys(g, x, y, z) -> np.ndarray:
+    key = np.empty(x.size, dtype=np.int64)
+    _check(lib().ora_cell_keys(C.byref(g), x.size, _d(_f64(x)), _d(_f64(y)), _d(_f64(z)), _l(key)),
+           "cell_keys")
+    return key
+
+
+def counting_sort(ncell: int, key: np.ndarray):
+    perm = np.empty(key.size, dtype=np.int64)
+    off = np.empty(ncell + 1, dtype=np.int64)
+    _check(lib().ora_counting_sort(ncell, key.size, _l(key), _l(perm), _l(off)), "counting_sort")
+    return perm, off
+
+
+class _Species:
+    __slots__ = ("q", "m", "x", "y", "z", "ux", "uy", "uz", "w", "id")
+
+
+class OracleSim:
+    """The PIC cycle of SURVEY.md 8(c.1), steps 1-8, on host arrays.  Mirrors
+    the method names of the CUDA binding so one test can drive both."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, dt, order, nspecies):
+        self.g = make_grid(nx, ny, nz, dx, dy, dz, xmin, ymin, zmin)
+        if order not in (1, 2, 3):
+            raise ValueError("order must be 1, 2 or 3")
+        if not (0.0 < dt <= courant_dt(self.g)):
+            raise ValueError("dt outside (0, Courant limit]")
+        self.dt, self.order = float(dt), int(order)
+        self.ncell = nx * ny * nz
+        self.E = [np.zeros(self.ncell) for _ in range(3)]
+        self.B = [np.zeros(self.ncell) for _ in range(3)]
+        self.J = [np.zeros(self.ncell) for _ in range(3)]
+        self.species: list[_Species | None] = [None] * nspecies
+        self.cell_offset: list[np.ndarray | None] = [None] * nspecies
+
+    def set_fields(self, Ex=None, Ey=None, Ez=None, Bx=None, By=None, Bz=None):
+        for dst, src in zip(self.E + self.B, (Ex, Ey, Ez, Bx, By, Bz)):
+            dst[:] = 0.0 if src is None else np.asarray(src, dtype=np.float64).reshape(-1)
+
+    def load_particles(self, s, q, m, x, y, z, ux, uy, uz, w):
+        sp = _Species()
+        sp.q, sp.m = float(q), float(m)
+        for name, a in zip(("x", "y", "z", "ux", "uy", "uz", "w"), (x, y, z, ux, uy, uz, w)):
+            setattr(sp, name, np.array(a, dtype=np.float64, copy=True).reshape(-1))
+        sp.id = np.arange(sp.x.size, dtype=np.uint64)
+        self.species[s] = sp
+        self.cell_offset[s] = None
+
+    def step(self, nsteps=1):
+        g, dt, n = self.g, self.dt, self.order
+        for _ in range(nsteps):
+            for a in self.J:                       # reading R13: J overwritten each step
+                a[:] = 0.0
+            for sp in self.species:
+                if sp is None or sp.x.size == 0:
+                    continue
+                F = gather(g, n, sp.x, sp.y, sp.z, self.E, self.B)                 # step 1
+                boris(sp.q, sp.m, dt, sp.ux, sp.uy, sp.uz, F[:3], F[3:])          # step 2
+                x1, y1, z1 = move(dt, sp.x, sp.y, sp.z, sp.ux, sp.uy, sp.uz)      # step 3
+                deposit_esirkepov(g, n, sp.q, dt, sp.w, (sp.x, sp.y, sp.z), (x1, y1, z1), self.J)  # 4
+                wrap(g, x1, y1, z1)                                               # step 5
+                sp.x, sp.y, sp.z = x1, y1, z1
+            yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 6
+            yee_push_E(g, dt, self.E, self.B, self.J)                             # step 7
+            yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 8
+
+    def sort(self):
+        for s, sp in enumerate(self.species):
+            if sp is None:
+                continue
+            key = cell_keys(self.g, sp.x, sp.y, sp.z)
+            perm, off = counting_sort(self.ncell, key)
+            for name in ("x", "y", "z", "ux", "uy", "uz", "w", "id"):
+                setattr(sp, name, np.ascontiguousarray(getattr(sp, name)[perm]))
+            self.cell_offset[s] = off
+
+    def get_fields(self):
+        return {k: v.copy() for k, v in zip(("Ex", "Ey", "Ez", "Bx", "By", "Bz", "Jx", "Jy", "Jz"),
+                                            self.E + self.B + self.J)}
+
+    def get_particles(self, s):
+        sp = self.species[s]
+        return {k: getattr(sp, k).copy() for k in ("x", "y", "z", "ux", "uy", "uz", "w", "id")}
+
+    def deposit_rho(self, s=-1):
+        rho = np.zeros(self.ncell)
+        for i, sp in enumerate(self.species):
+            if sp is None or (s >= 0 and i != s):
+                continue
+            deposit_rho(self.g, self.order, sp.q, sp.w, sp.x, sp.y, sp.z, rho)
+        return rho
