@@ -1,0 +1,226 @@
+/*
+ * pic.h -- C ABI of libpic_b200.so: the fp64 explicit electromagnetic
+ * particle-in-cell (PIC) hot path on one NVIDIA B200 (sm_100a).
+ *
+ * What the calls follow.  PAPER.md:45 (section II) fixes the method: a
+ * "fully-kinetic, electromagnetic particle-in-cell" code with "explicit
+ * algorithms, which iterate forward in time"; PAPER.md:57 (section III.A)
+ * fixes the figure of merit ("parallel particle-and-cell update rate per
+ * second").  The five parts of one cycle -- order-1/2/3 field gather from the
+ * staggered Yee grid, relativistic Boris push, Esirkepov charge-conserving
+ * current deposition, Yee FDTD update of E and B, periodic per-cell counting
+ * sort -- and the names pic_init_grid / pic_load_particles / pic_step /
+ * pic_sort / pic_get_fields / pic_get_particles are stated in
+ * BASELINE.json:north_star; their arithmetic is written out in SURVEY.md
+ * section 8(c.1) and DESIGN.md ("The path", "Readings").
+ *
+ * Conventions common to all calls
+ *   - SI units.  u = gamma*v [m/s].  c = 299792458 m/s, eps0 = 8.8541878128e-12
+ *     F/m are compiled in; charge q [C] and mass m [kg] are per species.
+ *   - Field arrays crossing this ABI are GUARD-FREE, nx*ny*nz doubles per
+ *     component, index = i + nx*(j + ny*k) (x fastest).  All boundaries are
+ *     periodic.  Yee staggering is implied by the component:
+ *       Ex,Jx (i+1/2,j,k)   Ey,Jy (i,j+1/2,k)   Ez,Jz (i,j,k+1/2)
+ *       Bx (i,j+1/2,k+1/2)  By (i+1/2,j,k+1/2)  Bz (i+1/2,j+1/2,k)
+ *       rho at nodes (i,j,k); node i sits at xmin + i*dx.
+ *     (Inside the library every component carries PIC_NG periodic guard cells
+ *     per side; they never cross the ABI.)
+ *   - Every pointer argument is tagged host or device by an *_on_device flag
+ *     of the call (0 = host memory, 1 = device memory of the same GPU).
+ *   - Ownership: the caller owns the device arena and the CUDA stream given
+ *     to pic_init_grid and keeps both alive until pic_destroy.  The library
+ *     never allocates or frees device memory; it owns only its host context.
+ *     pic_load_particles / pic_set_fields copy in, pic_get_* copy out into
+ *     caller buffers.
+ *   - Errors: every call returns PIC_OK (0) or a negative code; no exceptions,
+ *     no abort; a NULL context gives PIC_EINVAL.  pic_last_error returns a
+ *     context-owned string describing the last failure.
+ *   - All device work is enqueued on the context's stream.  pic_step and
+ *     pic_sort are asynchronous; pic_get_*, pic_deposit_rho, pic_sync and
+ *     pic_get_counters synchronise that stream.
+ *   - There is no CPU fallback anywhere behind this ABI.
+ */
+#ifndef PIC_B200_H
+#define PIC_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pic_ctx pic_ctx; /* opaque: one simulation on one GPU */
+
+enum {
+    PIC_OK = 0,
+    PIC_EINVAL = -1, /* bad argument: order, sizes, NULL, dt above the Courant limit,
+                        particle outside the box or non-finite at load              */
+    PIC_ENOMEM = -2, /* arena too small / more particles than np_max               */
+    PIC_ECUDA = -3,  /* CUDA runtime error (text in pic_last_error)                */
+    PIC_ESTATE = -4, /* call order: step/sort/get before the species were loaded   */
+    PIC_EPHYS = -5   /* raised on the device during a step: a particle moved >= 1
+                        cell in one step or its position became non-finite; it is
+                        reported by the next synchronising call                    */
+};
+
+#define PIC_NG 4 /* guard cells per side of every internal field array */
+
+/* Number of entries written by pic_get_counters. */
+#define PIC_NCOUNTERS 8
+
+/*
+ * Bytes of device arena pic_init_grid needs.  Pure function of its arguments
+ * (no CUDA call).  np_max[s] = capacity of species s (particles); the library
+ * holds two SoA copies of every species (out-of-place sort).
+ * Errors: PIC_EINVAL (nx,ny,nz < 1, order not in 1..3, nspecies not in 1..8,
+ * np_max[s] < 0 or >= 2^31, NULL pointers).
+ */
+int pic_query_arena(int nx, int ny, int nz, int order, int nspecies,
+                    const long long* np_max /*host*/, size_t* bytes /*host*/);
+
+/*
+ * Create a simulation (SURVEY 8(c.1) "State at the start of step n").
+ *   nx,ny,nz        cells per dimension (= unknowns per field component)
+ *   dx,dy,dz        cell sizes [m] (> 0);  xmin,ymin,zmin  position of node 0
+ *   dt              time step [s], 0 < dt <= 1/(c*sqrt(1/dx^2+1/dy^2+1/dz^2))
+ *                   (3-D Courant limit, reading R17), else PIC_EINVAL
+ *   order           B-spline degree of the particle shape, 1, 2 or 3 (R4)
+ *   nspecies, np_max[s]   as in pic_query_arena
+ *   arena_dev, arena_bytes  DEVICE memory, 256-byte aligned, >= pic_query_arena
+ *   cuda_stream     a cudaStream_t (NULL = legacy default stream)
+ * All fields start at zero and every species is empty.  The arena is zeroed
+ * asynchronously on the stream.
+ */
+int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, double dz,
+                  double xmin, double ymin, double zmin, double dt, int order, int nspecies,
+                  const long long* np_max /*host*/, void* arena_dev, size_t arena_bytes,
+                  void* cuda_stream);
+
+/*
+ * Overwrite E^n and B^n (both at integer time, reading R1).  Any pointer may
+ * be NULL (= that component becomes zero).  Guard-free arrays (see top);
+ * the library refreshes its periodic guard cells.
+ */
+int pic_set_fields(pic_ctx*, const double* Ex, const double* Ey, const double* Ez,
+                   const double* Bx, const double* By, const double* Bz, int src_on_device);
+
+/*
+ * Replace the content of species `species` by n particles: positions x,y,z [m]
+ * inside [min, min + N*d), momenta ux,uy,uz = gamma*v [m/s] taken as
+ * u^{n-1/2} (R9: no backward half-push is applied), weights w (real particles
+ * per macro-particle).  Particle p receives id = p (its load index), which
+ * travels with it through every sort.  The species becomes "unsorted".
+ * Errors: PIC_EINVAL (species index, n < 0, NULL with n > 0, a position
+ * outside the box or non-finite -- checked on the device, the call
+ * synchronises), PIC_ENOMEM (n > np_max[species]).
+ */
+int pic_load_particles(pic_ctx*, int species, double q, double m, long long n,
+                       const double* x, const double* y, const double* z,
+                       const double* ux, const double* uy, const double* uz,
+                       const double* w, int src_on_device);
+
+/*
+ * Advance nsteps PIC cycles (SURVEY 8(c.1) steps 1-8 per cycle):
+ *   J := 0;  for every species: gather E,B at x^n (order-n B-splines read at
+ *   the Yee locations), Boris push u^{n-1/2} -> u^{n+1/2}, move
+ *   x~ = x + dt*u/gamma, Esirkepov deposition of J^{n+1/2} from (x^n, x~),
+ *   periodic wrap;  B -= (dt/2) curl E;  E += dt (c^2 curl B - J/eps0);
+ *   B -= (dt/2) curl E.
+ * Correct for ANY particle order; a species that has been sorted (pic_sort)
+ * and is still close to sorted runs the fused per-tile kernel, anything else
+ * the global-atomic path.  Asynchronous.  Errors: PIC_ESTATE (no species
+ * loaded), PIC_EINVAL (nsteps < 0), PIC_ECUDA.
+ */
+int pic_step(pic_ctx*, int nsteps);
+
+/*
+ * Counting sort of every loaded species by cell key = i + nx*(j + ny*k),
+ * (i,j,k) = clamp(floor((x - xmin)/dx), 0, nx-1) etc. of the stored position:
+ * histogram, exclusive scan, scatter of x,y,z,ux,uy,uz,w,id into the second
+ * SoA buffer, buffer swap.  Afterwards keys are non-decreasing in container
+ * order; the order inside one cell is unspecified (R24).  Asynchronous.
+ */
+int pic_sort(pic_ctx*);
+
+/*
+ * Copy out E^n, B^n and the J^{n+1/2} of the last step (zeros before the
+ * first), guard-free.  NULL = skip that component.  Synchronises.
+ */
+int pic_get_fields(pic_ctx*, double* Ex, double* Ey, double* Ez, double* Bx, double* By,
+                   double* Bz, double* Jx, double* Jy, double* Jz, int dst_on_device);
+
+/*
+ * Copy out species `species` in container order.  *n (host) receives the
+ * particle count; every array pointer may be NULL (= skip) and otherwise has
+ * room for that many entries (call once with all-NULL arrays to learn n).
+ * id = load index.  Synchronises.
+ */
+int pic_get_particles(pic_ctx*, int species, long long* n /*host*/, double* x, double* y,
+                      double* z, double* ux, double* uy, double* uz, double* w,
+                      unsigned long long* id, int dst_on_device);
+
+/*
+ * Diagnostic (not on the step path): nodal charge density
+ * rho[i,j,k] = sum_p q w/(dx dy dz) S(xi-i) S(eta-j) S(zeta-k), same order as
+ * the simulation, of one species (species >= 0) or of all (-1).  nx*ny*nz
+ * doubles, guard-free.  Synchronises.
+ */
+int pic_deposit_rho(pic_ctx*, int species, double* rho, int dst_on_device);
+
+/*
+ * Copy out the cell offsets of the last pic_sort of `species`:
+ * nx*ny*nz + 1 unsigned 32-bit entries, offset[c] = first container index of
+ * cell c, offset[ncell] = n.  PIC_ESTATE if the species was never sorted.
+ */
+int pic_get_cell_offsets(pic_ctx*, int species, unsigned int* offsets, int dst_on_device);
+
+/*
+ * Device counters since pic_init_grid (host array of PIC_NCOUNTERS unsigned
+ * 64-bit values).  Synchronises.
+ *   [0] particle updates done by the fused per-tile kernel (fast deposit path)
+ *   [1] particle updates done by the fused kernel's in-tile slow path
+ *       (particle crossed a cell face or was not in its listed cell)
+ *   [2] particle updates done with global atomics (unsorted species, or a
+ *       particle found outside its tile's halo)
+ *   [3] kernels launched by the library
+ *   [4] steps completed     [5] sorts completed     [6],[7] reserved
+ */
+int pic_get_counters(pic_ctx*, unsigned long long* counters /*host*/);
+
+/*
+ * Per-stage device time of the LAST pic_step call when stage timing is on
+ * (pic_set_option("stage_timing",1)): milliseconds summed over that call's
+ * steps for  [0] zero J  [1] particles (gather+push+deposit, all species)
+ * [2] J guard fold  [3] Yee B (both halves, incl. guards)  [4] Yee E (incl.
+ * guards).  Host array of 5 floats.  Synchronises.  PIC_ESTATE if off.
+ */
+int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
+
+/*
+ * Options (all default 0 unless stated):
+ *   "stage_timing"   1 = record CUDA events around every stage of pic_step
+ *   "force_path"     0 = automatic, 1 = always the global-atomic particle
+ *                    kernel, 2 = always the fused per-tile kernel (requires a
+ *                    prior pic_sort, else PIC_ESTATE at pic_step)
+ *   "yee_tma"        1 (default) = TMA-staged Yee kernels, 0 = plain loads
+ * Unknown name: PIC_EINVAL.
+ */
+int pic_set_option(pic_ctx*, const char* name, long long value);
+
+/* Wait for the context's stream; returns a pending PIC_EPHYS / PIC_ECUDA. */
+int pic_sync(pic_ctx*);
+
+/* Context-owned, valid until the next call on this context.  NULL ctx gives a
+ * static string. */
+const char* pic_last_error(pic_ctx*);
+
+/* Free the host context (the arena and the stream stay the caller's). */
+int pic_destroy(pic_ctx*);
+
+/* Library version string, e.g. "pic_b200 0.1 (sm_100a)". */
+const char* pic_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIC_B200_H */

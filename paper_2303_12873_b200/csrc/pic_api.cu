@@ -1,0 +1,550 @@
+// pic_api.cu -- the C ABI of libpic_b200.so (include/pic.h): host context,
+// arena carving, call-order state machine, copies across the boundary, and
+// the per-step launch sequence of SURVEY 8(c.1) steps 1-8.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "pic_internal.h"
+
+using namespace pic;
+
+namespace {
+
+struct Species {
+    bool loaded = false;
+    bool sorted = false;        // cell_offset valid for the current buffer (up to drift since the last sort)
+    int steps_since_sort = 0;
+    long long n = 0, np_max = 0;
+    double q = 0.0, m = 1.0;
+    int cur = 0;                // which of the two SoA buffers is live
+    Particles buf[2];
+    unsigned int* cell_offset = nullptr;
+};
+
+constexpr int NSTAGE = 5;
+
+}  // namespace
+
+struct pic_ctx {
+    Grid g;
+    Fields f;
+    double* tmp = nullptr;      // one padded scratch component (rho, pack/unpack staging)
+    DevStatus* status = nullptr;
+    int order = 1, nspecies = 0;
+    Species sp[MAX_SPECIES];
+    SortScratch sort_scratch{};
+    cudaStream_t stream = nullptr;
+    char err[512] = {0};
+    int sticky = PIC_OK;
+    unsigned long long launches = 0, steps = 0, sorts = 0;
+    // options
+    int stage_timing = 0, force_path = 0, yee_tma = 1;
+    cudaEvent_t ev[NSTAGE + 2] = {};
+    bool ev_made = false;
+    float stage_ms[NSTAGE] = {};
+    bool stage_valid = false;
+};
+
+namespace {
+
+int fail(pic_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+int cuda_fail(pic_ctx* c, cudaError_t e, const char* what) {
+    c->sticky = PIC_ECUDA;
+    return fail(c, PIC_ECUDA, "CUDA error in %s: %s", what, cudaGetErrorString(e));
+}
+
+#define CU(c, call)                                         \
+    do {                                                    \
+        cudaError_t e_ = (call);                            \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); \
+    } while (0)
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+int padded_pitch(int nx) { return (nx + 2 * NG + 1) & ~1; }   // even: rows stay 16-byte aligned (TMA)
+
+struct Layout {
+    size_t status, fields, tmp, species[MAX_SPECIES], cell_offset[MAX_SPECIES], key, rank, block_sums, total;
+    size_t comp_bytes, np_bytes[MAX_SPECIES];
+};
+
+int make_layout(int nx, int ny, int nz, int nspecies, const long long* np_max, Layout* L) {
+    const size_t npad = (size_t)padded_pitch(nx) * (size_t)(ny + 2 * NG) * (size_t)(nz + 2 * NG);
+    const size_t ncell = (size_t)nx * ny * nz;
+    size_t off = 0;
+    L->status = off; off += align_up(sizeof(DevStatus));
+    L->comp_bytes = align_up(npad * sizeof(double));
+    L->fields = off; off += 9 * L->comp_bytes;
+    L->tmp = off; off += L->comp_bytes;
+    long long npm = 0;
+    for (int s = 0; s < nspecies; ++s) {
+        L->np_bytes[s] = align_up((size_t)np_max[s] * sizeof(double));
+        L->species[s] = off; off += 2 * 8 * L->np_bytes[s];
+        L->cell_offset[s] = off; off += align_up((ncell + 1) * sizeof(unsigned int));
+        if (np_max[s] > npm) npm = np_max[s];
+    }
+    L->key = off; off += align_up((size_t)npm * sizeof(unsigned int));
+    L->rank = off; off += align_up((size_t)npm * sizeof(unsigned int));
+    L->block_sums = off; off += align_up((size_t)sort_block_sums_len((long long)ncell) * sizeof(unsigned int));
+    L->total = off;
+    return 0;
+}
+
+int check_dims(int nx, int ny, int nz, int order, int nspecies, const long long* np_max) {
+    if (nx < 1 || ny < 1 || nz < 1 || order < 1 || order > 3 || nspecies < 1 || nspecies > MAX_SPECIES || !np_max)
+        return PIC_EINVAL;
+    if ((long long)nx * ny * nz >= (1LL << 31) - 1) return PIC_EINVAL;
+    for (int s = 0; s < nspecies; ++s)
+        if (np_max[s] < 0 || np_max[s] >= (1LL << 31)) return PIC_EINVAL;
+    return PIC_OK;
+}
+
+// ---- pack / unpack between the padded layout and guard-free arrays --------
+__global__ void pack_kernel(Grid g, const double* __restrict__ pad, double* __restrict__ flat) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.nx) return;
+    const int j = blockIdx.y, k = blockIdx.z;
+    flat[(long long)i + (long long)g.nx * (j + (long long)g.ny * k)] = pad[g.idx(i, j, k)];
+}
+
+__global__ void unpack_kernel(Grid g, const double* __restrict__ flat, double* __restrict__ pad) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.nx) return;
+    const int j = blockIdx.y, k = blockIdx.z;
+    pad[g.idx(i, j, k)] = flat[(long long)i + (long long)g.nx * (j + (long long)g.ny * k)];
+}
+
+dim3 cell_grid(const Grid& g) { return dim3((g.nx + 127) / 128, g.ny, g.nz); }
+
+// padded component -> caller's guard-free array (host or device)
+int copy_out(pic_ctx* c, const double* pad, double* dst, int on_device) {
+    if (!dst) return PIC_OK;
+    const size_t bytes = (size_t)c->g.nx * c->g.ny * c->g.nz * sizeof(double);
+    if (on_device) {
+        pack_kernel<<<cell_grid(c->g), 128, 0, c->stream>>>(c->g, pad, dst);
+        ++c->launches;
+    } else {
+        pack_kernel<<<cell_grid(c->g), 128, 0, c->stream>>>(c->g, pad, c->tmp);
+        ++c->launches;
+        CU(c, cudaMemcpyAsync(dst, c->tmp, bytes, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));   // tmp is reused by the next component
+    }
+    return PIC_OK;
+}
+
+int copy_in(pic_ctx* c, const double* src, double* pad, int on_device) {
+    const size_t bytes = (size_t)c->g.nx * c->g.ny * c->g.nz * sizeof(double);
+    if (!src) {
+        CU(c, cudaMemsetAsync(pad, 0, (size_t)c->g.npad * sizeof(double), c->stream));
+        return PIC_OK;
+    }
+    if (on_device) {
+        unpack_kernel<<<cell_grid(c->g), 128, 0, c->stream>>>(c->g, src, pad);
+    } else {
+        CU(c, cudaMemcpyAsync(c->tmp, src, bytes, cudaMemcpyHostToDevice, c->stream));
+        unpack_kernel<<<cell_grid(c->g), 128, 0, c->stream>>>(c->g, c->tmp, pad);
+    }
+    launch_fill_guards(c->g, pad, c->stream);
+    c->launches += 2;
+    if (!on_device) CU(c, cudaStreamSynchronize(c->stream));
+    return PIC_OK;
+}
+
+// read and clear the device flags; returns a pending PIC_EPHYS
+int poll_status(pic_ctx* c) {
+    DevStatus h;
+    CU(c, cudaMemcpyAsync(&h, c->status, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (h.ephys) {
+        int zero = 0;
+        CU(c, cudaMemcpyAsync(&c->status->ephys, &zero, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        return fail(c, PIC_EPHYS, "a particle moved >= 1 cell in one step or its position became non-finite");
+    }
+    return PIC_OK;
+}
+
+int sync_and_check(pic_ctx* c) {
+    if (c->sticky != PIC_OK) return c->sticky;
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
+    return poll_status(c);
+}
+
+bool use_tile_path(const pic_ctx* c, const Species& s) {
+    if (c->force_path == 1) return false;
+    return s.sorted;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* pic_version(void) { return "pic_b200 0.1 (sm_100a)"; }
+
+int pic_query_arena(int nx, int ny, int nz, int order, int nspecies, const long long* np_max, size_t* bytes) {
+    if (!bytes) return PIC_EINVAL;
+    int rc = check_dims(nx, ny, nz, order, nspecies, np_max);
+    if (rc != PIC_OK) return rc;
+    Layout L;
+    make_layout(nx, ny, nz, nspecies, np_max, &L);
+    *bytes = L.total;
+    return PIC_OK;
+}
+
+int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, double dz, double xmin, double ymin,
+                  double zmin, double dt, int order, int nspecies, const long long* np_max, void* arena_dev,
+                  size_t arena_bytes, void* cuda_stream) {
+    if (!out) return PIC_EINVAL;
+    *out = nullptr;
+    int rc = check_dims(nx, ny, nz, order, nspecies, np_max);
+    if (rc != PIC_OK) return rc;
+    if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !isfinite(dx) || !isfinite(dy) || !isfinite(dz) ||
+        !isfinite(xmin) || !isfinite(ymin) || !isfinite(zmin))
+        return PIC_EINVAL;
+    const double dt_max = 1.0 / (C_LIGHT * sqrt(1.0 / (dx * dx) + 1.0 / (dy * dy) + 1.0 / (dz * dz)));
+    if (!(dt > 0.0) || !(dt <= dt_max)) return PIC_EINVAL;
+    if (!arena_dev || ((uintptr_t)arena_dev & 255u)) return PIC_EINVAL;
+    Layout L;
+    make_layout(nx, ny, nz, nspecies, np_max, &L);
+    if (arena_bytes < L.total) return PIC_ENOMEM;
+
+    pic_ctx* c = new (std::nothrow) pic_ctx();
+    if (!c) return PIC_ENOMEM;
+    Grid& g = c->g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.px = padded_pitch(nx); g.py = ny + 2 * NG; g.pz = nz + 2 * NG;
+    g.sy = g.px; g.sz = (long long)g.px * g.py;
+    g.npad = g.sz * g.pz;
+    g.dx = dx; g.dy = dy; g.dz = dz;
+    g.inv_dx = 1.0 / dx; g.inv_dy = 1.0 / dy; g.inv_dz = 1.0 / dz;
+    g.xmin = xmin; g.ymin = ymin; g.zmin = zmin;
+    g.Lx = nx * dx; g.Ly = ny * dy; g.Lz = nz * dz;
+    g.xmax = xmin + g.Lx; g.ymax = ymin + g.Ly; g.zmax = zmin + g.Lz;
+    g.dt = dt;
+    c->order = order;
+    c->nspecies = nspecies;
+    c->stream = (cudaStream_t)cuda_stream;
+
+    char* base = (char*)arena_dev;
+    c->status = (DevStatus*)(base + L.status);
+    double** comps[9] = {&c->f.Ex, &c->f.Ey, &c->f.Ez, &c->f.Bx, &c->f.By, &c->f.Bz, &c->f.Jx, &c->f.Jy, &c->f.Jz};
+    for (int k = 0; k < 9; ++k) *comps[k] = (double*)(base + L.fields + (size_t)k * L.comp_bytes);
+    c->tmp = (double*)(base + L.tmp);
+    for (int s = 0; s < nspecies; ++s) {
+        Species& S = c->sp[s];
+        S.np_max = np_max[s];
+        for (int b = 0; b < 2; ++b) {
+            char* pb = base + L.species[s] + (size_t)b * 8 * L.np_bytes[s];
+            double** arr[7] = {&S.buf[b].x, &S.buf[b].y, &S.buf[b].z, &S.buf[b].ux, &S.buf[b].uy, &S.buf[b].uz,
+                               &S.buf[b].w};
+            for (int a = 0; a < 7; ++a) *arr[a] = (double*)(pb + (size_t)a * L.np_bytes[s]);
+            S.buf[b].id = (unsigned long long*)(pb + (size_t)7 * L.np_bytes[s]);
+        }
+        S.cell_offset = (unsigned int*)(base + L.cell_offset[s]);
+    }
+    c->sort_scratch.key = (unsigned int*)(base + L.key);
+    c->sort_scratch.rank = (unsigned int*)(base + L.rank);
+    c->sort_scratch.block_sums = (unsigned int*)(base + L.block_sums);
+    c->sort_scratch.block_sums_len = sort_block_sums_len((long long)nx * ny * nz);
+
+    // zero the status block, the fields and the scratch component (particles are written at load)
+    cudaError_t e = cudaMemsetAsync(base, 0, L.tmp + L.comp_bytes, c->stream);
+    if (e == cudaSuccess) e = (cudaError_t)tile_setup();
+    if (e != cudaSuccess) {
+        delete c;
+        return PIC_ECUDA;
+    }
+    *out = c;
+    return PIC_OK;
+}
+
+int pic_set_fields(pic_ctx* c, const double* Ex, const double* Ey, const double* Ez, const double* Bx,
+                   const double* By, const double* Bz, int src_on_device) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    const double* src[6] = {Ex, Ey, Ez, Bx, By, Bz};
+    double* dst[6] = {c->f.Ex, c->f.Ey, c->f.Ez, c->f.Bx, c->f.By, c->f.Bz};
+    for (int k = 0; k < 6; ++k) {
+        int rc = copy_in(c, src[k], dst[k], src_on_device);
+        if (rc != PIC_OK) return rc;
+    }
+    return PIC_OK;
+}
+
+int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n, const double* x, const double* y,
+                       const double* z, const double* ux, const double* uy, const double* uz, const double* w,
+                       int src_on_device) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    if (species < 0 || species >= c->nspecies) return fail(c, PIC_EINVAL, "species index %d out of range", species);
+    if (n < 0 || !(m > 0.0) || !isfinite(q) || !isfinite(m)) return fail(c, PIC_EINVAL, "bad n, q or m");
+    if (n > 0 && (!x || !y || !z || !ux || !uy || !uz || !w)) return fail(c, PIC_EINVAL, "NULL particle array");
+    Species& S = c->sp[species];
+    if (n > S.np_max) return fail(c, PIC_ENOMEM, "n = %lld exceeds np_max = %lld", n, S.np_max);
+    S.cur = 0;
+    Particles& P = S.buf[0];
+    const double* src[7] = {x, y, z, ux, uy, uz, w};
+    double* dst[7] = {P.x, P.y, P.z, P.ux, P.uy, P.uz, P.w};
+    const cudaMemcpyKind kind = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    for (int a = 0; a < 7 && n > 0; ++a)
+        CU(c, cudaMemcpyAsync(dst[a], src[a], (size_t)n * sizeof(double), kind, c->stream));
+    launch_iota(P.id, n, c->stream);
+    launch_validate(c->g, P, n, c->status, c->stream);
+    c->launches += (n > 0) ? 2 : 0;
+    DevStatus h;
+    CU(c, cudaMemcpyAsync(&h, c->status, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    S.q = q; S.m = m; S.n = n;
+    S.sorted = false; S.steps_since_sort = 0;
+    if (h.ebox) {
+        int zero = 0;
+        CU(c, cudaMemcpyAsync(&c->status->ebox, &zero, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        S.loaded = false; S.n = 0;
+        return fail(c, PIC_EINVAL, "species %d: a particle is outside the box or non-finite", species);
+    }
+    S.loaded = true;
+    return PIC_OK;
+}
+
+int pic_step(pic_ctx* c, int nsteps) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    if (nsteps < 0) return fail(c, PIC_EINVAL, "nsteps < 0");
+    bool any = false;
+    for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
+    if (!any) return fail(c, PIC_ESTATE, "pic_step before any pic_load_particles");
+    if (c->force_path == 2)
+        for (int s = 0; s < c->nspecies; ++s)
+            if (c->sp[s].loaded && !c->sp[s].sorted)
+                return fail(c, PIC_ESTATE, "force_path=2 needs pic_sort before pic_step (species %d)", s);
+    const bool timing = c->stage_timing != 0;
+    if (timing && !c->ev_made) {
+        for (int k = 0; k < NSTAGE + 2; ++k) CU(c, cudaEventCreate(&c->ev[k]));
+        c->ev_made = true;
+    }
+    if (timing) {
+        for (int k = 0; k < NSTAGE; ++k) c->stage_ms[k] = 0.f;
+        c->stage_valid = false;
+    }
+    const Grid& g = c->g;
+    const size_t comp_bytes = (size_t)g.npad * sizeof(double);
+    const bool tma = c->yee_tma != 0;
+    for (int it = 0; it < nsteps; ++it) {
+        if (timing) cudaEventRecord(c->ev[0], c->stream);
+        // J := 0 (R13).  Jx,Jy,Jz are contiguous in the arena.
+        CU(c, cudaMemsetAsync(c->f.Jx, 0, comp_bytes, c->stream));
+        CU(c, cudaMemsetAsync(c->f.Jy, 0, comp_bytes, c->stream));
+        CU(c, cudaMemsetAsync(c->f.Jz, 0, comp_bytes, c->stream));
+        if (timing) cudaEventRecord(c->ev[1], c->stream);
+        // steps 1-5 per species, in index order (R37)
+        for (int s = 0; s < c->nspecies; ++s) {
+            Species& S = c->sp[s];
+            if (!S.loaded || S.n == 0) continue;
+            const Particles& P = S.buf[S.cur];
+            if (use_tile_path(c, S)) {
+                c->launches += launch_particles_tile(g, c->f, P, S.n, S.q, S.m, c->order, S.cell_offset, c->status,
+                                                     c->stream);
+            } else {
+                launch_particles_global(g, c->f, P, S.n, S.q, S.m, c->order, c->status, c->stream);
+                c->launches += 1;
+            }
+            S.steps_since_sort += 1;
+        }
+        if (timing) cudaEventRecord(c->ev[2], c->stream);
+        // periodic fold of the J guard cells into the interior
+        launch_fold_guards(g, c->f.Jx, c->stream);
+        launch_fold_guards(g, c->f.Jy, c->stream);
+        launch_fold_guards(g, c->f.Jz, c->stream);
+        c->launches += 3;
+        if (timing) cudaEventRecord(c->ev[3], c->stream);
+        // steps 6-8
+        launch_push_B(g, c->f, 0.5 * g.dt, tma, c->stream);
+        if (timing) cudaEventRecord(c->ev[4], c->stream);
+        launch_push_E(g, c->f, g.dt, tma, c->stream);
+        if (timing) cudaEventRecord(c->ev[5], c->stream);
+        launch_push_B(g, c->f, 0.5 * g.dt, tma, c->stream);
+        c->launches += 3 * yee_num_launches(tma);
+        c->steps += 1;
+        if (timing) {
+            CU(c, cudaEventRecord(c->ev[6], c->stream));
+            CU(c, cudaEventSynchronize(c->ev[6]));
+            float t[6];
+            for (int k = 0; k < 6; ++k) cudaEventElapsedTime(&t[k], c->ev[k], c->ev[k + 1]);
+            c->stage_ms[0] += t[0];
+            c->stage_ms[1] += t[1];
+            c->stage_ms[2] += t[2];
+            c->stage_ms[3] += t[3] + t[5];
+            c->stage_ms[4] += t[4];
+            c->stage_valid = true;
+        }
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_step launch");
+    return PIC_OK;
+}
+
+int pic_sort(pic_ctx* c) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    bool any = false;
+    for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
+    if (!any) return fail(c, PIC_ESTATE, "pic_sort before any pic_load_particles");
+    for (int s = 0; s < c->nspecies; ++s) {
+        Species& S = c->sp[s];
+        if (!S.loaded) continue;
+        c->launches += launch_sort(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, S.cell_offset, c->sort_scratch,
+                                   c->stream);
+        S.cur ^= 1;
+        S.sorted = true;
+        S.steps_since_sort = 0;
+    }
+    c->sorts += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_sort launch");
+    return PIC_OK;
+}
+
+int pic_get_fields(pic_ctx* c, double* Ex, double* Ey, double* Ez, double* Bx, double* By, double* Bz, double* Jx,
+                   double* Jy, double* Jz, int dst_on_device) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    double* dst[9] = {Ex, Ey, Ez, Bx, By, Bz, Jx, Jy, Jz};
+    const double* src[9] = {c->f.Ex, c->f.Ey, c->f.Ez, c->f.Bx, c->f.By, c->f.Bz, c->f.Jx, c->f.Jy, c->f.Jz};
+    for (int k = 0; k < 9; ++k) {
+        int rc = copy_out(c, src[k], dst[k], dst_on_device);
+        if (rc != PIC_OK) return rc;
+    }
+    return sync_and_check(c);
+}
+
+int pic_get_particles(pic_ctx* c, int species, long long* n, double* x, double* y, double* z, double* ux,
+                      double* uy, double* uz, double* w, unsigned long long* id, int dst_on_device) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    if (species < 0 || species >= c->nspecies) return fail(c, PIC_EINVAL, "species index %d out of range", species);
+    Species& S = c->sp[species];
+    if (!S.loaded) return fail(c, PIC_ESTATE, "species %d was never loaded", species);
+    if (n) *n = S.n;
+    const Particles& P = S.buf[S.cur];
+    const cudaMemcpyKind kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    void* dst[8] = {x, y, z, ux, uy, uz, w, id};
+    const void* src[8] = {P.x, P.y, P.z, P.ux, P.uy, P.uz, P.w, P.id};
+    for (int a = 0; a < 8; ++a)
+        if (dst[a] && S.n > 0) CU(c, cudaMemcpyAsync(dst[a], src[a], (size_t)S.n * 8, kind, c->stream));
+    return sync_and_check(c);
+}
+
+int pic_deposit_rho(pic_ctx* c, int species, double* rho, int dst_on_device) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    if (species < -1 || species >= c->nspecies || !rho) return fail(c, PIC_EINVAL, "bad species index or NULL rho");
+    if (species >= 0 && !c->sp[species].loaded) return fail(c, PIC_ESTATE, "species %d was never loaded", species);
+    // tmp serves as the padded rho: deposit with global atomics, fold the guards, strip them on the way out
+    CU(c, cudaMemsetAsync(c->tmp, 0, (size_t)c->g.npad * sizeof(double), c->stream));
+    for (int s = 0; s < c->nspecies; ++s) {
+        Species& S = c->sp[s];
+        if (!S.loaded || (species >= 0 && s != species) || S.n == 0) continue;
+        launch_deposit_rho(c->g, S.buf[S.cur], S.n, S.q, c->order, c->tmp, c->stream);
+        c->launches += 1;
+    }
+    launch_fold_guards(c->g, c->tmp, c->stream);
+    c->launches += 1;
+    if (dst_on_device) {
+        pack_kernel<<<cell_grid(c->g), 128, 0, c->stream>>>(c->g, c->tmp, rho);
+        c->launches += 1;
+    } else {
+        // strided copy straight from the padded scratch to the caller's guard-free host array
+        cudaMemcpy3DParms p;
+        memset(&p, 0, sizeof(p));
+        p.srcPtr = make_cudaPitchedPtr(c->tmp, (size_t)c->g.px * sizeof(double), (size_t)c->g.px, (size_t)c->g.py);
+        p.srcPos = make_cudaPos((size_t)NG * sizeof(double), NG, NG);
+        p.dstPtr = make_cudaPitchedPtr(rho, (size_t)c->g.nx * sizeof(double), (size_t)c->g.nx, (size_t)c->g.ny);
+        p.extent = make_cudaExtent((size_t)c->g.nx * sizeof(double), (size_t)c->g.ny, (size_t)c->g.nz);
+        p.kind = cudaMemcpyDeviceToHost;
+        CU(c, cudaMemcpy3DAsync(&p, c->stream));
+    }
+    return sync_and_check(c);
+}
+
+int pic_get_cell_offsets(pic_ctx* c, int species, unsigned int* offsets, int dst_on_device) {
+    if (!c) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    if (species < 0 || species >= c->nspecies || !offsets) return fail(c, PIC_EINVAL, "bad species or NULL offsets");
+    Species& S = c->sp[species];
+    if (!S.loaded || !S.sorted) return fail(c, PIC_ESTATE, "species %d was never sorted", species);
+    const size_t bytes = ((size_t)c->g.nx * c->g.ny * c->g.nz + 1) * sizeof(unsigned int);
+    CU(c, cudaMemcpyAsync(offsets, S.cell_offset, bytes,
+                          dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+    return sync_and_check(c);
+}
+
+int pic_get_counters(pic_ctx* c, unsigned long long* counters) {
+    if (!c || !counters) return PIC_EINVAL;
+    if (c->sticky != PIC_OK) return c->sticky;
+    DevStatus h;
+    CU(c, cudaMemcpyAsync(&h, c->status, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    counters[0] = h.n_fast;
+    counters[1] = h.n_slow;
+    counters[2] = h.n_global;
+    counters[3] = c->launches;
+    counters[4] = c->steps;
+    counters[5] = c->sorts;
+    counters[6] = counters[7] = 0;
+    return PIC_OK;
+}
+
+int pic_get_stage_ms(pic_ctx* c, float* ms) {
+    if (!c || !ms) return PIC_EINVAL;
+    if (!c->stage_timing || !c->stage_valid) return fail(c, PIC_ESTATE, "stage timing is off or no step was timed");
+    for (int k = 0; k < NSTAGE; ++k) ms[k] = c->stage_ms[k];
+    return PIC_OK;
+}
+
+int pic_set_option(pic_ctx* c, const char* name, long long value) {
+    if (!c || !name) return PIC_EINVAL;
+    if (!strcmp(name, "stage_timing")) c->stage_timing = value != 0;
+    else if (!strcmp(name, "force_path")) {
+        if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "force_path must be 0, 1 or 2");
+        c->force_path = (int)value;
+    } else if (!strcmp(name, "yee_tma")) c->yee_tma = value != 0;
+    else return fail(c, PIC_EINVAL, "unknown option '%s'", name);
+    return PIC_OK;
+}
+
+int pic_sync(pic_ctx* c) {
+    if (!c) return PIC_EINVAL;
+    return sync_and_check(c);
+}
+
+const char* pic_last_error(pic_ctx* c) {
+    if (!c) return "NULL context";
+    return c->err;
+}
+
+int pic_destroy(pic_ctx* c) {
+    if (!c) return PIC_EINVAL;
+    if (c->ev_made)
+        for (int k = 0; k < NSTAGE + 2; ++k) cudaEventDestroy(c->ev[k]);
+    delete c;
+    return PIC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,93 @@
+// pic_internal.h -- shared declarations of libpic_b200 (CUDA side only; never
+// seen by the oracle).  Layout of the device arena, the by-value grid
+// descriptor handed to kernels, and the launcher prototypes of each stage.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/pic.h"
+
+namespace pic {
+
+constexpr int NG = PIC_NG;          // guard cells per side
+constexpr int MAX_SPECIES = 8;
+constexpr double C_LIGHT = 299792458.0;       // CODATA 2018 (exact)
+constexpr double EPS0 = 8.8541878128e-12;     // CODATA 2018
+
+// Grid descriptor, passed by value to every kernel.
+struct Grid {
+    int nx, ny, nz;          // interior cells
+    int px, py, pz;          // padded extents: px = pitch (even, >= nx + 2 NG), py = ny + 2 NG, ...
+    long long sy, sz;        // strides in elements: sy = px, sz = px * py
+    long long npad;          // px * py * pz elements per component
+    double dx, dy, dz;
+    double inv_dx, inv_dy, inv_dz;   // 1.0/dx rounded once (reading R30)
+    double xmin, ymin, zmin;
+    double xmax, ymax, zmax;         // xmin + nx*dx
+    double Lx, Ly, Lz;               // nx*dx
+    double dt;
+    __host__ __device__ inline long long idx(int i, int j, int k) const {   // interior cell index -> padded offset
+        return (long long)(i + NG) + sy * (long long)(j + NG) + sz * (long long)(k + NG);
+    }
+};
+
+// Nine field components, padded layout.
+struct Fields {
+    double *Ex, *Ey, *Ez, *Bx, *By, *Bz, *Jx, *Jy, *Jz;
+};
+
+// One SoA particle buffer.
+struct Particles {
+    double *x, *y, *z, *ux, *uy, *uz, *w;
+    unsigned long long* id;
+};
+
+// Device-side flags and counters (one small block in the arena).
+struct DevStatus {
+    int ephys;                 // set by particle kernels: moved >= 1 cell or non-finite
+    int ebox;                  // set by the load validator: outside the box / non-finite
+    unsigned long long n_fast; // counters [0..2] of pic_get_counters
+    unsigned long long n_slow;
+    unsigned long long n_global;
+};
+
+// ---- yee.cu ---------------------------------------------------------------
+void launch_push_B(const Grid& g, const Fields& f, double dth, bool tma, cudaStream_t st);
+void launch_push_E(const Grid& g, const Fields& f, double dt, bool tma, cudaStream_t st);
+void launch_fill_guards(const Grid& g, double* F, cudaStream_t st);       // periodic images of one component
+int yee_num_launches(bool tma);
+
+// ---- particles_global.cu --------------------------------------------------
+// gather + Boris + move + Esirkepov with global fp64 atomics + wrap; any particle order.
+void launch_particles_global(const Grid& g, const Fields& f, const Particles& p, long long n, double q,
+                             double m, int order, DevStatus* status, cudaStream_t st);
+void launch_deposit_rho(const Grid& g, const Particles& p, long long n, double q, int order, double* rho_pad,
+                        cudaStream_t st);
+void launch_fold_guards(const Grid& g, double* F, cudaStream_t st);       // sum periodic images into the interior
+void launch_validate(const Grid& g, const Particles& p, long long n, DevStatus* status, cudaStream_t st);
+void launch_iota(unsigned long long* id, long long n, cudaStream_t st);
+
+// ---- sort.cu ----------------------------------------------------------------
+// scratch: key[n] u32, rank[n] u32, block_sums[...] u32
+struct SortScratch {
+    unsigned int* key;
+    unsigned int* rank;
+    unsigned int* block_sums;
+    long long block_sums_len;
+};
+int launch_sort(const Grid& g, const Particles& src, const Particles& dst, long long n, unsigned int* cell_offset,
+                const SortScratch& sc, cudaStream_t st);   // returns kernels launched
+long long sort_block_sums_len(long long ncell);
+
+// ---- particles_tile.cu ------------------------------------------------------
+// fused gather + push + deposit per cell-sorted tile (shared-memory stencil and J tile).
+struct TileScratch {
+    void* ptr;
+    size_t bytes;
+};
+int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, long long n, double q, double m,
+                          int order, const unsigned int* cell_offset, DevStatus* status, cudaStream_t st);  // kernels launched
+int tile_setup();   // one-time cudaFuncSetAttribute calls; returns cudaError_t as int
+
+}  // namespace pic

@@ -1,0 +1,169 @@
+"""GPU tests of the sort (integer work: bit-exact), of the invariants measured
+on the GPU result itself (continuity, Gauss), of the rho diagnostic, and of the
+error behaviour include/pic.h states.  ``-m gpu``."""
+import numpy as np
+import pytest
+
+from paper_2303_12873_b200 import workloads as W
+
+from parity_util import by_id, make_pair
+
+pytestmark = pytest.mark.gpu
+
+EPS0 = 8.8541878128e-12
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2303_12873_b200 import binding
+    return binding
+
+
+def test_sort_is_a_cell_ordered_permutation_and_offsets_match_oracle(ora, B):
+    wl = W.uniform_plasma(9, 7, 5, ppc=11, u_th=0.1, order=3, seed=31, shuffle=True)
+    o, g = make_pair(ora, B.Sim, wl)
+    before = g.get_particles(0)
+    g.sort()
+    after = g.get_particles(0)
+    # keys non-decreasing (keys computed by the oracle from the GPU's output positions)
+    key = ora.cell_keys(o.g, after["x"], after["y"], after["z"])
+    assert (np.diff(key) >= 0).all()
+    # id multiset unchanged, and every attribute travelled with its id (bit-exact: payload is only moved)
+    a, b = by_id(after), by_id(before)
+    for k in ("x", "y", "z", "ux", "uy", "uz", "w"):
+        assert np.array_equal(a[k], b[k]), k
+    # cell offsets = exclusive prefix of the brute-force histogram = the oracle's
+    o.sort()
+    off = g.get_cell_offsets(0)
+    assert np.array_equal(off.astype(np.int64), o.cell_offset[0])
+    assert np.array_equal(off.astype(np.int64),
+                          np.concatenate([[0], np.cumsum(np.bincount(key, minlength=wl.ncell))]))
+    # sorting twice changes nothing but (possibly) the order inside a cell
+    g.sort()
+    again = g.get_particles(0)
+    assert np.array_equal(ora.cell_keys(o.g, again["x"], again["y"], again["z"]), key)
+    assert g.counters()["sorts"] == 2
+
+
+def test_sort_large_spans_many_scan_chunks(ora, B):
+    wl = W.uniform_plasma(40, 40, 40, ppc=4, u_th=0.05, order=1, seed=37, shuffle=True)   # 64,000 cells > 31 chunks
+    o, g = make_pair(ora, B.Sim, wl)
+    g.sort()
+    p = g.get_particles(0)
+    key = ora.cell_keys(o.g, p["x"], p["y"], p["z"])
+    assert (np.diff(key) >= 0).all()
+    assert np.array_equal(np.sort(p["id"]), np.arange(wl.nparticles, dtype=np.uint64))
+    off = g.get_cell_offsets(0).astype(np.int64)
+    assert np.array_equal(off, np.concatenate([[0], np.cumsum(np.bincount(key, minlength=wl.ncell))]))
+
+
+def _div_back(F, wl):
+    """Backward-difference divergence at nodes of a staggered vector field (periodic)."""
+    sh = (wl.nz, wl.ny, wl.nx)
+    fx, fy, fz = (F[0].reshape(sh), F[1].reshape(sh), F[2].reshape(sh))
+    return ((fx - np.roll(fx, 1, 2)) / wl.dx + (fy - np.roll(fy, 1, 1)) / wl.dy + (fz - np.roll(fz, 1, 0)) / wl.dz)
+
+
+@pytest.mark.parametrize("order", [1, 2, 3])
+def test_gpu_continuity_and_rho_parity(ora, B, order):
+    """(rho^{n+1} - rho^n)/dt + div J = 0 to roundoff on the GPU's own arrays (R20), every order, both paths."""
+    wl = W.uniform_plasma(10, 9, 8, ppc=6, u_th=0.4, order=order, seed=41 + order, dx=0.5e-6, dy=0.4e-6, dz=0.6e-6)
+    for path in (1, 2):
+        o, g = make_pair(ora, B.Sim, wl, sort_first=(path == 2), force_path=path)
+        rho0 = g.deposit_rho(0)
+        assert np.abs(rho0 - o.deposit_rho(0)).max() <= 1e-12 * np.abs(rho0).max()
+        g.step(1)
+        rho1 = g.deposit_rho(0)
+        f = g.get_fields(("Jx", "Jy", "Jz"))
+        res = (rho1 - rho0).reshape(wl.nz, wl.ny, wl.nx) / wl.dt + _div_back((f["Jx"], f["Jy"], f["Jz"]), wl)
+        assert np.abs(res).max() <= 1e-13 * np.abs(rho1).max() / wl.dt, (order, path)
+
+
+def test_gpu_gauss_law_constant_over_100_steps(ora, B):
+    """G = div E - rho/eps0 stays constant in time (R19) -- couples push, wrap, deposit, E update, sort."""
+    wl = W.uniform_plasma(8, 8, 8, ppc=8, u_th=0.05, order=3, seed=43, protons=True)
+    _, g = make_pair(ora, B.Sim, wl, sort_first=True)
+
+    def gauss():
+        f = g.get_fields(("Ex", "Ey", "Ez"))
+        return _div_back((f["Ex"], f["Ey"], f["Ez"]), wl) - g.deposit_rho(-1).reshape(wl.nz, wl.ny, wl.nx) / EPS0
+
+    rho_e = np.abs(g.deposit_rho(0)).max()
+    G0 = gauss()
+    assert np.abs(G0).max() <= 1e-12 * rho_e / EPS0          # co-located pairs: G = 0 at t = 0
+    for it in range(100):
+        if it % 4 == 0:
+            g.sort()
+        g.step(1)
+    assert np.abs(gauss() - G0).max() <= 1e-11 * rho_e / EPS0
+
+
+def test_roundtrip_fields_and_particles_bit_exact(B):
+    wl = W.uniform_plasma(7, 6, 5, ppc=3, u_th=0.1, order=2, seed=47)
+    rng = np.random.default_rng(1)
+    wl.fields = {n: rng.standard_normal(wl.ncell) for n in ("Ex", "Ey", "Ez", "Bx", "By", "Bz")}
+    g = B.Sim.from_workload(wl)
+    f = g.get_fields()
+    for n, a in wl.fields.items():
+        assert np.array_equal(f[n], a), n
+    assert not f["Jx"].any() and not f["Jy"].any() and not f["Jz"].any()
+    p = g.get_particles(0)
+    for k, a in zip(("x", "y", "z", "ux", "uy", "uz", "w"), wl.species[0].arrays()):
+        assert np.array_equal(p[k], a), k
+    assert np.array_equal(p["id"], np.arange(wl.nparticles, dtype=np.uint64))
+    # device-resident round trip
+    fd = g.get_fields(device=True)
+    for n, a in wl.fields.items():
+        assert np.array_equal(fd[n].cpu().numpy(), a), n
+    pd = g.get_particles(0, device=True)
+    assert np.array_equal(pd["uz"].cpu().numpy(), wl.species[0].uz)
+
+
+def test_error_codes(B):
+    d = 0.5e-6
+    dt = W.courant_dt(d, d, d)
+    with pytest.raises(B.PicError) as e:                       # dt above the Courant limit
+        B.Sim(4, 4, 4, d, d, d, 0, 0, 0, dt * 1.02, 1, [8])
+    assert e.value.code == B.PIC_EINVAL
+    with pytest.raises(B.PicError) as e:                       # order 4
+        B.Sim(4, 4, 4, d, d, d, 0, 0, 0, dt, 4, [8])
+    assert e.value.code == B.PIC_EINVAL
+    g = B.Sim(4, 4, 4, d, d, d, 0, 0, 0, dt, 1, [8])
+    with pytest.raises(B.PicError) as e:                       # step before load
+        g.step(1)
+    assert e.value.code == B.PIC_ESTATE
+    with pytest.raises(B.PicError) as e:                       # sort before load
+        g.sort()
+    assert e.value.code == B.PIC_ESTATE
+    one = np.array([1e-6]); zero = np.zeros(1)
+    with pytest.raises(B.PicError) as e:                       # outside the box (x = L exactly)
+        g.load_particles(0, -W.Q_E, W.M_E, np.array([4 * d]), one, one, zero, zero, zero, np.ones(1))
+    assert e.value.code == B.PIC_EINVAL and "outside" in str(e.value)
+    with pytest.raises(B.PicError) as e:                       # NaN
+        g.load_particles(0, -W.Q_E, W.M_E, np.array([np.nan]), one, one, zero, zero, zero, np.ones(1))
+    assert e.value.code == B.PIC_EINVAL
+    with pytest.raises(B.PicError) as e:                       # more than np_max
+        z9 = np.full(9, 1e-6)
+        g.load_particles(0, -W.Q_E, W.M_E, z9, z9, z9, z9 * 0, z9 * 0, z9 * 0, z9)
+    assert e.value.code == B.PIC_ENOMEM
+    with pytest.raises(B.PicError) as e:
+        g.load_particles(3, -W.Q_E, W.M_E, one, one, one, zero, zero, zero, np.ones(1))
+    assert e.value.code == B.PIC_EINVAL
+    with pytest.raises(B.PicError) as e:
+        g.set_option("no_such_option", 1)
+    assert e.value.code == B.PIC_EINVAL
+    g.load_particles(0, -W.Q_E, W.M_E, one, one, one, zero, zero, zero, np.ones(1))
+    with pytest.raises(B.PicError) as e:                       # fused path forced without a sort
+        g.set_option("force_path", 2)
+        g.step(1)
+    assert e.value.code == B.PIC_ESTATE
+    g.set_option("force_path", 0)
+    g.step(1)
+    g.sync()
+    assert g.counters()["steps"] == 1
+    # an infinite field makes the new position non-finite during the step -> PIC_EPHYS at the next sync
+    g.set_fields(Ex=np.full(64, np.inf))
+    g.step(1)
+    with pytest.raises(B.PicError) as e:
+        g.sync()
+    assert e.value.code == B.PIC_EPHYS
