@@ -1,0 +1,173 @@
+// particle_update.cuh -- device code shared by the two particle kernels (CUDA
+// path only): gather of one component from the padded global arrays, the
+// general Esirkepov deposition of one particle through an "adder" (global
+// fp64 atomics, or the fused kernel's shared-memory tile), and the complete
+// order-independent update of one particle against the GLOBAL arrays.
+// Follows SURVEY 8(c.1) steps 1-5 (BASELINE.json:north_star parts 1-3).
+#pragma once
+#include "shapes.cuh"
+
+namespace pic {
+
+// ---------------------------------------------------------------- gather ----
+// One component: sum over the (N+1)^3 support, factored z(y(x)).
+template <int N>
+__device__ __forceinline__ double gather_comp(const double* __restrict__ F, const Grid& g, int fx, int fy, int fz,
+                                              const double (&wx)[N + 1], const double (&wy)[N + 1],
+                                              const double (&wz)[N + 1]) {
+    const double* base = F + g.idx(fx, fy, fz);
+    double acc = 0.0;
+#pragma unroll
+    for (int c = 0; c <= N; ++c) {
+        double accy = 0.0;
+#pragma unroll
+        for (int b = 0; b <= N; ++b) {
+            const double* row = base + b * g.sy + c * g.sz;
+            double accx = 0.0;
+#pragma unroll
+            for (int a = 0; a <= N; ++a) accx = fma(wx[a], __ldg(row + a), accx);
+            accy = fma(wy[b], accx, accy);
+        }
+        acc = fma(wz[c], accy, acc);
+    }
+    return acc;
+}
+
+// Esirkepov deposition of one particle through an adder:
+//   Jx[i+1/2,j,k] += cx * sum_{i'<=i} DSx[i'] (S0y[j] S0z[k] + DSy[j] S0z[k]/2 + S0y[j] DSz[k]/2 + DSy[j] DSz[k]/3)
+// written as cx * PDx[i] * (S0z[k] Ay[j] + DSz[k] By[j]),  A = S0 + DS/2,  B = S0/2 + DS/3.
+// add(comp, ix, iy, iz, v) receives NODE indices (ix may be -2 .. nx+2) and must be atomic.
+// Zero contributions are skipped, so only the (N+1)(N+2)^2 live points cost an atomic.
+template <int N, class Adder>
+__device__ __forceinline__ void deposit_esirkepov(const Grid& g, double xi0, double et0, double ze0, double xi1,
+                                                  double et1, double ze1, double qw, bool& bad, Adder add) {
+    constexpr int W = N + 3;
+    double s0x[W], dsx[W], s0y[W], dsy[W], s0z[W], dsz[W];
+    const int nx0 = esirkepov_shapes<N>(xi0, xi1, s0x, dsx, bad);
+    const int ny0 = esirkepov_shapes<N>(et0, et1, s0y, dsy, bad);
+    const int nz0 = esirkepov_shapes<N>(ze0, ze1, s0z, dsz, bad);
+    if (bad) return;
+    const double inv_dt = 1.0 / g.dt;
+    const double cx = -qw * inv_dt * g.inv_dy * g.inv_dz;
+    const double cy = -qw * inv_dt * g.inv_dx * g.inv_dz;
+    const double cz = -qw * inv_dt * g.inv_dx * g.inv_dy;
+    // Jx
+    {
+        double pd[W];
+        double acc = 0.0;
+#pragma unroll
+        for (int a = 0; a < W; ++a) { acc += dsx[a]; pd[a] = cx * acc; }
+#pragma unroll
+        for (int c = 0; c < W; ++c)
+#pragma unroll
+            for (int b = 0; b < W; ++b) {
+                double t = s0z[c] * (s0y[b] + 0.5 * dsy[b]) + dsz[c] * (0.5 * s0y[b] + (1.0 / 3.0) * dsy[b]);
+                if (t != 0.0) {
+#pragma unroll
+                    for (int a = 0; a < W - 1; ++a) {
+                        double v = pd[a] * t;
+                        if (v != 0.0) add(0, nx0 + a, ny0 + b, nz0 + c, v);
+                    }
+                }
+            }
+    }
+    // Jy
+    {
+        double pd[W];
+        double acc = 0.0;
+#pragma unroll
+        for (int b = 0; b < W; ++b) { acc += dsy[b]; pd[b] = cy * acc; }
+#pragma unroll
+        for (int c = 0; c < W; ++c)
+#pragma unroll
+            for (int a = 0; a < W; ++a) {
+                double t = s0x[a] * (s0z[c] + 0.5 * dsz[c]) + dsx[a] * (0.5 * s0z[c] + (1.0 / 3.0) * dsz[c]);
+                if (t != 0.0) {
+#pragma unroll
+                    for (int b = 0; b < W - 1; ++b) {
+                        double v = pd[b] * t;
+                        if (v != 0.0) add(1, nx0 + a, ny0 + b, nz0 + c, v);
+                    }
+                }
+            }
+    }
+    // Jz
+    {
+        double pd[W];
+        double acc = 0.0;
+#pragma unroll
+        for (int c = 0; c < W; ++c) { acc += dsz[c]; pd[c] = cz * acc; }
+#pragma unroll
+        for (int b = 0; b < W; ++b)
+#pragma unroll
+            for (int a = 0; a < W; ++a) {
+                double t = s0y[b] * (s0x[a] + 0.5 * dsx[a]) + dsy[b] * (0.5 * s0x[a] + (1.0 / 3.0) * dsx[a]);
+                if (t != 0.0) {
+#pragma unroll
+                    for (int c = 0; c < W - 1; ++c) {
+                        double v = pd[c] * t;
+                        if (v != 0.0) add(2, nx0 + a, ny0 + b, nz0 + c, v);
+                    }
+                }
+            }
+    }
+}
+
+// Adder onto the padded global J arrays: one REDG.E.ADD.F64 per live point.
+struct GlobalAdder {
+    double* J[3];
+    long long sy, sz;
+    __device__ __forceinline__ void operator()(int comp, int ix, int iy, int iz, double v) const {
+        atomicAdd(J[comp] + ((long long)(ix + NG) + sy * (long long)(iy + NG) + sz * (long long)(iz + NG)), v);
+    }
+};
+
+template <int N>
+__device__ __forceinline__ void deposit_global(const Grid& g, const Fields& f, double xi0, double et0, double ze0,
+                                               double xi1, double et1, double ze1, double qw, bool& bad) {
+    GlobalAdder add{{f.Jx, f.Jy, f.Jz}, g.sy, g.sz};
+    deposit_esirkepov<N>(g, xi0, et0, ze0, xi1, et1, ze1, qw, bad, add);
+}
+
+// Device function used by both particle paths: the whole update of one
+// particle against the GLOBAL field arrays.
+template <int N>
+__device__ __forceinline__ void update_particle_global(const Grid& g, const Fields& f, const Particles& p,
+                                                       long long ip, double q, double h, DevStatus* status) {
+    const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
+    double ux = p.ux[ip], uy = p.uy[ip], uz = p.uz[ip];
+    const double w = p.w[ip];
+    // normalised coordinates: a subtraction then a multiplication (R30)
+    const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy, ze = (z - g.zmin) * g.inv_dz;
+    // step 1: gather
+    double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[N + 1], wys[N + 1], wzs[N + 1];
+    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn), fzn = shape_weights<N>(ze, wzn);
+    const int fxs = shape_weights<N>(xi - 0.5, wxs), fys = shape_weights<N>(et - 0.5, wys),
+              fzs = shape_weights<N>(ze - 0.5, wzs);
+    const double ex = gather_comp<N>(f.Ex, g, fxs, fyn, fzn, wxs, wyn, wzn);
+    const double ey = gather_comp<N>(f.Ey, g, fxn, fys, fzn, wxn, wys, wzn);
+    const double ez = gather_comp<N>(f.Ez, g, fxn, fyn, fzs, wxn, wyn, wzs);
+    const double bx = gather_comp<N>(f.Bx, g, fxn, fys, fzs, wxn, wys, wzs);
+    const double by = gather_comp<N>(f.By, g, fxs, fyn, fzs, wxs, wyn, wzs);
+    const double bz = gather_comp<N>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
+    // step 2: Boris
+    const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
+    boris_push(h, inv_c2, ux, uy, uz, ex, ey, ez, bx, by, bz);
+    // step 3: move (unwrapped)
+    const double gam = sqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
+    const double x1 = x + g.dt * ux / gam, y1 = y + g.dt * uy / gam, z1 = z + g.dt * uz / gam;
+    // step 4: deposit from (x^n, x~^{n+1})
+    const double xi1 = (x1 - g.xmin) * g.inv_dx, et1 = (y1 - g.ymin) * g.inv_dy, ze1 = (z1 - g.zmin) * g.inv_dz;
+    bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1));
+    if (!bad && q != 0.0) deposit_global<N>(g, f, xi, et, ze, xi1, et1, ze1, q * w, bad);
+    if (bad) status->ephys = 1;
+    // step 5: wrap and store
+    p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
+    p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
+    p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
+    p.ux[ip] = ux;
+    p.uy[ip] = uy;
+    p.uz[ip] = uz;
+}
+
+}  // namespace pic
