@@ -1,0 +1,365 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole PIC hot path on B200 (driver contract).
+
+A "step" is one pass of every row of SURVEY.md 8(a): zero J, fused
+gather + Boris push + Esirkepov deposition (all species), J guard fold, Yee
+B half / E / B half, with the per-cell counting sort run every
+``sort_every`` steps INSIDE the timed region (so its cost is amortised into
+the step time).  N = 1 workload: BASELINE.json configs[2] (256^3 cells, 8 ppc
+electrons = 134,217,728 particles, order 3, u_th = 0.05 c) -- the
+configuration BASELINE.json:north_star quotes its target on; it fits one GPU
+(about 19 GB of arena).  N > 1: independent replicas of that workload, one per
+GPU (replicas only, no data-path collective).
+
+  value     particle-updates/s of the whole step, inputs resident in HBM
+  e2e       the same metric through the C ABI with HOST buffers: every step
+            pic_load_particles (H2D) + pic_sort + pic_step + pic_get_particles
+            and pic_get_fields (D2H) from/to pinned host memory
+  roofline  the dominant kernel (fused per-tile particle kernel): algorithmic
+            bytes per launch / its average launch duration, measured with CUDA
+            events on the library's stream over the timed region
+  cpu_baseline   the oracle (oracle/, as it stands) timed on the host cores on
+            a bounded sample of the same workload
+
+``--impl reference`` times the oracle alone (this tier's reference arm).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle-updates/sec (gather+push+deposit, fp64) and Yee cell-updates/sec on 1 B200"
+UNIT = "particle-updates/s"
+
+# Algorithmic HBM bytes of the fused particle kernel:
+# per particle read x,y,z,ux,uy,uz,w (56 B) + write x,y,z,ux,uy,uz (48 B); per cell read the
+# six E,B values (48 B) and read-modify-write the three J values (48 B).
+BYTES_PER_PARTICLE = 104.0
+BYTES_PER_CELL = 96.0
+# Yee: B half (72 B/cell) + E (96 B/cell) + B half (72 B/cell)
+YEE_BYTES_PER_CELL = 240.0
+
+
+def _peaks():
+    """(HBM GB/s, 'measured'|'fallback') from MEASURED_PEAKS.json, else the guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured"
+    except Exception:
+        return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.fh = open(self.path, "w")
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=self.fh, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.fh.close()
+        sm, mx, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        with open(self.path) as fh:
+            for line in fh:
+                p = [t.strip() for t in line.split(",")]
+                if len(p) < 7:
+                    continue
+                try:
+                    sm.append(float(p[0])); mx.append(float(p[1])); power.append(float(p[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, p[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+        os.unlink(self.path)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), power_w_max=max(power),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# --------------------------------------------------------------------------- oracle legs
+def _oracle_sample(index: int):
+    """The bounded sample of configs[index] the oracle is timed on (last column)."""
+    from paper_2303_12873_b200 import workloads as W
+    # configs 1-2: a 16^3 crop (same ppc, u_th, order, dx, dt) keeps one oracle step under a second
+    wl = W.config(index, parity=True, **({"n": 16} if index in (1, 2) else {}))
+    desc = "%s: %dx%dx%d cells, %d particles, order %d (crop of configs[%d], same ppc/u_th/order/dx/dt)" % (
+        wl.name, wl.nx, wl.ny, wl.nz, wl.nparticles, wl.order, index)
+    return wl, desc
+
+
+def _oracle_sim(wl):
+    from oracle import ora
+    o = ora.OracleSim(*wl.grid_args(), wl.dt, wl.order, len(wl.species))
+    if wl.fields:
+        o.set_fields(**wl.fields)
+    for s, sp in enumerate(wl.species):
+        o.load_particles(s, sp.q, sp.m, *sp.arrays())
+    return o
+
+
+def time_oracle(index: int, budget_s: float = 12.0, max_steps: int = 40):
+    """particle-updates/s of the oracle as it stands, single-threaded, on the host."""
+    wl, desc = _oracle_sample(index)
+    o = _oracle_sim(wl)
+    o.step(1)                                   # warm-up (page in, build tables)
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_steps and (n < 2 or time.perf_counter() - t0 < budget_s):
+        o.step(1)
+        n += 1
+    dt = time.perf_counter() - t0
+    return {"value": wl.nparticles * n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "%s, %d steps in %.1f s" % (desc, n, dt),
+            "cell_updates_per_s": wl.ncell * n / dt}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, K steps of a bounded sample after W warm-ups."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl, desc = _oracle_sample(args.config)
+    o = _oracle_sim(wl)
+    for _ in range(args.warmup):
+        o.step(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(1)
+    dt = time.perf_counter() - t0
+    val = wl.nparticles * args.steps / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": "configs[%d]" % args.config, "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------- GPU leg
+def _pinned_copy(torch, a):
+    t = torch.empty(a.shape, dtype=torch.float64, pin_memory=True)
+    t.numpy()[...] = a
+    return t
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_2303_12873_b200 import workloads as W
+    from paper_2303_12873_b200.binding import Sim      # raises if libpic_b200.so is missing: no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # ---- workload: configs[index], one replica per rank (seed offset by rank) ----
+    t_gen = time.perf_counter()
+    kw = {}
+    if args.n is not None:
+        kw["n"] = args.n
+    wl = W.config(args.config, parity=False, **kw)
+    if rank:
+        for sp in wl.species:       # replicas differ only by a cyclic shift of the particle momenta
+            for nm in ("ux", "uy", "uz"):
+                setattr(sp, nm, np.roll(getattr(sp, nm), 8 * rank))
+    sort_every = wl.sort_every if wl.sort_every > 0 else 0
+    t_gen = time.perf_counter() - t_gen
+    npart, ncell = wl.nparticles, wl.ncell
+
+    sim = Sim.from_workload(wl, device="cuda:%d" % local)
+    sim.sort()
+    sim.sync()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def run_steps(k, first_index):
+        for it in range(k):
+            if sort_every and (first_index + it) % sort_every == 0 and (first_index + it) > 0:
+                sim.sort()
+            sim.step(1)
+
+    # ---- device-resident timing: W warm-ups, then exactly K steps ----
+    run_steps(args.warmup, 0)
+    sim.sync()
+    sim.set_option("stage_timing", 1)
+    c0 = sim.counters()
+    clocks = ClockSampler(local)
+    clocks.start()
+    barrier()
+    ev0 = torch.cuda.Event(enable_timing=True)
+    ev1 = torch.cuda.Event(enable_timing=True)
+    ev0.record(sim.stream)
+    run_steps(args.steps, args.warmup)
+    ev1.record(sim.stream)
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    clk = clocks.stop()
+    st = sim.stage_ms()
+    sim.set_option("stage_timing", 0)
+    c1 = sim.counters()
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * npart * args.steps / (ms_total * 1e-3)
+
+    # ---- roofline of the dominant kernel (fused particle kernel, one launch per species per step) ----
+    nspec = sum(1 for s in wl.species if s.n > 0)
+    n_launch = max(1, int(round(st["steps"])) * nspec)
+    ms_launch = st["particles"] / n_launch
+    alg_bytes = (BYTES_PER_PARTICLE * npart + BYTES_PER_CELL * ncell * nspec) / nspec
+    peak, peak_kind = _peaks()
+    achieved = alg_bytes / (ms_launch * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "particles_tile_kernel<%d>" % wl.order, "achieved": achieved,
+                "peak": peak, "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured"
+                else "fallback (B200_PROFILING.md)", "unit": "GB/s", "frac": achieved / peak,
+                "traffic": args.traffic, "ms_per_launch": ms_launch,
+                "algorithmic_bytes_per_launch": alg_bytes,
+                "particle_updates_per_s_kernel_only": npart / nspec / (ms_launch * 1e-3)}
+    nsteps_t = max(1.0, st["steps"])
+    yee_ms = (st["yee_B"] + st["yee_E"]) / nsteps_t
+    stages = {"per_step_ms": {k: st[k] / nsteps_t for k in ("zero_J", "particles", "fold_J", "yee_B", "yee_E")},
+              "sort_ms_each": (st["sort"] / st["sorts"]) if st["sorts"] else None,
+              "sorts_in_timed_region": int(st["sorts"]),
+              "yee_cell_updates_per_s": ncell / (yee_ms * 1e-3) if yee_ms > 0 else None,
+              "yee_gbs": YEE_BYTES_PER_CELL * ncell / (yee_ms * 1e-3) / 1e9 if yee_ms > 0 else None}
+    paths = {k: c1[k] - c0[k] for k in ("fast", "slow", "global")}
+
+    # ---- end to end through the C ABI with pinned HOST buffers (rank-local; max over ranks) ----
+    e2e = None
+    if args.e2e_steps > 0:
+        host_in = [[_pinned_copy(torch, a) for a in sp.arrays()] for sp in wl.species]
+        host_out = [{nm: torch.empty(sp.n, dtype=torch.float64, pin_memory=True)
+                     for nm in ("x", "y", "z", "ux", "uy", "uz")} for sp in wl.species]
+        fld_out = {nm: torch.empty(ncell, dtype=torch.float64, pin_memory=True) for nm in Sim.FIELD_NAMES}
+        h2d = sum(7 * 8 * sp.n for sp in wl.species)
+        d2h = sum(6 * 8 * sp.n for sp in wl.species) + 9 * 8 * ncell
+        del sim
+        torch.cuda.empty_cache()
+        sim = Sim.from_workload(wl, device="cuda:%d" % local, load=False)
+        if wl.fields:
+            sim.set_fields(**wl.fields)
+
+        def e2e_step():
+            for s, sp in enumerate(wl.species):
+                sim.load_particles(s, sp.q, sp.m, *host_in[s])
+            sim.sort()
+            sim.step(1)
+            for s in range(len(wl.species)):
+                sim.get_particles_into(s, host_out[s])
+            sim.get_fields_into(fld_out)
+
+        e2e_step()                                   # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        barrier()
+        dt_e = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt_e], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt_e = float(t.item())
+        e2e = {"value": world * npart * args.e2e_steps / dt_e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": args.e2e_steps, "ms_per_step": 1e3 * dt_e / args.e2e_steps,
+               "what": "pic_load_particles(host) + pic_sort + pic_step(1) + pic_get_particles(host) + "
+                       "pic_get_fields(host), pinned buffers, wall clock around synchronising calls"}
+
+    # ---- the oracle beside it (rank 0, N = 1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = time_oracle(args.config)
+
+    if dist is not None:
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[%d]" % args.config, "name": wl.name,
+                       "grid": [wl.nx, wl.ny, wl.nz], "particles": npart, "species": len(wl.species),
+                       "order": wl.order, "sort_every": sort_every, "replicas": world,
+                       "l2": "inputs larger than L2 (%.1f GB of particles + fields per step)" % (
+                           (BYTES_PER_PARTICLE * npart + 9 * 8 * ncell) / 1e9),
+                       "generation_s": round(t_gen, 1)},
+            "cell_updates_per_s": world * ncell * args.steps / (ms_total * 1e-3),
+            "roofline": roofline, "stages": stages, "particle_paths": paths,
+            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(c1["launches"] - c0["launches"]),
+            "clocks": clk}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=4)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: 256^3 x 8 ppc)")
+    ap.add_argument("--n", type=int, default=None, help="override the cube edge of configs 0-2 (debugging)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="DRAM bytes per launch of the dominant kernel from the committed ncu capture")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

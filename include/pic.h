@@ -68,6 +68,9 @@ enum {
 /* Number of entries written by pic_get_counters. */
 #define PIC_NCOUNTERS 8
 
+/* Number of entries written by pic_get_stage_ms. */
+#define PIC_NSTAGES 8
+
 /*
  * Bytes of device arena pic_init_grid needs.  Pure function of its arguments
  * (no CUDA call).  np_max[s] = capacity of species s (particles); the library
@@ -188,11 +191,16 @@ int pic_get_cell_offsets(pic_ctx*, int species, unsigned int* offsets, int dst_o
 int pic_get_counters(pic_ctx*, unsigned long long* counters /*host*/);
 
 /*
- * Per-stage device time of the LAST pic_step call when stage timing is on
- * (pic_set_option("stage_timing",1)): milliseconds summed over that call's
- * steps for  [0] zero J  [1] particles (gather+push+deposit, all species)
- * [2] J guard fold  [3] Yee B (both halves, incl. guards)  [4] Yee E (incl.
- * guards).  Host array of 5 floats.  Synchronises.  PIC_ESTATE if off.
+ * Per-stage device time, in milliseconds, summed over every pic_step iteration
+ * and every pic_sort issued since stage timing was switched on
+ * (pic_set_option("stage_timing",1)) or since the previous pic_get_stage_ms,
+ * whichever is later.  CUDA events are recorded on the context's stream around
+ * each stage; pic_step / pic_sort never wait on them, so timing does not
+ * serialise the host with the device.  Host array of PIC_NSTAGES floats:
+ *   [0] zero J   [1] particles (gather+push+deposit, all species)
+ *   [2] J guard fold   [3] Yee B (both half pushes)   [4] Yee E
+ *   [5] sort (all species)   [6] step iterations summed   [7] sorts summed
+ * Synchronises and resets the sums.  PIC_ESTATE if stage timing is off.
  */
 int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
 

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libpic_b200.so")
 
 PIC_OK, PIC_EINVAL, PIC_ENOMEM, PIC_ECUDA, PIC_ESTATE, PIC_EPHYS = 0, -1, -2, -3, -4, -5
 PIC_NCOUNTERS = 8
+PIC_NSTAGES = 8
 _CODE_NAMES = {0: "PIC_OK", -1: "PIC_EINVAL", -2: "PIC_ENOMEM", -3: "PIC_ECUDA", -4: "PIC_ESTATE",
                -5: "PIC_EPHYS"}
 
@@ -235,6 +236,23 @@ class Sim:
                     "pic_get_particles")
         return out
 
+    def get_fields_into(self, out):
+        """pic_get_fields into caller buffers: dict name -> contiguous float64 buffer of ncell entries
+        (numpy / pinned torch CPU tensors = host, torch.cuda tensors = device); missing names are skipped."""
+        dev = _on_device(out.values())
+        ptrs = [_ptr(out.get(nm), np.float64, dev) for nm in self.FIELD_NAMES]
+        self._check(self._L.pic_get_fields(self._ctx, *ptrs, int(dev)), "pic_get_fields")
+
+    def get_particles_into(self, species, out):
+        """pic_get_particles into caller buffers: dict with any of x,y,z,ux,uy,uz,w (float64) and id (uint64/int64)."""
+        dev = _on_device(out.values())
+        nn = C.c_longlong(0)
+        ptrs = [_ptr(out.get(nm), np.float64, dev) for nm in ("x", "y", "z", "ux", "uy", "uz", "w")]
+        ptrs.append(_ptr(out.get("id"), np.uint64, dev))
+        self._check(self._L.pic_get_particles(self._ctx, species, C.byref(nn), *ptrs, int(dev)),
+                    "pic_get_particles")
+        return int(nn.value)
+
     def deposit_rho(self, species=-1, device=False):
         t = self._torch
         rho = t.empty(self.ncell, dtype=t.float64, device=self.device) if device else np.empty(self.ncell)
@@ -258,9 +276,9 @@ class Sim:
         self._check(self._L.pic_set_option(self._ctx, name.encode(), int(value)), "pic_set_option")
 
     def stage_ms(self):
-        arr = (C.c_float * 5)()
+        arr = (C.c_float * PIC_NSTAGES)()
         self._check(self._L.pic_get_stage_ms(self._ctx, arr), "pic_get_stage_ms")
-        return dict(zip(("zero_J", "particles", "fold_J", "yee_B", "yee_E"), list(arr)))
+        return dict(zip(("zero_J", "particles", "fold_J", "yee_B", "yee_E", "sort", "steps", "sorts"), list(arr)))
 
     def last_error(self) -> str:
         return (self._L.pic_last_error(self._ctx) or b"").decode()

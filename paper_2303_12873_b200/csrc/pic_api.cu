@@ -7,6 +7,7 @@
 #include <string.h>
 
 #include <new>
+#include <vector>
 
 #include "pic_internal.h"
 
@@ -25,7 +26,14 @@ struct Species {
     unsigned int* cell_offset = nullptr;
 };
 
-constexpr int NSTAGE = 5;
+constexpr int NSTAGE = PIC_NSTAGES;
+constexpr int EV_PER_STEP = 7, EV_PER_SORT = 2;
+
+// one timed pic_step iteration (7 consecutive events) or one timed pic_sort (2 events)
+struct TimedSpan {
+    size_t first;
+    int kind;   // 0 = step, 1 = sort
+};
 
 }  // namespace
 
@@ -43,10 +51,9 @@ struct pic_ctx {
     unsigned long long launches = 0, steps = 0, sorts = 0;
     // options
     int stage_timing = 0, force_path = 0, yee_tma = 1;
-    cudaEvent_t ev[NSTAGE + 2] = {};
-    bool ev_made = false;
-    float stage_ms[NSTAGE] = {};
-    bool stage_valid = false;
+    std::vector<cudaEvent_t> ev_pool;   // grows on demand; never waited on inside pic_step / pic_sort
+    size_t ev_used = 0;
+    std::vector<TimedSpan> spans;
 };
 
 namespace {
@@ -184,6 +191,18 @@ int sync_and_check(pic_ctx* c) {
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
     return poll_status(c);
+}
+
+// n consecutive events from the pool (created on first use); returns the index of the first
+bool take_events(pic_ctx* c, int n, size_t* first) {
+    while (c->ev_pool.size() < c->ev_used + (size_t)n) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return false;
+        c->ev_pool.push_back(e);
+    }
+    *first = c->ev_used;
+    c->ev_used += (size_t)n;
+    return true;
 }
 
 bool use_tile_path(const pic_ctx* c, const Species& s) {
@@ -335,24 +354,23 @@ int pic_step(pic_ctx* c, int nsteps) {
             if (c->sp[s].loaded && !c->sp[s].sorted)
                 return fail(c, PIC_ESTATE, "force_path=2 needs pic_sort before pic_step (species %d)", s);
     const bool timing = c->stage_timing != 0;
-    if (timing && !c->ev_made) {
-        for (int k = 0; k < NSTAGE + 2; ++k) CU(c, cudaEventCreate(&c->ev[k]));
-        c->ev_made = true;
-    }
-    if (timing) {
-        for (int k = 0; k < NSTAGE; ++k) c->stage_ms[k] = 0.f;
-        c->stage_valid = false;
-    }
     const Grid& g = c->g;
     const size_t comp_bytes = (size_t)g.npad * sizeof(double);
     const bool tma = c->yee_tma != 0;
     for (int it = 0; it < nsteps; ++it) {
-        if (timing) cudaEventRecord(c->ev[0], c->stream);
+        cudaEvent_t* ev = nullptr;
+        if (timing) {
+            size_t first;
+            if (!take_events(c, EV_PER_STEP, &first)) return fail(c, PIC_ECUDA, "cudaEventCreate failed");
+            c->spans.push_back(TimedSpan{first, 0});
+            ev = c->ev_pool.data() + first;
+            cudaEventRecord(ev[0], c->stream);
+        }
         // J := 0 (R13).  Jx,Jy,Jz are contiguous in the arena.
         CU(c, cudaMemsetAsync(c->f.Jx, 0, comp_bytes, c->stream));
         CU(c, cudaMemsetAsync(c->f.Jy, 0, comp_bytes, c->stream));
         CU(c, cudaMemsetAsync(c->f.Jz, 0, comp_bytes, c->stream));
-        if (timing) cudaEventRecord(c->ev[1], c->stream);
+        if (timing) cudaEventRecord(ev[1], c->stream);
         // steps 1-5 per species, in index order (R37)
         for (int s = 0; s < c->nspecies; ++s) {
             Species& S = c->sp[s];
@@ -367,33 +385,22 @@ int pic_step(pic_ctx* c, int nsteps) {
             }
             S.steps_since_sort += 1;
         }
-        if (timing) cudaEventRecord(c->ev[2], c->stream);
+        if (timing) cudaEventRecord(ev[2], c->stream);
         // periodic fold of the J guard cells into the interior
         launch_fold_guards(g, c->f.Jx, c->stream);
         launch_fold_guards(g, c->f.Jy, c->stream);
         launch_fold_guards(g, c->f.Jz, c->stream);
         c->launches += 3;
-        if (timing) cudaEventRecord(c->ev[3], c->stream);
+        if (timing) cudaEventRecord(ev[3], c->stream);
         // steps 6-8
         launch_push_B(g, c->f, 0.5 * g.dt, tma, c->stream);
-        if (timing) cudaEventRecord(c->ev[4], c->stream);
+        if (timing) cudaEventRecord(ev[4], c->stream);
         launch_push_E(g, c->f, g.dt, tma, c->stream);
-        if (timing) cudaEventRecord(c->ev[5], c->stream);
+        if (timing) cudaEventRecord(ev[5], c->stream);
         launch_push_B(g, c->f, 0.5 * g.dt, tma, c->stream);
         c->launches += 3 * yee_num_launches(tma);
         c->steps += 1;
-        if (timing) {
-            CU(c, cudaEventRecord(c->ev[6], c->stream));
-            CU(c, cudaEventSynchronize(c->ev[6]));
-            float t[6];
-            for (int k = 0; k < 6; ++k) cudaEventElapsedTime(&t[k], c->ev[k], c->ev[k + 1]);
-            c->stage_ms[0] += t[0];
-            c->stage_ms[1] += t[1];
-            c->stage_ms[2] += t[2];
-            c->stage_ms[3] += t[3] + t[5];
-            c->stage_ms[4] += t[4];
-            c->stage_valid = true;
-        }
+        if (timing) cudaEventRecord(ev[6], c->stream);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_step launch");
@@ -406,6 +413,14 @@ int pic_sort(pic_ctx* c) {
     bool any = false;
     for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
     if (!any) return fail(c, PIC_ESTATE, "pic_sort before any pic_load_particles");
+    cudaEvent_t* ev = nullptr;
+    if (c->stage_timing) {
+        size_t first;
+        if (!take_events(c, EV_PER_SORT, &first)) return fail(c, PIC_ECUDA, "cudaEventCreate failed");
+        c->spans.push_back(TimedSpan{first, 1});
+        ev = c->ev_pool.data() + first;
+        cudaEventRecord(ev[0], c->stream);
+    }
     for (int s = 0; s < c->nspecies; ++s) {
         Species& S = c->sp[s];
         if (!S.loaded) continue;
@@ -415,6 +430,7 @@ int pic_sort(pic_ctx* c) {
         S.sorted = true;
         S.steps_since_sort = 0;
     }
+    if (ev) cudaEventRecord(ev[1], c->stream);
     c->sorts += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_sort launch");
@@ -513,14 +529,39 @@ int pic_get_counters(pic_ctx* c, unsigned long long* counters) {
 
 int pic_get_stage_ms(pic_ctx* c, float* ms) {
     if (!c || !ms) return PIC_EINVAL;
-    if (!c->stage_timing || !c->stage_valid) return fail(c, PIC_ESTATE, "stage timing is off or no step was timed");
-    for (int k = 0; k < NSTAGE; ++k) ms[k] = c->stage_ms[k];
+    if (!c->stage_timing) return fail(c, PIC_ESTATE, "stage timing is off");
+    CU(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < NSTAGE; ++k) ms[k] = 0.f;
+    for (const TimedSpan& sp : c->spans) {
+        const cudaEvent_t* ev = c->ev_pool.data() + sp.first;
+        float t = 0.f;
+        if (sp.kind == 0) {
+            // spans between the 7 events: zero J, particles, fold, B half, E, B half
+            static const int stage_of[6] = {0, 1, 2, 3, 4, 3};
+            for (int k = 0; k < 6; ++k) {
+                CU(c, cudaEventElapsedTime(&t, ev[k], ev[k + 1]));
+                ms[stage_of[k]] += t;
+            }
+            ms[6] += 1.f;
+        } else {
+            CU(c, cudaEventElapsedTime(&t, ev[0], ev[1]));
+            ms[5] += t;
+            ms[7] += 1.f;
+        }
+    }
+    c->spans.clear();
+    c->ev_used = 0;
     return PIC_OK;
 }
 
 int pic_set_option(pic_ctx* c, const char* name, long long value) {
     if (!c || !name) return PIC_EINVAL;
-    if (!strcmp(name, "stage_timing")) c->stage_timing = value != 0;
+    if (!strcmp(name, "stage_timing")) {
+        if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail(c, PIC_ECUDA, "cudaStreamSynchronize");
+        c->stage_timing = value != 0;
+        c->spans.clear();
+        c->ev_used = 0;
+    }
     else if (!strcmp(name, "force_path")) {
         if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "force_path must be 0, 1 or 2");
         c->force_path = (int)value;
@@ -541,8 +582,7 @@ const char* pic_last_error(pic_ctx* c) {
 
 int pic_destroy(pic_ctx* c) {
     if (!c) return PIC_EINVAL;
-    if (c->ev_made)
-        for (int k = 0; k < NSTAGE + 2; ++k) cudaEventDestroy(c->ev[k]);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PIC_OK;
 }
