@@ -1,53 +1,64 @@
 // particles_tile.cu -- fused gather + Boris push + Esirkepov deposition per
 // cell-sorted tile (BASELINE.json:north_star parts
-// 1-3, "fused per cell-sorted tile").
+// 1-3, "fused per cell-sorted tile").  Kernel v2.
 //
-// One thread block owns a tile of TX x TY x TZ cells and the particles the last
-// pic_sort listed in those cells (TY*TZ contiguous segments of the SoA arrays).
-//   load    the tile's E,B stencil (+ halo for the shape support and D cells of
-//           drift since the last sort) goes to shared memory; the J tile is zeroed
-//   phase A particle-major, coalesced: thread <-> particle in container order.
-//           Gather from the shared stencil (lanes of a warp sit in the same few
-//           cells: broadcast LDS), Boris, move, coalesced store of the wrapped
-//           state; (xi0,xi1,q*w) goes to a shared staging buffer.
-//   phase B cell-major: lane <-> cell, so the 32 lanes of a warp deposit into 32
-//           DIFFERENT windows and every shared-memory add of a warp instruction
-//           hits 32 distinct addresses.  (fp64 atomicAdd on shared memory is a
-//           CAS loop on sm_100a -- ATOMS.CAST.SPIN -- which costs 8.5 clk per warp
-//           op with distinct addresses but 58 clk when 8 lanes share one; the
-//           particle-major mapping of a sorted species would be the second case.)
-//   flush   one global fp64 atomic (REDG.E.ADD.F64) per non-zero tile point.
-// A particle whose cell left the tile's halo (drift > D cells, periodic wrap far
-// from the tile) takes the global-memory update of particle_update.cuh instead:
-// the kernel is correct for any particle order, only slower.
+// One thread block owns a tile of TX x TY x TZ cells; its E,B stencil (+ halo
+// for the shape support and DRIFT cells of drift since the last pic_sort) is
+// staged in shared memory once.  After that the block's warps run without any
+// block-wide barrier: a warp pulls x-rows of the tile (TX cells, contiguous in
+// the cell-sorted SoA arrays) from a shared counter and processes each row in
+// chunks of 32 consecutive particles:
+//   phase A  lane <-> particle (coalesced loads/stores).  Gather from the
+//            shared stencil (the 32 lanes sit in ~4 cells: broadcast LDS),
+//            Boris, move, store of the wrapped state.  A particle that stayed
+//            inside its listed cell ("fast") writes its old/new nodal shapes
+//            and the three prefix-summed current factors to a per-warp staging
+//            slot.
+//   phase B  lane <-> (cell q of the row, plane s of that cell's window).  The
+//            four lanes of a cell walk the cell's staged particles and
+//            accumulate the Esirkepov window of the CELL in registers
+//            (3 x 12 accumulators per lane at order 3), so the per-particle
+//            cost is FMAs and broadcast LDS, not atomics.
+//   slow     a particle that crossed a cell face or is not in its listed cell
+//            is deposited by the whole warp: its (N+2)^3 window is spread over
+//            the lanes, one global RED.ADD.F64 per non-zero point.
+//   flush    at the end of a row every lane adds its accumulators to the
+//            padded global J arrays with RED.ADD.F64 (fire-and-forget; fp64
+//            atomicAdd on SHARED memory is a CAS loop on sm_100a, which is why
+//            there is no shared J tile).
+// A particle outside the tile's halo gathers from global memory instead; the
+// kernel is correct for any particle order, only slower (R39).
 #include "particle_update.cuh"
 
 namespace pic {
 
 namespace {
 
-constexpr int DRIFT = 1;   // cells a particle may sit outside its listed cell and still use the tile
+constexpr int DRIFT = 1;   // cells a particle may sit outside the tile and still gather from shared memory
 
-template <int TX_, int TY_, int TZ_, int NT_, int CH_>
+template <int N>
+struct FastWin {
+    static constexpr int FW = (N == 1) ? 2 : 4;    // nodes of the per-cell window (old and new cell identical)
+    static constexpr int FA = (N == 1) ? 0 : -1;   // first window node relative to the cell index
+};
+
+template <int TX_, int TY_, int TZ_, int NW_, int MINB_>
 struct TileCfg {
-    static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NT = NT_, CH = CH_;
-    static constexpr int NCELL = TX * TY * TZ;
-    static constexpr int NSEG = TY * TZ;
-    static constexpr int NSUB = NT / NCELL;               // threads per cell in phase B
+    static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NW = NW_, NT = 32 * NW_, MINB = MINB_;
+    static constexpr int NROW = TY * TZ;
     // gather stencil: nodes i-2 .. i+2 of a particle in cell i (every order, every staggering)
     static constexpr int GL = 2 + DRIFT;
     static constexpr int EX = TX + 2 * GL, EY = TY + 2 * GL, EZ = TZ + 2 * GL;
     static constexpr int ESZ = EX * EY * EZ;
-    // deposit window: nodes i-2 .. i+3
-    static constexpr int JL = 2 + DRIFT, JH = 3 + DRIFT;
-    static constexpr int JX = TX + JL + JH + 1, JY = TY + JL + JH, JZ = TZ + JL + JH;   // JX even
-    static constexpr int JSZ = JX * JY * JZ;
-    static constexpr int STG = CH + CH / 8 + 8;           // skewed staging rows (slot + slot/8)
-    static constexpr size_t SMEM = sizeof(double) * (6 * (size_t)ESZ + 3 * (size_t)JSZ + 7 * (size_t)STG) +
-                                   sizeof(int) * (2 * NSEG + 2 + 2 * NCELL);
-    static_assert(NT % NCELL == 0 && NSUB >= 1, "block size must be a multiple of the tile's cell count");
-    static_assert(NCELL % 32 == 0, "a warp must map onto whole cells");
+    // per-warp staging: 32 skewed slots of PITCH doubles
+    static constexpr int PITCH = 35, NSLOT = 34;
+    static constexpr int STG_W = PITCH * NSLOT;
+    static constexpr int NOFF = NROW * (TX + 1);
+    static constexpr size_t SMEM = sizeof(double) * (6 * (size_t)ESZ + (size_t)NW * STG_W) + sizeof(int) * (NOFF + 4);
+    static_assert(TX == 8, "phase B maps 8 cells x 4 planes onto a warp");
 };
+
+__device__ __forceinline__ int skew(int slot) { return slot + (slot >> 4); }
 
 // Old and new nodal shapes on the common window of N+2 slots anchored at
 // min(first old node, first new node); returns that node.  |move| < 1 cell.
@@ -76,79 +87,19 @@ __device__ __forceinline__ int shapes_pair(double xi0, double xi1, double (&s0)[
     return (s < 0) ? f1 : f0;
 }
 
-// Shared-memory adder: CAS-loop fp64 add (correct under any collision).
-template <class C>
-struct SmemAdder {
-    double* J;    // 3 * JSZ
-    __device__ __forceinline__ void operator()(int comp, int o, double v) const { atomicAdd(J + comp * C::JSZ + o, v); }
-};
-
-// Esirkepov deposition of one particle into the shared J tile.  (ox,oy,oz) =
-// tile-relative slot of the window's first node.
-template <int N, class C>
-__device__ __forceinline__ void deposit_tile(double* Jt, int ox, int oy, int oz, const double (&s0x)[N + 2],
-                                             const double (&dsx)[N + 2], const double (&s0y)[N + 2],
-                                             const double (&dsy)[N + 2], const double (&s0z)[N + 2],
-                                             const double (&dsz)[N + 2], double cx, double cy, double cz) {
-    constexpr int W = N + 2;
-    const int o0 = ox + C::JX * (oy + C::JY * oz);
-    SmemAdder<C> add{Jt};
-    {   // Jx[a,b,c] = cx * prefix_a(DSx) * (S0z[c] (S0y[b] + DSy[b]/2) + DSz[c] (S0y[b]/2 + DSy[b]/3))
-        double pd[W - 1];
-        double acc = 0.0;
+// N+1 weights whose first node is `first`, placed on the per-cell window that starts at node `anchor`.
+template <int N>
+__device__ __forceinline__ void to_fast_window(const double (&w)[N + 1], int first, int anchor,
+                                               double (&out)[FastWin<N>::FW]) {
+    if constexpr (N == 2) {
+        const bool up = first != anchor;    // base = floor(xi + 1/2) is the cell's upper node
+        out[0] = up ? 0.0 : w[0];
+        out[1] = up ? w[0] : w[1];
+        out[2] = up ? w[1] : w[2];
+        out[3] = up ? w[2] : 0.0;
+    } else {
 #pragma unroll
-        for (int a = 0; a < W - 1; ++a) { acc += dsx[a]; pd[a] = cx * acc; }
-#pragma unroll
-        for (int c = 0; c < W; ++c)
-#pragma unroll
-            for (int b = 0; b < W; ++b) {
-                const double t = s0z[c] * (s0y[b] + 0.5 * dsy[b]) + dsz[c] * (0.5 * s0y[b] + (1.0 / 3.0) * dsy[b]);
-                if (t != 0.0) {
-#pragma unroll
-                    for (int a = 0; a < W - 1; ++a) {
-                        const double v = pd[a] * t;
-                        if (v != 0.0) add(0, o0 + a + C::JX * (b + C::JY * c), v);
-                    }
-                }
-            }
-    }
-    {   // Jy
-        double pd[W - 1];
-        double acc = 0.0;
-#pragma unroll
-        for (int b = 0; b < W - 1; ++b) { acc += dsy[b]; pd[b] = cy * acc; }
-#pragma unroll
-        for (int c = 0; c < W; ++c)
-#pragma unroll
-            for (int a = 0; a < W; ++a) {
-                const double t = s0x[a] * (s0z[c] + 0.5 * dsz[c]) + dsx[a] * (0.5 * s0z[c] + (1.0 / 3.0) * dsz[c]);
-                if (t != 0.0) {
-#pragma unroll
-                    for (int b = 0; b < W - 1; ++b) {
-                        const double v = pd[b] * t;
-                        if (v != 0.0) add(1, o0 + a + C::JX * (b + C::JY * c), v);
-                    }
-                }
-            }
-    }
-    {   // Jz
-        double pd[W - 1];
-        double acc = 0.0;
-#pragma unroll
-        for (int c = 0; c < W - 1; ++c) { acc += dsz[c]; pd[c] = cz * acc; }
-#pragma unroll
-        for (int b = 0; b < W; ++b)
-#pragma unroll
-            for (int a = 0; a < W; ++a) {
-                const double t = s0y[b] * (s0x[a] + 0.5 * dsx[a]) + dsy[b] * (0.5 * s0x[a] + (1.0 / 3.0) * dsx[a]);
-                if (t != 0.0) {
-#pragma unroll
-                    for (int c = 0; c < W - 1; ++c) {
-                        const double v = pd[c] * t;
-                        if (v != 0.0) add(2, o0 + a + C::JX * (b + C::JY * c), v);
-                    }
-                }
-            }
+        for (int a = 0; a <= N; ++a) out[a] = w[a];
     }
 }
 
@@ -175,6 +126,22 @@ __device__ __forceinline__ double gather_tile(const double* __restrict__ F, int 
     return acc;
 }
 
+// Gather of all six components from the padded GLOBAL arrays (particle outside the tile's halo).
+template <int N>
+__device__ __noinline__ void gather_global6(const Grid& g, const Fields& f, double xi, double et, double ze,
+                                            double (&eb)[6]) {
+    double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[N + 1], wys[N + 1], wzs[N + 1];
+    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn), fzn = shape_weights<N>(ze, wzn);
+    const int fxs = shape_weights<N>(xi - 0.5, wxs), fys = shape_weights<N>(et - 0.5, wys),
+              fzs = shape_weights<N>(ze - 0.5, wzs);
+    eb[0] = gather_comp<N>(f.Ex, g, fxs, fyn, fzn, wxs, wyn, wzn);
+    eb[1] = gather_comp<N>(f.Ey, g, fxn, fys, fzn, wxn, wys, wzn);
+    eb[2] = gather_comp<N>(f.Ez, g, fxn, fyn, fzs, wxn, wyn, wzs);
+    eb[3] = gather_comp<N>(f.Bx, g, fxn, fys, fzs, wxn, wys, wzs);
+    eb[4] = gather_comp<N>(f.By, g, fxs, fyn, fzs, wxs, wyn, wzs);
+    eb[5] = gather_comp<N>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
+}
+
 // tile-relative cell index with the periodic image nearest to the tile
 __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
     int r = i - t0;
@@ -187,67 +154,222 @@ __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
 
 namespace {
 
+// ---- slow path: one particle deposited by the whole warp -----------------------------------
+// Layout of the record the owning lane writes at the start of the warp's staging area.
+template <int N>
+struct SlowRec {
+    static constexpr int W = N + 2;
+    static constexpr int S0X = 0, DSX = W, S0Y = 2 * W, DSY = 3 * W, S0Z = 4 * W, DSZ = 5 * W, CQ = 6 * W,
+                         ORG = 6 * W + 3;
+};
+
+// Called by the owning lane only.
+template <int N>
+__device__ __forceinline__ void slow_write(double* rec, const Grid& g, double xi0, double et0, double ze0,
+                                           double xi1, double et1, double ze1, double qw, double inv_dt) {
+    using R = SlowRec<N>;
+    constexpr int W = R::W;
+    double s0[W], ds[W];
+    bool bad = false;
+    const int nx0 = shapes_pair<N>(xi0, xi1, s0, ds, bad);
+#pragma unroll
+    for (int a = 0; a < W; ++a) { rec[R::S0X + a] = s0[a]; rec[R::DSX + a] = ds[a]; }
+    const int ny0 = shapes_pair<N>(et0, et1, s0, ds, bad);
+#pragma unroll
+    for (int a = 0; a < W; ++a) { rec[R::S0Y + a] = s0[a]; rec[R::DSY + a] = ds[a]; }
+    const int nz0 = shapes_pair<N>(ze0, ze1, s0, ds, bad);
+#pragma unroll
+    for (int a = 0; a < W; ++a) { rec[R::S0Z + a] = s0[a]; rec[R::DSZ + a] = ds[a]; }
+    rec[R::CQ + 0] = -qw * inv_dt * g.inv_dy * g.inv_dz;
+    rec[R::CQ + 1] = -qw * inv_dt * g.inv_dx * g.inv_dz;
+    rec[R::CQ + 2] = -qw * inv_dt * g.inv_dx * g.inv_dy;
+    rec[R::ORG] = __longlong_as_double(g.idx(nx0, ny0, nz0));   // window nodes stay inside the guard shell
+}
+
+// Called by all 32 lanes: lane <-> one (u,v) pair of the window's cross-section; W-1 points along the
+// prefix direction each.  Jx = cqx prefix_a(DSx) (S0y Az + DSy Bz), A = S0 + DS/2, B = S0/2 + DS/3, and
+// cyclic permutations.
+template <int N>
+__device__ __forceinline__ void slow_deposit(const double* rec, const Grid& g, const Fields& f, int lane) {
+    using R = SlowRec<N>;
+    constexpr int W = R::W;
+    if (lane >= W * W) return;
+    const int u = lane % W, v = lane / W;
+    const long long o0 = __double_as_longlong(rec[R::ORG]);
+    const double third = 1.0 / 3.0;
+    {   // Jx: (u,v) = (b,c)
+        const double s0z = rec[R::S0Z + v], dsz = rec[R::DSZ + v];
+        const double t = rec[R::S0Y + u] * (s0z + 0.5 * dsz) + rec[R::DSY + u] * (0.5 * s0z + third * dsz);
+        if (t != 0.0) {
+            const double cq = rec[R::CQ + 0];
+            double* dst = f.Jx + o0 + g.sy * u + g.sz * v;
+            double acc = 0.0;
+#pragma unroll
+            for (int a = 0; a < W - 1; ++a) {
+                acc += rec[R::DSX + a];
+                const double val = (cq * acc) * t;
+                if (val != 0.0) atomicAdd(dst + a, val);
+            }
+        }
+    }
+    {   // Jy: (u,v) = (a,c)
+        const double s0z = rec[R::S0Z + v], dsz = rec[R::DSZ + v];
+        const double t = rec[R::S0X + u] * (s0z + 0.5 * dsz) + rec[R::DSX + u] * (0.5 * s0z + third * dsz);
+        if (t != 0.0) {
+            const double cq = rec[R::CQ + 1];
+            double* dst = f.Jy + o0 + u + g.sz * v;
+            double acc = 0.0;
+#pragma unroll
+            for (int b = 0; b < W - 1; ++b) {
+                acc += rec[R::DSY + b];
+                const double val = (cq * acc) * t;
+                if (val != 0.0) atomicAdd(dst + g.sy * b, val);
+            }
+        }
+    }
+    {   // Jz: (u,v) = (a,b)
+        const double s0y = rec[R::S0Y + v], dsy = rec[R::DSY + v];
+        const double t = rec[R::S0X + u] * (s0y + 0.5 * dsy) + rec[R::DSX + u] * (0.5 * s0y + third * dsy);
+        if (t != 0.0) {
+            const double cq = rec[R::CQ + 2];
+            double* dst = f.Jz + o0 + u + g.sy * v;
+            double acc = 0.0;
+#pragma unroll
+            for (int c = 0; c < W - 1; ++c) {
+                acc += rec[R::DSZ + c];
+                const double val = (cq * acc) * t;
+                if (val != 0.0) atomicAdd(dst + g.sz * c, val);
+            }
+        }
+    }
+}
+
+// ---- fast path: per-(cell, plane) register accumulators --------------------------------------
+// Staging slot layout (FW = window nodes): s0x dsx s0y dsy s0z dsz (FW each), then pdx pdy pdz
+// (FW-1 each) with pd_d[a] = cq_d * sum_{a' <= a} ds_d[a'].
+template <int N>
+struct FastRec {
+    static constexpr int FW = FastWin<N>::FW;
+    static constexpr int S0X = 0, DSX = FW, S0Y = 2 * FW, DSY = 3 * FW, S0Z = 4 * FW, DSZ = 5 * FW, PDX = 6 * FW,
+                         PDY = 6 * FW + (FW - 1), PDZ = 6 * FW + 2 * (FW - 1), LEN = 6 * FW + 3 * (FW - 1);
+};
+
+template <int N>
+struct CellAcc {
+    static constexpr int FW = FastWin<N>::FW;
+    double jx[FW - 1][FW];   // Jx[a][b] on plane c = s
+    double jy[FW][FW - 1];   // Jy[a][b] on plane c = s
+    double jz[FW][FW - 1];   // Jz[a][c] on row   b = s
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int a = 0; a < FW - 1; ++a)
+#pragma unroll
+            for (int b = 0; b < FW; ++b) jx[a][b] = 0.0;
+#pragma unroll
+        for (int a = 0; a < FW; ++a)
+#pragma unroll
+            for (int b = 0; b < FW - 1; ++b) { jy[a][b] = 0.0; jz[a][b] = 0.0; }
+    }
+    // one staged particle; s = this lane's plane
+    __device__ __forceinline__ void add(const double* __restrict__ r, int s) {
+        using R = FastRec<N>;
+        const double third = 1.0 / 3.0;
+        const double s0z = r[R::S0Z + s], dsz = r[R::DSZ + s];
+        const double az = s0z + 0.5 * dsz, bz = 0.5 * s0z + third * dsz;
+        const double s0ys = r[R::S0Y + s], dsys = r[R::DSY + s];
+        const double ay = s0ys + 0.5 * dsys, by = 0.5 * s0ys + third * dsys;
+        double pd[FW - 1];
+#pragma unroll
+        for (int a = 0; a < FW - 1; ++a) pd[a] = r[R::PDX + a];
+#pragma unroll
+        for (int b = 0; b < FW; ++b) {
+            const double t = r[R::S0Y + b] * az + r[R::DSY + b] * bz;
+#pragma unroll
+            for (int a = 0; a < FW - 1; ++a) jx[a][b] = fma(pd[a], t, jx[a][b]);
+        }
+        double s0x[FW], dsx[FW];
+#pragma unroll
+        for (int a = 0; a < FW; ++a) { s0x[a] = r[R::S0X + a]; dsx[a] = r[R::DSX + a]; }
+#pragma unroll
+        for (int b = 0; b < FW - 1; ++b) pd[b] = r[R::PDY + b];
+#pragma unroll
+        for (int a = 0; a < FW; ++a) {
+            const double t = s0x[a] * az + dsx[a] * bz;
+#pragma unroll
+            for (int b = 0; b < FW - 1; ++b) jy[a][b] = fma(pd[b], t, jy[a][b]);
+        }
+#pragma unroll
+        for (int c = 0; c < FW - 1; ++c) pd[c] = r[R::PDZ + c];
+#pragma unroll
+        for (int a = 0; a < FW; ++a) {
+            const double t = s0x[a] * ay + dsx[a] * by;
+#pragma unroll
+            for (int c = 0; c < FW - 1; ++c) jz[a][c] = fma(pd[c], t, jz[a][c]);
+        }
+    }
+    // add to the padded global arrays; o = offset of the window's first node, s = this lane's plane
+    __device__ __forceinline__ void flush(const Grid& g, const Fields& f, long long o, int s) const {
+        double* px = f.Jx + o + g.sz * s;
+        double* py = f.Jy + o + g.sz * s;
+        double* pz = f.Jz + o + g.sy * s;
+#pragma unroll
+        for (int b = 0; b < FW; ++b)
+#pragma unroll
+            for (int a = 0; a < FW - 1; ++a)
+                if (jx[a][b] != 0.0) atomicAdd(px + a + g.sy * b, jx[a][b]);
+#pragma unroll
+        for (int b = 0; b < FW - 1; ++b)
+#pragma unroll
+            for (int a = 0; a < FW; ++a)
+                if (jy[a][b] != 0.0) atomicAdd(py + a + g.sy * b, jy[a][b]);
+#pragma unroll
+        for (int c = 0; c < FW - 1; ++c)
+#pragma unroll
+            for (int a = 0; a < FW; ++a)
+                if (jz[a][c] != 0.0) atomicAdd(pz + a + g.sz * c, jz[a][c]);
+    }
+};
+
+}  // namespace
+
+namespace {
+
 template <int N, class C>
-__global__ void __launch_bounds__(C::NT, 1)
+__global__ void __launch_bounds__(C::NT, C::MINB)
 particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const unsigned int* __restrict__ cell_offset,
                       int ntx, int nty, DevStatus* status) {
+    constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA;
+    using FR = FastRec<N>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* Et = reinterpret_cast<double*>(smem_raw);            // 6 * ESZ: Ex Ey Ez Bx By Bz
-    double* Jt = Et + 6 * C::ESZ;                                // 3 * JSZ
-    double* stg = Jt + 3 * C::JSZ;                               // 7 * STG
-    int* seg_start = reinterpret_cast<int*>(stg + 7 * C::STG);   // NSEG: container index of the segment's first particle
-    int* seg_pref = seg_start + C::NSEG;                         // NSEG + 1: tile index of the segment's first particle
-    int* cell_lo = seg_pref + C::NSEG + 2;                       // NCELL: tile-index range of every cell
-    int* cell_hi = cell_lo + C::NCELL;
+    double* stg_all = Et + 6 * C::ESZ;                           // NW * STG_W
+    int* row_off = reinterpret_cast<int*>(stg_all + C::NW * C::STG_W);   // NROW x (TX+1) container indices
+    int* next_row = row_off + C::NOFF;
 
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     int b = blockIdx.x;
     const int bx = b % ntx; b /= ntx;
     const int by = b % nty;
     const int bz = b / nty;
     const int t0x = bx * C::TX, t0y = by * C::TY, t0z = bz * C::TZ;
 
-    // ---- segments and cell ranges -------------------------------------------------
-    if (tid < C::NSEG) {
-        const int j = t0y + tid % C::TY, k = t0z + tid / C::TY;
-        int s0 = 0, len = 0;
-        if (j < g.ny && k < g.nz) {
-            const long long row = (long long)g.nx * (j + (long long)g.ny * k);
-            const int x1 = min(t0x + C::TX, g.nx);
-            s0 = (int)cell_offset[row + t0x];
-            len = (int)cell_offset[row + x1] - s0;
-        }
-        seg_start[tid] = s0;
-        seg_pref[tid + 1] = len;    // lengths; prefix-summed below
+    // ---- container index of every cell boundary of the tile's rows --------------------------
+    for (int e = tid; e < C::NOFF; e += C::NT) {
+        const int r = e / (C::TX + 1), c = e % (C::TX + 1);
+        const int j = t0y + r % C::TY, k = t0z + r / C::TY;
+        int v = 0;
+        if (j < g.ny && k < g.nz)
+            v = (int)cell_offset[(long long)g.nx * (j + (long long)g.ny * k) + min(t0x + c, g.nx)];
+        row_off[e] = v;
     }
-    if (tid == 0) seg_pref[0] = 0;
+    if (tid == 0) *next_row = 0;
     __syncthreads();
-    if (tid == 0) {
-        int run = 0;
-        for (int s = 0; s < C::NSEG; ++s) {
-            const int len = seg_pref[s + 1];
-            seg_pref[s] = run;
-            run += len;
-        }
-        seg_pref[C::NSEG] = run;
-    }
-    __syncthreads();
-    const int n_tile = seg_pref[C::NSEG];
-    if (n_tile == 0) return;    // empty tile: nothing to gather, nothing to deposit (block-uniform)
-    for (int c = tid; c < C::NCELL; c += C::NT) {
-        const int cx = c % C::TX, cy = (c / C::TX) % C::TY, cz = c / (C::TX * C::TY);
-        const int i = t0x + cx, j = t0y + cy, k = t0z + cz;
-        int lo = 0, hi = 0;
-        if (i < g.nx && j < g.ny && k < g.nz) {
-            const long long key = i + (long long)g.nx * (j + (long long)g.ny * k);
-            const int s = cy + C::TY * cz;
-            lo = seg_pref[s] + ((int)cell_offset[key] - seg_start[s]);
-            hi = seg_pref[s] + ((int)cell_offset[key + 1] - seg_start[s]);
-        }
-        cell_lo[c] = lo;
-        cell_hi[c] = hi;
-    }
-    // ---- stage the field stencil, zero the J tile -----------------------------------
+    int n_tile = 0;
+#pragma unroll 4
+    for (int r = 0; r < C::NROW; ++r) n_tile += row_off[r * (C::TX + 1) + C::TX] - row_off[r * (C::TX + 1)];
+    if (n_tile == 0) return;    // empty tile (block-uniform)
+
+    // ---- stage the field stencil ----------------------------------------------------------------
     {
         const double* src[6] = {f.Ex, f.Ey, f.Ez, f.Bx, f.By, f.Bz};
         for (int e = tid; e < C::ESZ; e += C::NT) {
@@ -258,137 +380,184 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
 #pragma unroll
             for (int cpt = 0; cpt < 6; ++cpt) Et[cpt * C::ESZ + e] = ok ? __ldg(src[cpt] + o) : 0.0;
         }
-        for (int e = tid; e < 3 * C::JSZ; e += C::NT) Jt[e] = 0.0;
     }
     __syncthreads();
 
     const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
     const double inv_dt = 1.0 / g.dt;
+    double* stg = stg_all + warp * C::STG_W;
+    const int bq = lane >> 2, bs = lane & 3;     // phase B role: cell of the row, plane of the window
     unsigned int n_fast = 0, n_slow = 0, n_glob = 0;
     bool bad_any = false;
 
-    for (int lo = 0; lo < n_tile; lo += C::CH) {
-        const int hi = min(lo + C::CH, n_tile);
-        // ---------------- phase A: gather + push + move, particle-major ----------------
-        for (int idx = lo + tid; idx < hi; idx += C::NT) {
-            int s = 0;
-#pragma unroll
-            for (int step = C::NSEG / 2; step >= 1; step >>= 1)
-                if (s + step < C::NSEG && seg_pref[s + step] <= idx) s += step;
-            const long long ip = (long long)seg_start[s] + (idx - seg_pref[s]);
-            const int slot = idx - lo, sl = slot + (slot >> 3);
-            const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
-            const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy, ze = (z - g.zmin) * g.inv_dz;
-            const int ci = __double2int_rd(xi), cj = __double2int_rd(et), ck = __double2int_rd(ze);
-            const int rx = rel_cell(ci, t0x, C::TX, g.nx), ry = rel_cell(cj, t0y, C::TY, g.ny),
-                      rz = rel_cell(ck, t0z, C::TZ, g.nz);
-            const bool in_tile = rx >= -DRIFT && rx <= C::TX - 1 + DRIFT && t0x + rx <= g.nx - 1 + DRIFT &&
-                                 ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
-                                 rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
-            if (!in_tile) {
-                // left the tile's halo since the last sort: whole update against the global arrays
-                update_particle_global<N>(g, f, p, ip, q, h, status);
-                stg[6 * C::STG + sl] = 0.0;    // nothing to deposit in phase B
-                ++n_glob;
-                continue;
-            }
-            double ux = p.ux[ip], uy = p.uy[ip], uz = p.uz[ip];
-            const double w = p.w[ip];
-            double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[N + 1], wys[N + 1], wzs[N + 1];
-            // first nodes, shifted from global node index to tile slot: slot = node - (t0 - GL) + (image shift)
-            const int shx = (rx - (ci - t0x)) + C::GL - t0x, shy = (ry - (cj - t0y)) + C::GL - t0y,
-                      shz = (rz - (ck - t0z)) + C::GL - t0z;
-            const int fxn = shape_weights<N>(xi, wxn) + shx, fyn = shape_weights<N>(et, wyn) + shy,
-                      fzn = shape_weights<N>(ze, wzn) + shz;
-            const int fxs = shape_weights<N>(xi - 0.5, wxs) + shx, fys = shape_weights<N>(et - 0.5, wys) + shy,
-                      fzs = shape_weights<N>(ze - 0.5, wzs) + shz;
-            const double ex = gather_tile<N, C>(Et + 0 * C::ESZ, fxs, fyn, fzn, wxs, wyn, wzn);
-            const double ey = gather_tile<N, C>(Et + 1 * C::ESZ, fxn, fys, fzn, wxn, wys, wzn);
-            const double ez = gather_tile<N, C>(Et + 2 * C::ESZ, fxn, fyn, fzs, wxn, wyn, wzs);
-            const double bxp = gather_tile<N, C>(Et + 3 * C::ESZ, fxn, fys, fzs, wxn, wys, wzs);
-            const double byp = gather_tile<N, C>(Et + 4 * C::ESZ, fxs, fyn, fzs, wxs, wyn, wzs);
-            const double bzp = gather_tile<N, C>(Et + 5 * C::ESZ, fxs, fys, fzn, wxs, wys, wzn);
-            boris_push(h, inv_c2, ux, uy, uz, ex, ey, ez, bxp, byp, bzp);
-            const double gam = sqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
-            const double x1 = x + g.dt * ux / gam, y1 = y + g.dt * uy / gam, z1 = z + g.dt * uz / gam;
-            const double xi1 = (x1 - g.xmin) * g.inv_dx, et1 = (y1 - g.ymin) * g.inv_dy,
-                         ze1 = (z1 - g.zmin) * g.inv_dz;
-            const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
-                             !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
-            bad_any = bad_any || bad;
-            p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
-            p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
-            p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
-            p.ux[ip] = ux;
-            p.uy[ip] = uy;
-            p.uz[ip] = uz;
-            stg[0 * C::STG + sl] = xi;
-            stg[1 * C::STG + sl] = et;
-            stg[2 * C::STG + sl] = ze;
-            stg[3 * C::STG + sl] = xi1;
-            stg[4 * C::STG + sl] = et1;
-            stg[5 * C::STG + sl] = ze1;
-            stg[6 * C::STG + sl] = bad ? 0.0 : q * w;
-            if (rx == ci - t0x + 0 && ry == cj - t0y && rz == ck - t0z) ++n_fast; else ++n_slow;
-        }
-        __syncthreads();
-        // ---------------- phase B: Esirkepov deposition, cell-major ----------------------
-        {
-            const int c = tid % C::NCELL, sub = tid / C::NCELL;
-            const int p0 = max(cell_lo[c], lo), p1 = min(cell_hi[c], hi);
-            for (int idx = p0 + sub; idx < p1; idx += C::NSUB) {
-                const int slot = idx - lo, sl = slot + (slot >> 3);
-                const double qw = stg[6 * C::STG + sl];
-                if (qw == 0.0) continue;
-                const double xi = stg[0 * C::STG + sl], et = stg[1 * C::STG + sl], ze = stg[2 * C::STG + sl];
-                const double xi1 = stg[3 * C::STG + sl], et1 = stg[4 * C::STG + sl], ze1 = stg[5 * C::STG + sl];
-                double s0x[N + 2], dsx[N + 2], s0y[N + 2], dsy[N + 2], s0z[N + 2], dsz[N + 2];
-                bool bad = false;
-                const int nx0 = shapes_pair<N>(xi, xi1, s0x, dsx, bad);
-                const int ny0 = shapes_pair<N>(et, et1, s0y, dsy, bad);
-                const int nz0 = shapes_pair<N>(ze, ze1, s0z, dsz, bad);
-                // image shift of the OLD cell, as in phase A
+    for (;;) {
+        int row = 0;
+        if (lane == 0) row = atomicAdd(next_row, 1);
+        row = __shfl_sync(0xffffffffu, row, 0);
+        if (row >= C::NROW) break;
+        const int* off = row_off + row * (C::TX + 1);
+        const int row_lo = off[0], row_hi = off[C::TX];
+        if (row_lo >= row_hi) continue;
+        const int ry0 = row % C::TY, rz0 = row / C::TY;     // the row's tile-relative (y, z) cell
+        const int cell_lo = off[bq], cell_hi = off[bq + 1];  // phase B: this lane's cell
+        CellAcc<N> acc;
+        acc.clear();
+        bool touched = false;
+
+        for (int base = row_lo; base < row_hi; base += 32) {
+            // ---------------- phase A: lane <-> particle ------------------------------------------
+            const int ip = base + lane;
+            const bool active = ip < row_hi;
+            bool is_slow = false;
+            double xi = 0.0, et = 0.0, ze = 0.0, xi1 = 0.0, et1 = 0.0, ze1 = 0.0, qw = 0.0;
+            if (active) {
+                const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
+                double ux = p.ux[ip], uy = p.uy[ip], uz = p.uz[ip];
+                qw = q * p.w[ip];
+                xi = (x - g.xmin) * g.inv_dx; et = (y - g.ymin) * g.inv_dy; ze = (z - g.zmin) * g.inv_dz;
                 const int ci = __double2int_rd(xi), cj = __double2int_rd(et), ck = __double2int_rd(ze);
-                const int ox = nx0 + (rel_cell(ci, t0x, C::TX, g.nx) - ci) + C::JL;
-                const int oy = ny0 + (rel_cell(cj, t0y, C::TY, g.ny) - cj) + C::JL;
-                const int oz = nz0 + (rel_cell(ck, t0z, C::TZ, g.nz) - ck) + C::JL;
-                const double cqx = -qw * inv_dt * g.inv_dy * g.inv_dz;
-                const double cqy = -qw * inv_dt * g.inv_dx * g.inv_dz;
-                const double cqz = -qw * inv_dt * g.inv_dx * g.inv_dy;
-                deposit_tile<N, C>(Jt, ox, oy, oz, s0x, dsx, s0y, dsy, s0z, dsz, cqx, cqy, cqz);
-            }
-        }
-        __syncthreads();
-    }
-    // ---- flush: one global atomic per non-zero tile point ---------------------------------
-    {
-        double* dst[3] = {f.Jx, f.Jy, f.Jz};
-        for (int e = tid; e < C::JSZ; e += C::NT) {
-            const int jx = e % C::JX, jy = (e / C::JX) % C::JY, jz = e / (C::JX * C::JY);
-            const int gx = t0x - C::JL + jx + NG, gy = t0y - C::JL + jy + NG, gz = t0z - C::JL + jz + NG;
-            const bool ok = gx >= 0 && gx < g.nx + 2 * NG && gy >= 0 && gy < g.py && gz >= 0 && gz < g.pz;
-            if (!ok) continue;
-            const long long o = gx + g.sy * gy + g.sz * gz;
+                const int rx = rel_cell(ci, t0x, C::TX, g.nx), ry = rel_cell(cj, t0y, C::TY, g.ny),
+                          rz = rel_cell(ck, t0z, C::TZ, g.nz);
+                const bool in_tile = rx >= -DRIFT && rx <= C::TX - 1 + DRIFT && t0x + rx <= g.nx - 1 + DRIFT &&
+                                     ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
+                                     rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
+                double wxn[N + 1], wyn[N + 1], wzn[N + 1];
+                const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn),
+                          fzn = shape_weights<N>(ze, wzn);
+                double eb[6];
+                if (in_tile) {
+                    double wxs[N + 1], wys[N + 1], wzs[N + 1];
+                    // first nodes, shifted from global node index to tile slot: slot = node - (t0 - GL) + image shift
+                    const int shx = (rx - (ci - t0x)) + C::GL - t0x, shy = (ry - (cj - t0y)) + C::GL - t0y,
+                              shz = (rz - (ck - t0z)) + C::GL - t0z;
+                    const int fxs = shape_weights<N>(xi - 0.5, wxs) + shx, fys = shape_weights<N>(et - 0.5, wys) + shy,
+                              fzs = shape_weights<N>(ze - 0.5, wzs) + shz;
+                    const int gxn = fxn + shx, gyn = fyn + shy, gzn = fzn + shz;
+                    eb[0] = gather_tile<N, C>(Et + 0 * C::ESZ, fxs, gyn, gzn, wxs, wyn, wzn);
+                    eb[1] = gather_tile<N, C>(Et + 1 * C::ESZ, gxn, fys, gzn, wxn, wys, wzn);
+                    eb[2] = gather_tile<N, C>(Et + 2 * C::ESZ, gxn, gyn, fzs, wxn, wyn, wzs);
+                    eb[3] = gather_tile<N, C>(Et + 3 * C::ESZ, gxn, fys, fzs, wxn, wys, wzs);
+                    eb[4] = gather_tile<N, C>(Et + 4 * C::ESZ, fxs, gyn, fzs, wxs, wyn, wzs);
+                    eb[5] = gather_tile<N, C>(Et + 5 * C::ESZ, fxs, fys, gzn, wxs, wys, wzn);
+                } else {
+                    gather_global6<N>(g, f, xi, et, ze, eb);
+                    ++n_glob;
+                }
+                boris_push(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
+                const double gam = sqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
+                const double x1 = x + g.dt * ux / gam, y1 = y + g.dt * uy / gam, z1 = z + g.dt * uz / gam;
+                xi1 = (x1 - g.xmin) * g.inv_dx; et1 = (y1 - g.ymin) * g.inv_dy; ze1 = (z1 - g.zmin) * g.inv_dz;
+                const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
+                                 !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
+                bad_any = bad_any || bad;
+                p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
+                p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
+                p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
+                p.ux[ip] = ux;
+                p.uy[ip] = uy;
+                p.uz[ip] = uz;
+                // ---- classify: fast = stayed inside the cell the sort listed it in -------------
+                int lc = 0;
 #pragma unroll
-            for (int cpt = 0; cpt < 3; ++cpt) {
-                const double v = Jt[cpt * C::JSZ + e];
-                if (v != 0.0) atomicAdd(dst[cpt] + o, v);
+                for (int c = 1; c < C::TX; ++c) lc += (off[c] <= ip) ? 1 : 0;
+                const bool same = __double2int_rd(xi1) == ci && __double2int_rd(et1) == cj &&
+                                  __double2int_rd(ze1) == ck;
+                const bool listed = in_tile && rx == lc && ry == ry0 && rz == rz0;
+                const bool deposits = !bad && qw != 0.0;
+                const bool fast = deposits && same && listed;
+                is_slow = deposits && !fast;
+                if (in_tile) { if (is_slow) ++n_slow; else ++n_fast; }
+                // ---- stage the fast record (zeros when the particle is not fast) ---------------
+                double* r = stg + skew(lane) * C::PITCH;
+                {
+                    double w1[N + 1], s0[FW], s1[FW];
+                    int f1;
+                    double cq, run;
+                    // x
+                    f1 = shape_weights<N>(xi1, w1);
+                    to_fast_window<N>(wxn, fxn, ci + FA, s0);
+                    to_fast_window<N>(w1, f1, ci + FA, s1);
+                    cq = fast ? -qw * inv_dt * g.inv_dy * g.inv_dz : 0.0;
+                    run = 0.0;
+#pragma unroll
+                    for (int a = 0; a < FW; ++a) {
+                        const double d = s1[a] - s0[a];
+                        r[FR::S0X + a] = fast ? s0[a] : 0.0;
+                        r[FR::DSX + a] = fast ? d : 0.0;
+                        run += d;
+                        if (a < FW - 1) r[FR::PDX + a] = fast ? cq * run : 0.0;
+                    }
+                    // y
+                    f1 = shape_weights<N>(et1, w1);
+                    to_fast_window<N>(wyn, fyn, cj + FA, s0);
+                    to_fast_window<N>(w1, f1, cj + FA, s1);
+                    cq = fast ? -qw * inv_dt * g.inv_dx * g.inv_dz : 0.0;
+                    run = 0.0;
+#pragma unroll
+                    for (int a = 0; a < FW; ++a) {
+                        const double d = s1[a] - s0[a];
+                        r[FR::S0Y + a] = fast ? s0[a] : 0.0;
+                        r[FR::DSY + a] = fast ? d : 0.0;
+                        run += d;
+                        if (a < FW - 1) r[FR::PDY + a] = fast ? cq * run : 0.0;
+                    }
+                    // z
+                    f1 = shape_weights<N>(ze1, w1);
+                    to_fast_window<N>(wzn, fzn, ck + FA, s0);
+                    to_fast_window<N>(w1, f1, ck + FA, s1);
+                    cq = fast ? -qw * inv_dt * g.inv_dx * g.inv_dy : 0.0;
+                    run = 0.0;
+#pragma unroll
+                    for (int a = 0; a < FW; ++a) {
+                        const double d = s1[a] - s0[a];
+                        r[FR::S0Z + a] = fast ? s0[a] : 0.0;
+                        r[FR::DSZ + a] = fast ? d : 0.0;
+                        run += d;
+                        if (a < FW - 1) r[FR::PDZ + a] = fast ? cq * run : 0.0;
+                    }
+                }
+            }
+            __syncwarp();
+            // ---------------- phase B: lane <-> (cell, plane) ------------------------------------
+            {
+                const int lo = max(cell_lo, base), hi = min(cell_hi, base + 32);
+                const int len = (bs < FW) ? hi - lo : 0;
+                const int maxlen = __reduce_max_sync(0xffffffffu, max(len, 0));
+                for (int t = 0; t < maxlen; ++t) {
+                    if (t < len) {
+                        acc.add(stg + skew(lo + t - base) * C::PITCH, bs);
+                        touched = true;
+                    }
+                }
+            }
+            __syncwarp();
+            // ---------------- slow path: one particle at a time, whole warp ---------------------
+            unsigned int slow_mask = __ballot_sync(0xffffffffu, is_slow);
+            while (slow_mask) {
+                const int L = __ffs(slow_mask) - 1;
+                slow_mask &= slow_mask - 1;
+                if (lane == L) slow_write<N>(stg, g, xi, et, ze, xi1, et1, ze1, qw, inv_dt);
+                __syncwarp();
+                slow_deposit<N>(stg, g, f, lane);
+                __syncwarp();
             }
         }
+        // ---------------- flush the row's accumulators ---------------------------------------------
+        if (touched) acc.flush(g, f, g.idx(t0x + bq + FA, t0y + ry0 + FA, t0z + rz0 + FA), bs);
     }
-    // ---- counters ----------------------------------------------------------------------------
+    // ---- flags and counters ----------------------------------------------------------------------
     if (bad_any) status->ephys = 1;
     n_fast = __reduce_add_sync(0xffffffffu, n_fast);
     n_slow = __reduce_add_sync(0xffffffffu, n_slow);
     n_glob = __reduce_add_sync(0xffffffffu, n_glob);
-    if ((tid & 31) == 0) {
+    if (lane == 0) {
         if (n_fast) atomicAdd(&status->n_fast, (unsigned long long)n_fast);
         if (n_slow) atomicAdd(&status->n_slow, (unsigned long long)n_slow);
         if (n_glob) atomicAdd(&status->n_global, (unsigned long long)n_glob);
     }
 }
 
-using Cfg = TileCfg<8, 4, 4, 256, 512>;
+using Cfg = TileCfg<8, 4, 4, 8, 1>;
 
 template <int N>
 void launch_tile(const Grid& g, const Fields& f, const Particles& p, double q, double h,
