@@ -50,15 +50,16 @@ struct TileCfg {
     static constexpr int GL = 2 + DRIFT;
     static constexpr int EX = TX + 2 * GL, EY = TY + 2 * GL, EZ = TZ + 2 * GL;
     static constexpr int ESZ = EX * EY * EZ;
-    // per-warp staging: 32 skewed slots of PITCH doubles
-    static constexpr int PITCH = 35, NSLOT = 34;
+    // per-warp staging: CHUNK skewed slots of PITCH doubles (PITCH/2 odd and the skew make the eight
+    // 16-byte words a phase-B warp load touches fall into eight different 16-byte bank groups)
+    static constexpr int CHUNK = 64, PITCH = 34, NSLOT = CHUNK + CHUNK / 8;
     static constexpr int STG_W = PITCH * NSLOT;
     static constexpr int NOFF = NROW * (TX + 1);
     static constexpr size_t SMEM = sizeof(double) * (6 * (size_t)ESZ + (size_t)NW * STG_W) + sizeof(int) * (NOFF + 4);
     static_assert(TX == 8, "phase B maps 8 cells x 4 planes onto a warp");
 };
 
-__device__ __forceinline__ int skew(int slot) { return slot + (slot >> 4); }
+__device__ __forceinline__ int skew(int slot) { return slot + (slot >> 3); }
 
 // Old and new nodal shapes on the common window of N+2 slots anchored at
 // min(first old node, first new node); returns that node.  |move| < 1 cell.
@@ -103,27 +104,55 @@ __device__ __forceinline__ void to_fast_window(const double (&w)[N + 1], int fir
     }
 }
 
-// One component from the shared stencil; (fx,fy,fz) = tile slot of the first node.
+// One z-plane of one component from the shared stencil: sum_b wy[b] sum_a wx[a] F[a,b].
 template <int N, class C>
-__device__ __forceinline__ double gather_tile(const double* __restrict__ F, int fx, int fy, int fz,
-                                              const double (&wx)[N + 1], const double (&wy)[N + 1],
-                                              const double (&wz)[N + 1]) {
-    const double* base = F + fx + C::EX * (fy + C::EY * fz);
-    double acc = 0.0;
+__device__ __forceinline__ double gather_plane(const double* __restrict__ base, const double (&wx)[N + 1],
+                                               const double (&wy)[N + 1]) {
+    double accy = 0.0;
 #pragma unroll
-    for (int c = 0; c <= N; ++c) {
-        double accy = 0.0;
+    for (int b = 0; b <= N; ++b) {
+        const double* row = base + C::EX * b;
+        double accx = 0.0;
 #pragma unroll
-        for (int b = 0; b <= N; ++b) {
-            const double* row = base + C::EX * (b + C::EY * c);
-            double accx = 0.0;
-#pragma unroll
-            for (int a = 0; a <= N; ++a) accx = fma(wx[a], row[a], accx);
-            accy = fma(wy[b], accx, accy);
-        }
-        acc = fma(wz[c], accy, acc);
+        for (int a = 0; a <= N; ++a) accx = fma(wx[a], row[a], accx);
+        accy = fma(wy[b], accx, accy);
     }
-    return acc;
+    return accy;
+}
+
+// All six components from the shared stencil.  (g*n) / (f*s) = tile slot of the first nodal /
+// staggered node per dimension.  The z loop is kept ROLLED (the z weights rotate through their
+// register arrays and are back in place after N+1 trips): the body is ~250 instructions that stay in
+// the L0 instruction cache instead of ~1000 straight-line ones.
+template <int N, class C>
+__device__ __forceinline__ void gather6_tile(const double* __restrict__ Et, int gxn, int gyn, int gzn, int fxs,
+                                             int fys, int fzs, const double (&wxn)[N + 1],
+                                             const double (&wyn)[N + 1], double (&wzn)[N + 1],
+                                             const double (&wxs)[N + 1], const double (&wys)[N + 1],
+                                             double (&wzs)[N + 1], double (&eb)[6]) {
+    const int o_ex = 0 * C::ESZ + fxs + C::EX * (gyn + C::EY * gzn);
+    const int o_ey = 1 * C::ESZ + gxn + C::EX * (fys + C::EY * gzn);
+    const int o_ez = 2 * C::ESZ + gxn + C::EX * (gyn + C::EY * fzs);
+    const int o_bx = 3 * C::ESZ + gxn + C::EX * (fys + C::EY * fzs);
+    const int o_by = 4 * C::ESZ + fxs + C::EX * (gyn + C::EY * fzs);
+    const int o_bz = 5 * C::ESZ + fxs + C::EX * (fys + C::EY * gzn);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) eb[k] = 0.0;
+    const double* pl = Et;
+#pragma unroll 1
+    for (int c = 0; c <= N; ++c, pl += C::EX * C::EY) {
+        const double zn = wzn[0], zs = wzs[0];
+        eb[0] = fma(zn, gather_plane<N, C>(pl + o_ex, wxs, wyn), eb[0]);
+        eb[1] = fma(zn, gather_plane<N, C>(pl + o_ey, wxn, wys), eb[1]);
+        eb[2] = fma(zs, gather_plane<N, C>(pl + o_ez, wxn, wyn), eb[2]);
+        eb[3] = fma(zs, gather_plane<N, C>(pl + o_bx, wxn, wys), eb[3]);
+        eb[4] = fma(zs, gather_plane<N, C>(pl + o_by, wxs, wyn), eb[4]);
+        eb[5] = fma(zn, gather_plane<N, C>(pl + o_bz, wxs, wys), eb[5]);
+#pragma unroll
+        for (int k = 0; k < N; ++k) { wzn[k] = wzn[k + 1]; wzs[k] = wzs[k + 1]; }
+        wzn[N] = zn;
+        wzs[N] = zs;
+    }
 }
 
 // Gather of all six components from the padded GLOBAL arrays (particle outside the tile's halo).
@@ -154,41 +183,61 @@ __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
 
 namespace {
 
+constexpr int FLAG = 33;           // last double of every staging slot: record kind
+constexpr double REC_FAST = 0.0;   // fast record (FastRec layout), accumulated by phase B
+constexpr double REC_SLOW = 1.0;   // slow record (SlowRec layout), deposited by the whole warp
+constexpr double REC_NONE = 2.0;   // nothing to deposit (q = 0, or the particle raised PIC_EPHYS)
+
+// fp64 add to GLOBAL memory without a return value: REDG.E.ADD.F64 (fire-and-forget).  atomicAdd on a
+// pointer whose address space the compiler cannot prove emits a generic ATOM with a returned value
+// plus shared-memory CAS fallbacks, and every use then waits a full L2 round trip.
+__device__ __forceinline__ void red_add(double* p, double v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
+__device__ __forceinline__ double2 ld2(const double* r, int i) { return *reinterpret_cast<const double2*>(r + i); }
+__device__ __forceinline__ void st2(double* r, int i, double a, double b) {
+    *reinterpret_cast<double2*>(r + i) = make_double2(a, b);
+}
+
 // ---- slow path: one particle deposited by the whole warp -----------------------------------
-// Layout of the record the owning lane writes at the start of the warp's staging area.
 template <int N>
 struct SlowRec {
     static constexpr int W = N + 2;
+    // per dimension d: s0 at 2 W d, ds at 2 W d + W;  then -q w / dt and the window's first padded offset
     static constexpr int S0X = 0, DSX = W, S0Y = 2 * W, DSY = 3 * W, S0Z = 4 * W, DSZ = 5 * W, CQ = 6 * W,
-                         ORG = 6 * W + 3;
+                         ORG = 6 * W + 1;
+    static_assert(ORG < FLAG, "slow record overlaps the flag");
 };
 
-// Called by the owning lane only.
+// Written by the owning lane (all slow lanes of a chunk in parallel, each into its own slot).
 template <int N>
 __device__ __forceinline__ void slow_write(double* rec, const Grid& g, double xi0, double et0, double ze0,
                                            double xi1, double et1, double ze1, double qw, double inv_dt) {
     using R = SlowRec<N>;
     constexpr int W = R::W;
-    double s0[W], ds[W];
-    bool bad = false;
-    const int nx0 = shapes_pair<N>(xi0, xi1, s0, ds, bad);
+    long long o = 0;
+#pragma unroll 1
+    for (int d = 0; d < 3; ++d) {
+        const double a0 = (d == 0) ? xi0 : ((d == 1) ? et0 : ze0);
+        const double a1 = (d == 0) ? xi1 : ((d == 1) ? et1 : ze1);
+        const long long stride = (d == 0) ? 1 : ((d == 1) ? g.sy : g.sz);
+        double s0[W], ds[W];
+        bool bad = false;
+        const int n0 = shapes_pair<N>(a0, a1, s0, ds, bad);
+        double* r = rec + 2 * W * d;
 #pragma unroll
-    for (int a = 0; a < W; ++a) { rec[R::S0X + a] = s0[a]; rec[R::DSX + a] = ds[a]; }
-    const int ny0 = shapes_pair<N>(et0, et1, s0, ds, bad);
-#pragma unroll
-    for (int a = 0; a < W; ++a) { rec[R::S0Y + a] = s0[a]; rec[R::DSY + a] = ds[a]; }
-    const int nz0 = shapes_pair<N>(ze0, ze1, s0, ds, bad);
-#pragma unroll
-    for (int a = 0; a < W; ++a) { rec[R::S0Z + a] = s0[a]; rec[R::DSZ + a] = ds[a]; }
-    rec[R::CQ + 0] = -qw * inv_dt * g.inv_dy * g.inv_dz;
-    rec[R::CQ + 1] = -qw * inv_dt * g.inv_dx * g.inv_dz;
-    rec[R::CQ + 2] = -qw * inv_dt * g.inv_dx * g.inv_dy;
-    rec[R::ORG] = __longlong_as_double(g.idx(nx0, ny0, nz0));   // window nodes stay inside the guard shell
+        for (int a = 0; a < W; ++a) { r[a] = s0[a]; r[W + a] = ds[a]; }
+        o += stride * (long long)(n0 + NG);     // window nodes stay inside the guard shell
+    }
+    rec[R::CQ] = -qw * inv_dt;
+    rec[R::ORG] = __longlong_as_double(o);
+    rec[FLAG] = REC_SLOW;
 }
 
 // Called by all 32 lanes: lane <-> one (u,v) pair of the window's cross-section; W-1 points along the
 // prefix direction each.  Jx = cqx prefix_a(DSx) (S0y Az + DSy Bz), A = S0 + DS/2, B = S0/2 + DS/3, and
-// cyclic permutations.
+// cyclic permutations.  Rolled over the three components.
 template <int N>
 __device__ __forceinline__ void slow_deposit(const double* rec, const Grid& g, const Fields& f, int lane) {
     using R = SlowRec<N>;
@@ -196,49 +245,27 @@ __device__ __forceinline__ void slow_deposit(const double* rec, const Grid& g, c
     if (lane >= W * W) return;
     const int u = lane % W, v = lane / W;
     const long long o0 = __double_as_longlong(rec[R::ORG]);
+    const double cq0 = rec[R::CQ];
     const double third = 1.0 / 3.0;
-    {   // Jx: (u,v) = (b,c)
-        const double s0z = rec[R::S0Z + v], dsz = rec[R::DSZ + v];
-        const double t = rec[R::S0Y + u] * (s0z + 0.5 * dsz) + rec[R::DSY + u] * (0.5 * s0z + third * dsz);
+#pragma unroll 1
+    for (int d = 0; d < 3; ++d) {
+        // component d: prefix along d; (u,v) run over the other two dimensions (e1 < e2)
+        const int e1 = (d == 0) ? 1 : 0, e2 = (d == 2) ? 1 : 2;
+        const long long sd = (d == 0) ? 1 : ((d == 1) ? g.sy : g.sz);
+        const long long s1 = (e1 == 0) ? 1 : g.sy, s2 = (e2 == 1) ? g.sy : g.sz;
+        const double a2 = rec[2 * W * e2 + v], b2 = rec[2 * W * e2 + W + v];
+        const double t = rec[2 * W * e1 + u] * (a2 + 0.5 * b2) + rec[2 * W * e1 + W + u] * (0.5 * a2 + third * b2);
         if (t != 0.0) {
-            const double cq = rec[R::CQ + 0];
-            double* dst = f.Jx + o0 + g.sy * u + g.sz * v;
+            const double cq = cq0 * ((d == 0) ? g.inv_dy * g.inv_dz : ((d == 1) ? g.inv_dx * g.inv_dz
+                                                                                 : g.inv_dx * g.inv_dy));
+            double* dst = ((d == 0) ? f.Jx : ((d == 1) ? f.Jy : f.Jz)) + o0 + s1 * u + s2 * v;
+            const double* dsd = rec + 2 * W * d + W;
             double acc = 0.0;
 #pragma unroll
             for (int a = 0; a < W - 1; ++a) {
-                acc += rec[R::DSX + a];
+                acc += dsd[a];
                 const double val = (cq * acc) * t;
-                if (val != 0.0) atomicAdd(dst + a, val);
-            }
-        }
-    }
-    {   // Jy: (u,v) = (a,c)
-        const double s0z = rec[R::S0Z + v], dsz = rec[R::DSZ + v];
-        const double t = rec[R::S0X + u] * (s0z + 0.5 * dsz) + rec[R::DSX + u] * (0.5 * s0z + third * dsz);
-        if (t != 0.0) {
-            const double cq = rec[R::CQ + 1];
-            double* dst = f.Jy + o0 + u + g.sz * v;
-            double acc = 0.0;
-#pragma unroll
-            for (int b = 0; b < W - 1; ++b) {
-                acc += rec[R::DSY + b];
-                const double val = (cq * acc) * t;
-                if (val != 0.0) atomicAdd(dst + g.sy * b, val);
-            }
-        }
-    }
-    {   // Jz: (u,v) = (a,b)
-        const double s0y = rec[R::S0Y + v], dsy = rec[R::DSY + v];
-        const double t = rec[R::S0X + u] * (s0y + 0.5 * dsy) + rec[R::DSX + u] * (0.5 * s0y + third * dsy);
-        if (t != 0.0) {
-            const double cq = rec[R::CQ + 2];
-            double* dst = f.Jz + o0 + u + g.sy * v;
-            double acc = 0.0;
-#pragma unroll
-            for (int c = 0; c < W - 1; ++c) {
-                acc += rec[R::DSZ + c];
-                const double val = (cq * acc) * t;
-                if (val != 0.0) atomicAdd(dst + g.sz * c, val);
+                if (val != 0.0) red_add(dst + sd * a, val);
             }
         }
     }
@@ -246,87 +273,121 @@ __device__ __forceinline__ void slow_deposit(const double* rec, const Grid& g, c
 
 // ---- fast path: per-(cell, plane) register accumulators --------------------------------------
 // Staging slot layout (FW = window nodes): s0x dsx s0y dsy s0z dsz (FW each), then pdx pdy pdz
-// (FW-1 each) with pd_d[a] = cq_d * sum_{a' <= a} ds_d[a'].
+// (FW-1 each) with pd_d[a] = cq_d * sum_{a' <= a} ds_d[a'].  At FW = 4: 33 doubles + the flag.
 template <int N>
 struct FastRec {
     static constexpr int FW = FastWin<N>::FW;
     static constexpr int S0X = 0, DSX = FW, S0Y = 2 * FW, DSY = 3 * FW, S0Z = 4 * FW, DSZ = 5 * FW, PDX = 6 * FW,
                          PDY = 6 * FW + (FW - 1), PDZ = 6 * FW + 2 * (FW - 1), LEN = 6 * FW + 3 * (FW - 1);
+    static_assert(LEN <= FLAG, "fast record overlaps the flag");
 };
 
 template <int N>
 struct CellAcc {
     static constexpr int FW = FastWin<N>::FW;
-    double jx[FW - 1][FW];   // Jx[a][b] on plane c = s
-    double jy[FW][FW - 1];   // Jy[a][b] on plane c = s
-    double jz[FW][FW - 1];   // Jz[a][c] on row   b = s
+    static constexpr int NACC = 3 * FW * (FW - 1);
+    double jx[FW][FW - 1];   // Jx[b][a] on plane c = s
+    double jy[FW - 1][FW];   // Jy[b][a] on plane c = s
+    double jz[FW - 1][FW];   // Jz[c][a] on row   b = s
     __device__ __forceinline__ void clear() {
 #pragma unroll
-        for (int a = 0; a < FW - 1; ++a)
+        for (int b = 0; b < FW; ++b)
 #pragma unroll
-            for (int b = 0; b < FW; ++b) jx[a][b] = 0.0;
-#pragma unroll
-        for (int a = 0; a < FW; ++a)
-#pragma unroll
-            for (int b = 0; b < FW - 1; ++b) { jy[a][b] = 0.0; jz[a][b] = 0.0; }
+            for (int a = 0; a < FW - 1; ++a) { jx[b][a] = 0.0; jy[a][b] = 0.0; jz[a][b] = 0.0; }
     }
-    // one staged particle; s = this lane's plane
-    __device__ __forceinline__ void add(const double* __restrict__ r, int s) {
+    // one staged particle; s = this lane's plane.  Returns false for a record that is not fast.
+    __device__ __forceinline__ bool add(const double* __restrict__ r, int s) {
         using R = FastRec<N>;
         const double third = 1.0 / 3.0;
+        double s0x[FW], dsx[FW], s0y[FW], dsy[FW], pdx[FW - 1], pdy[FW - 1], pdz[FW - 1];
+        if constexpr (FW == 4) {
+            const double2 tail = ld2(r, 32);                  // pdz[2], flag
+            if (tail.y != REC_FAST) return false;
+            double2 v;
+            v = ld2(r, R::S0X); s0x[0] = v.x; s0x[1] = v.y; v = ld2(r, R::S0X + 2); s0x[2] = v.x; s0x[3] = v.y;
+            v = ld2(r, R::DSX); dsx[0] = v.x; dsx[1] = v.y; v = ld2(r, R::DSX + 2); dsx[2] = v.x; dsx[3] = v.y;
+            v = ld2(r, R::S0Y); s0y[0] = v.x; s0y[1] = v.y; v = ld2(r, R::S0Y + 2); s0y[2] = v.x; s0y[3] = v.y;
+            v = ld2(r, R::DSY); dsy[0] = v.x; dsy[1] = v.y; v = ld2(r, R::DSY + 2); dsy[2] = v.x; dsy[3] = v.y;
+            v = ld2(r, 24); pdx[0] = v.x; pdx[1] = v.y;
+            v = ld2(r, 26); pdx[2] = v.x; pdy[0] = v.y;
+            v = ld2(r, 28); pdy[1] = v.x; pdy[2] = v.y;
+            v = ld2(r, 30); pdz[0] = v.x; pdz[1] = v.y;
+            pdz[2] = tail.x;
+        } else {
+            if (r[FLAG] != REC_FAST) return false;
+#pragma unroll
+            for (int a = 0; a < FW; ++a) {
+                s0x[a] = r[R::S0X + a]; dsx[a] = r[R::DSX + a]; s0y[a] = r[R::S0Y + a]; dsy[a] = r[R::DSY + a];
+            }
+#pragma unroll
+            for (int a = 0; a < FW - 1; ++a) { pdx[a] = r[R::PDX + a]; pdy[a] = r[R::PDY + a]; pdz[a] = r[R::PDZ + a]; }
+        }
         const double s0z = r[R::S0Z + s], dsz = r[R::DSZ + s];
         const double az = s0z + 0.5 * dsz, bz = 0.5 * s0z + third * dsz;
         const double s0ys = r[R::S0Y + s], dsys = r[R::DSY + s];
         const double ay = s0ys + 0.5 * dsys, by = 0.5 * s0ys + third * dsys;
-        double pd[FW - 1];
-#pragma unroll
-        for (int a = 0; a < FW - 1; ++a) pd[a] = r[R::PDX + a];
 #pragma unroll
         for (int b = 0; b < FW; ++b) {
-            const double t = r[R::S0Y + b] * az + r[R::DSY + b] * bz;
+            const double t = s0y[b] * az + dsy[b] * bz;
 #pragma unroll
-            for (int a = 0; a < FW - 1; ++a) jx[a][b] = fma(pd[a], t, jx[a][b]);
+            for (int a = 0; a < FW - 1; ++a) jx[b][a] = fma(pdx[a], t, jx[b][a]);
         }
-        double s0x[FW], dsx[FW];
-#pragma unroll
-        for (int a = 0; a < FW; ++a) { s0x[a] = r[R::S0X + a]; dsx[a] = r[R::DSX + a]; }
-#pragma unroll
-        for (int b = 0; b < FW - 1; ++b) pd[b] = r[R::PDY + b];
 #pragma unroll
         for (int a = 0; a < FW; ++a) {
             const double t = s0x[a] * az + dsx[a] * bz;
 #pragma unroll
-            for (int b = 0; b < FW - 1; ++b) jy[a][b] = fma(pd[b], t, jy[a][b]);
+            for (int b = 0; b < FW - 1; ++b) jy[b][a] = fma(pdy[b], t, jy[b][a]);
         }
-#pragma unroll
-        for (int c = 0; c < FW - 1; ++c) pd[c] = r[R::PDZ + c];
 #pragma unroll
         for (int a = 0; a < FW; ++a) {
             const double t = s0x[a] * ay + dsx[a] * by;
 #pragma unroll
-            for (int c = 0; c < FW - 1; ++c) jz[a][c] = fma(pd[c], t, jz[a][c]);
+            for (int c = 0; c < FW - 1; ++c) jz[c][a] = fma(pdz[c], t, jz[c][a]);
         }
+        return true;
     }
-    // add to the padded global arrays; o = offset of the window's first node, s = this lane's plane
-    __device__ __forceinline__ void flush(const Grid& g, const Fields& f, long long o, int s) const {
-        double* px = f.Jx + o + g.sz * s;
-        double* py = f.Jy + o + g.sz * s;
-        double* pz = f.Jz + o + g.sy * s;
+    // Add to the padded global arrays.  o = offset of the window's first node, s = this lane's plane,
+    // buf = NACC x 32 doubles of warp-private shared memory (lane-interleaved).  The accumulators are
+    // spilled there once so that the RED loops can stay rolled (short code, I-cache resident).
+    __device__ __forceinline__ void flush(const Grid& g, const Fields& f, long long o, int s, double* buf,
+                                          int lane) const {
+        double* mine = buf + lane;
 #pragma unroll
         for (int b = 0; b < FW; ++b)
 #pragma unroll
-            for (int a = 0; a < FW - 1; ++a)
-                if (jx[a][b] != 0.0) atomicAdd(px + a + g.sy * b, jx[a][b]);
+            for (int a = 0; a < FW - 1; ++a) mine[32 * (b * (FW - 1) + a)] = jx[b][a];
 #pragma unroll
         for (int b = 0; b < FW - 1; ++b)
 #pragma unroll
-            for (int a = 0; a < FW; ++a)
-                if (jy[a][b] != 0.0) atomicAdd(py + a + g.sy * b, jy[a][b]);
+            for (int a = 0; a < FW; ++a) {
+                mine[32 * (FW * (FW - 1) + b * FW + a)] = jy[b][a];
+                mine[32 * (2 * FW * (FW - 1) + b * FW + a)] = jz[b][a];
+            }
+        double* pr = f.Jx + o + g.sz * s;
+        const double* src = mine;
+#pragma unroll 1
+        for (int b = 0; b < FW; ++b, pr += g.sy, src += 32 * (FW - 1))
 #pragma unroll
-        for (int c = 0; c < FW - 1; ++c)
+            for (int a = 0; a < FW - 1; ++a) {
+                const double v = src[32 * a];
+                if (v != 0.0) red_add(pr + a, v);
+            }
+        pr = f.Jy + o + g.sz * s;
+#pragma unroll 1
+        for (int b = 0; b < FW - 1; ++b, pr += g.sy, src += 32 * FW)
 #pragma unroll
-            for (int a = 0; a < FW; ++a)
-                if (jz[a][c] != 0.0) atomicAdd(pz + a + g.sz * c, jz[a][c]);
+            for (int a = 0; a < FW; ++a) {
+                const double v = src[32 * a];
+                if (v != 0.0) red_add(pr + a, v);
+            }
+        pr = f.Jz + o + g.sy * s;
+#pragma unroll 1
+        for (int c = 0; c < FW - 1; ++c, pr += g.sz, src += 32 * FW)
+#pragma unroll
+            for (int a = 0; a < FW; ++a) {
+                const double v = src[32 * a];
+                if (v != 0.0) red_add(pr + a, v);
+            }
     }
 };
 
@@ -340,6 +401,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                       int ntx, int nty, DevStatus* status) {
     constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA;
     using FR = FastRec<N>;
+    static_assert(CellAcc<N>::NACC * 32 <= C::STG_W, "flush buffer does not fit the staging area");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* Et = reinterpret_cast<double*>(smem_raw);            // 6 * ESZ: Ex Ey Ez Bx By Bz
     double* stg_all = Et + 6 * C::ESZ;                           // NW * STG_W
@@ -402,148 +464,132 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
         const int cell_lo = off[bq], cell_hi = off[bq + 1];  // phase B: this lane's cell
         CellAcc<N> acc;
         acc.clear();
-        bool touched = false;
 
-        for (int base = row_lo; base < row_hi; base += 32) {
-            // ---------------- phase A: lane <-> particle ------------------------------------------
-            const int ip = base + lane;
-            const bool active = ip < row_hi;
-            bool is_slow = false;
-            double xi = 0.0, et = 0.0, ze = 0.0, xi1 = 0.0, et1 = 0.0, ze1 = 0.0, qw = 0.0;
-            if (active) {
-                const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
-                double ux = p.ux[ip], uy = p.uy[ip], uz = p.uz[ip];
-                qw = q * p.w[ip];
-                xi = (x - g.xmin) * g.inv_dx; et = (y - g.ymin) * g.inv_dy; ze = (z - g.zmin) * g.inv_dz;
-                const int ci = __double2int_rd(xi), cj = __double2int_rd(et), ck = __double2int_rd(ze);
-                const int rx = rel_cell(ci, t0x, C::TX, g.nx), ry = rel_cell(cj, t0y, C::TY, g.ny),
-                          rz = rel_cell(ck, t0z, C::TZ, g.nz);
-                const bool in_tile = rx >= -DRIFT && rx <= C::TX - 1 + DRIFT && t0x + rx <= g.nx - 1 + DRIFT &&
-                                     ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
-                                     rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
-                double wxn[N + 1], wyn[N + 1], wzn[N + 1];
-                const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn),
-                          fzn = shape_weights<N>(ze, wzn);
-                double eb[6];
-                if (in_tile) {
-                    double wxs[N + 1], wys[N + 1], wzs[N + 1];
-                    // first nodes, shifted from global node index to tile slot: slot = node - (t0 - GL) + image shift
-                    const int shx = (rx - (ci - t0x)) + C::GL - t0x, shy = (ry - (cj - t0y)) + C::GL - t0y,
-                              shz = (rz - (ck - t0z)) + C::GL - t0z;
-                    const int fxs = shape_weights<N>(xi - 0.5, wxs) + shx, fys = shape_weights<N>(et - 0.5, wys) + shy,
-                              fzs = shape_weights<N>(ze - 0.5, wzs) + shz;
-                    const int gxn = fxn + shx, gyn = fyn + shy, gzn = fzn + shz;
-                    eb[0] = gather_tile<N, C>(Et + 0 * C::ESZ, fxs, gyn, gzn, wxs, wyn, wzn);
-                    eb[1] = gather_tile<N, C>(Et + 1 * C::ESZ, gxn, fys, gzn, wxn, wys, wzn);
-                    eb[2] = gather_tile<N, C>(Et + 2 * C::ESZ, gxn, gyn, fzs, wxn, wyn, wzs);
-                    eb[3] = gather_tile<N, C>(Et + 3 * C::ESZ, gxn, fys, fzs, wxn, wys, wzs);
-                    eb[4] = gather_tile<N, C>(Et + 4 * C::ESZ, fxs, gyn, fzs, wxs, wyn, wzs);
-                    eb[5] = gather_tile<N, C>(Et + 5 * C::ESZ, fxs, fys, gzn, wxs, wys, wzn);
-                } else {
-                    gather_global6<N>(g, f, xi, et, ze, eb);
-                    ++n_glob;
+        for (int base = row_lo; base < row_hi; base += C::CHUNK) {
+            // ---------------- phase A: lane <-> particle, 32 at a time ---------------------------
+#pragma unroll 1
+            for (int sub = 0; sub < C::CHUNK; sub += 32) {
+                const int ip = base + sub + lane;
+                if (base + sub >= row_hi) break;
+                double* rec = stg + skew(sub + lane) * C::PITCH;
+                bool is_slow = false;
+                if (ip < row_hi) {
+                    const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
+                    double ux = p.ux[ip], uy = p.uy[ip], uz = p.uz[ip];
+                    const double qw = q * p.w[ip];
+                    const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy,
+                                 ze = (z - g.zmin) * g.inv_dz;
+                    const int ci = __double2int_rd(xi), cj = __double2int_rd(et), ck = __double2int_rd(ze);
+                    const int rx = rel_cell(ci, t0x, C::TX, g.nx), ry = rel_cell(cj, t0y, C::TY, g.ny),
+                              rz = rel_cell(ck, t0z, C::TZ, g.nz);
+                    const bool in_tile = rx >= -DRIFT && rx <= C::TX - 1 + DRIFT && t0x + rx <= g.nx - 1 + DRIFT &&
+                                         ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
+                                         rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
+                    double wxn[N + 1], wyn[N + 1], wzn[N + 1];
+                    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn),
+                              fzn = shape_weights<N>(ze, wzn);
+                    double eb[6];
+                    if (in_tile) {
+                        double wxs[N + 1], wys[N + 1], wzs[N + 1];
+                        // first nodes, from global node index to tile slot: slot = node - (t0 - GL) + image shift
+                        const int shx = (rx - (ci - t0x)) + C::GL - t0x, shy = (ry - (cj - t0y)) + C::GL - t0y,
+                                  shz = (rz - (ck - t0z)) + C::GL - t0z;
+                        const int fxs = shape_weights<N>(xi - 0.5, wxs) + shx,
+                                  fys = shape_weights<N>(et - 0.5, wys) + shy,
+                                  fzs = shape_weights<N>(ze - 0.5, wzs) + shz;
+                        gather6_tile<N, C>(Et, fxn + shx, fyn + shy, fzn + shz, fxs, fys, fzs, wxn, wyn, wzn, wxs,
+                                           wys, wzs, eb);
+                    } else {
+                        gather_global6<N>(g, f, xi, et, ze, eb);
+                        ++n_glob;
+                    }
+                    boris_push(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
+                    const double gam = sqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
+                    const double x1 = x + g.dt * ux / gam, y1 = y + g.dt * uy / gam, z1 = z + g.dt * uz / gam;
+                    const double xi1 = (x1 - g.xmin) * g.inv_dx, et1 = (y1 - g.ymin) * g.inv_dy,
+                                 ze1 = (z1 - g.zmin) * g.inv_dz;
+                    const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
+                                     !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
+                    bad_any = bad_any || bad;
+                    p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
+                    p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
+                    p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
+                    p.ux[ip] = ux;
+                    p.uy[ip] = uy;
+                    p.uz[ip] = uz;
+                    // ---- classify: fast = stayed inside the cell the sort listed it in -------------
+                    int lc = 0;
+#pragma unroll
+                    for (int c = 1; c < C::TX; ++c) lc += (off[c] <= ip) ? 1 : 0;
+                    const bool same = __double2int_rd(xi1) == ci && __double2int_rd(et1) == cj &&
+                                      __double2int_rd(ze1) == ck;
+                    const bool listed = in_tile && rx == lc && ry == ry0 && rz == rz0;
+                    const bool deposits = !bad && qw != 0.0;
+                    const bool fast = deposits && same && listed;
+                    is_slow = deposits && !fast;
+                    if (in_tile) { if (is_slow) ++n_slow; else ++n_fast; }
+                    if (fast) {
+                        // ---- fast record: old/new shapes on the cell's window, prefix-summed factors --
+                        double fr[FLAG + 1];
+#pragma unroll
+                        for (int k = 0; k <= FLAG; ++k) fr[k] = 0.0;
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) {
+                            const double a1 = (d == 0) ? xi1 : ((d == 1) ? et1 : ze1);
+                            const int cell = (d == 0) ? ci : ((d == 1) ? cj : ck);
+                            const int f0 = (d == 0) ? fxn : ((d == 1) ? fyn : fzn);
+                            const double (&w0)[N + 1] = (d == 0) ? wxn : ((d == 1) ? wyn : wzn);
+                            const double area = (d == 0) ? g.inv_dy * g.inv_dz
+                                                         : ((d == 1) ? g.inv_dx * g.inv_dz : g.inv_dx * g.inv_dy);
+                            double w1[N + 1], s0[FW], s1[FW];
+                            const int f1 = shape_weights<N>(a1, w1);
+                            to_fast_window<N>(w0, f0, cell + FA, s0);
+                            to_fast_window<N>(w1, f1, cell + FA, s1);
+                            const double cq = (-qw * inv_dt) * area;
+                            double run = 0.0;
+#pragma unroll
+                            for (int a = 0; a < FW; ++a) {
+                                const double dd = s1[a] - s0[a];
+                                fr[2 * FW * d + a] = s0[a];
+                                fr[2 * FW * d + FW + a] = dd;
+                                run += dd;
+                                if (a < FW - 1) fr[FR::PDX + (FW - 1) * d + a] = cq * run;
+                            }
+                        }
+                        fr[FLAG] = REC_FAST;
+#pragma unroll
+                        for (int k = 0; k < (FR::LEN + 1) / 2; ++k) st2(rec, 2 * k, fr[2 * k], fr[2 * k + 1]);
+                        if ((FR::LEN + 1) / 2 <= FLAG / 2) st2(rec, FLAG - 1, 0.0, REC_FAST);
+                    } else if (is_slow) {
+                        slow_write<N>(rec, g, xi, et, ze, xi1, et1, ze1, qw, inv_dt);
+                    } else {
+                        rec[FLAG] = REC_NONE;
+                    }
                 }
-                boris_push(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
-                const double gam = sqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
-                const double x1 = x + g.dt * ux / gam, y1 = y + g.dt * uy / gam, z1 = z + g.dt * uz / gam;
-                xi1 = (x1 - g.xmin) * g.inv_dx; et1 = (y1 - g.ymin) * g.inv_dy; ze1 = (z1 - g.zmin) * g.inv_dz;
-                const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
-                                 !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
-                bad_any = bad_any || bad;
-                p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
-                p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
-                p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
-                p.ux[ip] = ux;
-                p.uy[ip] = uy;
-                p.uz[ip] = uz;
-                // ---- classify: fast = stayed inside the cell the sort listed it in -------------
-                int lc = 0;
-#pragma unroll
-                for (int c = 1; c < C::TX; ++c) lc += (off[c] <= ip) ? 1 : 0;
-                const bool same = __double2int_rd(xi1) == ci && __double2int_rd(et1) == cj &&
-                                  __double2int_rd(ze1) == ck;
-                const bool listed = in_tile && rx == lc && ry == ry0 && rz == rz0;
-                const bool deposits = !bad && qw != 0.0;
-                const bool fast = deposits && same && listed;
-                is_slow = deposits && !fast;
-                if (in_tile) { if (is_slow) ++n_slow; else ++n_fast; }
-                // ---- stage the fast record (zeros when the particle is not fast) ---------------
-                double* r = stg + skew(lane) * C::PITCH;
-                {
-                    double w1[N + 1], s0[FW], s1[FW];
-                    int f1;
-                    double cq, run;
-                    // x
-                    f1 = shape_weights<N>(xi1, w1);
-                    to_fast_window<N>(wxn, fxn, ci + FA, s0);
-                    to_fast_window<N>(w1, f1, ci + FA, s1);
-                    cq = fast ? -qw * inv_dt * g.inv_dy * g.inv_dz : 0.0;
-                    run = 0.0;
-#pragma unroll
-                    for (int a = 0; a < FW; ++a) {
-                        const double d = s1[a] - s0[a];
-                        r[FR::S0X + a] = fast ? s0[a] : 0.0;
-                        r[FR::DSX + a] = fast ? d : 0.0;
-                        run += d;
-                        if (a < FW - 1) r[FR::PDX + a] = fast ? cq * run : 0.0;
-                    }
-                    // y
-                    f1 = shape_weights<N>(et1, w1);
-                    to_fast_window<N>(wyn, fyn, cj + FA, s0);
-                    to_fast_window<N>(w1, f1, cj + FA, s1);
-                    cq = fast ? -qw * inv_dt * g.inv_dx * g.inv_dz : 0.0;
-                    run = 0.0;
-#pragma unroll
-                    for (int a = 0; a < FW; ++a) {
-                        const double d = s1[a] - s0[a];
-                        r[FR::S0Y + a] = fast ? s0[a] : 0.0;
-                        r[FR::DSY + a] = fast ? d : 0.0;
-                        run += d;
-                        if (a < FW - 1) r[FR::PDY + a] = fast ? cq * run : 0.0;
-                    }
-                    // z
-                    f1 = shape_weights<N>(ze1, w1);
-                    to_fast_window<N>(wzn, fzn, ck + FA, s0);
-                    to_fast_window<N>(w1, f1, ck + FA, s1);
-                    cq = fast ? -qw * inv_dt * g.inv_dx * g.inv_dy : 0.0;
-                    run = 0.0;
-#pragma unroll
-                    for (int a = 0; a < FW; ++a) {
-                        const double d = s1[a] - s0[a];
-                        r[FR::S0Z + a] = fast ? s0[a] : 0.0;
-                        r[FR::DSZ + a] = fast ? d : 0.0;
-                        run += d;
-                        if (a < FW - 1) r[FR::PDZ + a] = fast ? cq * run : 0.0;
-                    }
+                __syncwarp();
+                // ---------------- slow path: one particle at a time, whole warp ---------------------
+                unsigned int slow_mask = __ballot_sync(0xffffffffu, is_slow);
+                while (slow_mask) {
+                    const int L = __ffs(slow_mask) - 1;
+                    slow_mask &= slow_mask - 1;
+                    slow_deposit<N>(stg + skew(sub + L) * C::PITCH, g, f, lane);
                 }
             }
-            __syncwarp();
             // ---------------- phase B: lane <-> (cell, plane) ------------------------------------
             {
-                const int lo = max(cell_lo, base), hi = min(cell_hi, base + 32);
+                const int lo = max(cell_lo, base), hi = min(cell_hi, base + C::CHUNK);
                 const int len = (bs < FW) ? hi - lo : 0;
                 const int maxlen = __reduce_max_sync(0xffffffffu, max(len, 0));
-                for (int t = 0; t < maxlen; ++t) {
-                    if (t < len) {
-                        acc.add(stg + skew(lo + t - base) * C::PITCH, bs);
-                        touched = true;
-                    }
-                }
+                const double* r0 = stg;
+#pragma unroll 1
+                for (int t = 0; t < maxlen; ++t)
+                    if (t < len) acc.add(r0 + skew(lo + t - base) * C::PITCH, bs);
             }
             __syncwarp();
-            // ---------------- slow path: one particle at a time, whole warp ---------------------
-            unsigned int slow_mask = __ballot_sync(0xffffffffu, is_slow);
-            while (slow_mask) {
-                const int L = __ffs(slow_mask) - 1;
-                slow_mask &= slow_mask - 1;
-                if (lane == L) slow_write<N>(stg, g, xi, et, ze, xi1, et1, ze1, qw, inv_dt);
-                __syncwarp();
-                slow_deposit<N>(stg, g, f, lane);
-                __syncwarp();
-            }
         }
         // ---------------- flush the row's accumulators ---------------------------------------------
-        if (touched) acc.flush(g, f, g.idx(t0x + bq + FA, t0y + ry0 + FA, t0z + rz0 + FA), bs);
+        if (bs < FW) acc.flush(g, f, g.idx(t0x + bq + FA, t0y + ry0 + FA, t0z + rz0 + FA), bs, stg, lane);
+        __syncwarp();
     }
     // ---- flags and counters ----------------------------------------------------------------------
     if (bad_any) status->ephys = 1;
