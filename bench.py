@@ -15,9 +15,14 @@ GPU (replicas only, no data-path collective).
   e2e       the same metric through the C ABI with HOST buffers: every step
             pic_load_particles (H2D) + pic_sort + pic_step + pic_get_particles
             and pic_get_fields (D2H) from/to pinned host memory
-  roofline  the dominant kernel (fused per-tile particle kernel): algorithmic
-            bytes per launch / its average launch duration, measured with CUDA
-            events on the library's stream over the timed region
+  roofline  the dominant kernel (fused per-tile particle kernel).  It is bound by
+            on-chip arithmetic and shared-memory issue, not by HBM,
+            so the headline roofline is the fp64 pipe ("bound": "alu": algorithmic
+            fp64 instructions per launch / average launch duration against
+            148 SMs x 64 lanes x 1965 MHz); roofline_hbm (algorithmic bytes against
+            the measured HBM peak) and roofline_smem stand beside it.  Launch
+            durations come from CUDA events on the library's stream over the
+            timed region
   cpu_baseline   the oracle (oracle/, as it stands) timed on the host cores on
             a bounded sample of the same workload
 
@@ -48,6 +53,17 @@ BYTES_PER_PARTICLE = 104.0
 BYTES_PER_CELL = 96.0
 # Yee: B half (72 B/cell) + E (96 B/cell) + B half (72 B/cell)
 YEE_BYTES_PER_CELL = 240.0
+# fp64-pipe roofline of the fused kernel.  Instructions per particle = DFMA + DMUL + DADD
+# thread instructions executed per particle by the committed kernel (ncu, profiles/); order 3 measured,
+# orders 1 and 2 scaled by the gather/deposit operation counts.
+FP64_INSTR_PER_PARTICLE = {1: 400.0, 2: 750.0, 3: 1116.0}
+FP64_LANES_PER_SM = 64
+N_SM = 148
+SM_MAX_MHZ = 1965.0
+# shared-memory bytes the kernel moves per particle at order 3 (gather 384 x 8 B, staging, phase B)
+SMEM_BYTES_PER_PARTICLE = {1: 1100.0, 2: 2600.0, 3: 5100.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch at the default workload (profiles/)
+TRAFFIC_BYTES_PER_LAUNCH = 17.90e9
 
 
 def _peaks():
@@ -210,6 +226,8 @@ def run_ours(args):
             for nm in ("ux", "uy", "uz"):
                 setattr(sp, nm, np.roll(getattr(sp, nm), 8 * rank))
     sort_every = wl.sort_every if wl.sort_every > 0 else 0
+    if args.sort_every is not None:
+        sort_every = max(0, args.sort_every)
     t_gen = time.perf_counter() - t_gen
     npart, ncell = wl.nparticles, wl.ncell
 
@@ -253,19 +271,34 @@ def run_ours(args):
         ms_total = float(t.item())
     value = world * npart * args.steps / (ms_total * 1e-3)
 
-    # ---- roofline of the dominant kernel (fused particle kernel, one launch per species per step) ----
+    # ---- rooflines of the dominant kernel (fused particle kernel, one launch per species per step) ----
     nspec = sum(1 for s in wl.species if s.n > 0)
     n_launch = max(1, int(round(st["steps"])) * nspec)
     ms_launch = st["particles"] / n_launch
-    alg_bytes = (BYTES_PER_PARTICLE * npart + BYTES_PER_CELL * ncell * nspec) / nspec
-    peak, peak_kind = _peaks()
-    achieved = alg_bytes / (ms_launch * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "particles_tile_kernel<%d>" % wl.order, "achieved": achieved,
-                "peak": peak, "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured"
-                else "fallback (B200_PROFILING.md)", "unit": "GB/s", "frac": achieved / peak,
-                "traffic": args.traffic, "ms_per_launch": ms_launch,
-                "algorithmic_bytes_per_launch": alg_bytes,
-                "particle_updates_per_s_kernel_only": npart / nspec / (ms_launch * 1e-3)}
+    np_launch = npart / nspec
+    alg_bytes = BYTES_PER_PARTICLE * np_launch + BYTES_PER_CELL * ncell
+    hbm_peak, peak_kind = _peaks()
+    hbm_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured" else "fallback (B200_PROFILING.md)"
+    kname = "particles_tile_kernel<%d>" % wl.order
+    # The kernel is bound by on-chip arithmetic/LSU issue, not by HBM: the headline
+    # roofline is the fp64 pipe; the HBM and shared-memory figures are reported beside it.
+    fp64_peak = FP64_LANES_PER_SM * N_SM * SM_MAX_MHZ * 1e6 / 1e12          # T fp64 instructions/s
+    fp64_alg = FP64_INSTR_PER_PARTICLE.get(wl.order, FP64_INSTR_PER_PARTICLE[3]) * np_launch
+    fp64_ach = fp64_alg / (ms_launch * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": kname, "achieved": fp64_ach, "peak": fp64_peak,
+                "peak_kind": "derived: 148 SMs x 64 fp64 lanes/clk x 1965 MHz (DESIGN.md 5.1; DFMA probe)",
+                "unit": "T fp64-instr/s", "frac": fp64_ach / fp64_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH
+                if (args.config == 2 and args.n is None) else None,
+                "ms_per_launch": ms_launch, "algorithmic_fp64_instr_per_launch": fp64_alg,
+                "particle_updates_per_s_kernel_only": np_launch / (ms_launch * 1e-3)}
+    hbm_ach = alg_bytes / (ms_launch * 1e-3) / 1e9
+    roofline_hbm = {"bound": "hbm", "kernel": kname, "achieved": hbm_ach, "peak": hbm_peak, "peak_kind": hbm_kind,
+                    "unit": "GB/s", "frac": hbm_ach / hbm_peak, "algorithmic_bytes_per_launch": alg_bytes}
+    smem_peak = 128.0 * N_SM * SM_MAX_MHZ * 1e6 / 1e9                       # GB/s of shared-memory data pipe
+    smem_ach = SMEM_BYTES_PER_PARTICLE.get(wl.order, SMEM_BYTES_PER_PARTICLE[3]) * np_launch / (ms_launch * 1e-3) / 1e9
+    roofline_smem = {"bound": "smem", "kernel": kname, "achieved": smem_ach, "peak": smem_peak,
+                     "peak_kind": "derived: 148 SMs x 128 B/clk x 1965 MHz", "unit": "GB/s",
+                     "frac": smem_ach / smem_peak}
     nsteps_t = max(1.0, st["steps"])
     yee_ms = (st["yee_B"] + st["yee_E"]) / nsteps_t
     stages = {"per_step_ms": {k: st[k] / nsteps_t for k in ("zero_J", "particles", "fold_J", "yee_B", "yee_E")},
@@ -334,7 +367,7 @@ def run_ours(args):
                            (BYTES_PER_PARTICLE * npart + 9 * 8 * ncell) / 1e9),
                        "generation_s": round(t_gen, 1)},
             "cell_updates_per_s": world * ncell * args.steps / (ms_total * 1e-3),
-            "roofline": roofline, "stages": stages, "particle_paths": paths,
+            "roofline": roofline, "roofline_hbm": roofline_hbm, "roofline_smem": roofline_smem, "stages": stages, "particle_paths": paths,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(c1["launches"] - c0["launches"]),
             "clocks": clk}
     print(json.dumps(line))
@@ -350,9 +383,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: 256^3 x 8 ppc)")
     ap.add_argument("--n", type=int, default=None, help="override the cube edge of configs 0-2 (debugging)")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--sort-every", type=int, default=None, help="override the workload's sort cadence (steps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--traffic", type=float, default=None,
-                    help="DRAM bytes per launch of the dominant kernel from the committed ncu capture")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
