@@ -204,9 +204,8 @@ def run_ours(args):
     from paper_2303_12873_b200 import workloads as W
     from paper_2303_12873_b200.binding import Sim      # raises if libpic_b200.so is missing: no fallback
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2303_12873_b200 import replicas as R
+    rank, local, world = R.rank_env(os.environ)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
@@ -221,10 +220,7 @@ def run_ours(args):
     if args.n is not None:
         kw["n"] = args.n
     wl = W.config(args.config, parity=False, **kw)
-    if rank:
-        for sp in wl.species:       # replicas differ only by a cyclic shift of the particle momenta
-            for nm in ("ux", "uy", "uz"):
-                setattr(sp, nm, np.roll(getattr(sp, nm), 8 * rank))
+    wl = R.make_replica(wl, rank)   # replicas differ only by a cyclic shift of the particle momenta
     sort_every = wl.sort_every if wl.sort_every > 0 else 0
     if args.sort_every is not None:
         sort_every = max(0, args.sort_every)
@@ -265,11 +261,8 @@ def run_ours(args):
     st = sim.stage_ms()
     sim.set_option("stage_timing", 0)
     c1 = sim.counters()
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    value = world * npart * args.steps / (ms_total * 1e-3)
+    ms_total = R.max_over_ranks(ms_total, dist, device="cuda")
+    value = R.job_rate(npart, args.steps, ms_total * 1e-3, world)
 
     # ---- rooflines of the dominant kernel (fused particle kernel, one launch per species per step) ----
     nspec = sum(1 for s in wl.species if s.n > 0)
@@ -339,11 +332,8 @@ def run_ours(args):
             e2e_step()
         barrier()
         dt_e = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt_e], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt_e = float(t.item())
-        e2e = {"value": world * npart * args.e2e_steps / dt_e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        dt_e = R.max_over_ranks(dt_e, dist, device="cuda")
+        e2e = {"value": R.job_rate(npart, args.e2e_steps, dt_e, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": args.e2e_steps, "ms_per_step": 1e3 * dt_e / args.e2e_steps,
                "what": "pic_load_particles(host) + pic_sort + pic_step(1) + pic_get_particles(host) + "
                        "pic_get_fields(host), pinned buffers, wall clock around synchronising calls"}
