@@ -104,6 +104,32 @@ __device__ __forceinline__ void to_fast_window(const double (&w)[N + 1], int fir
     }
 }
 
+// N+1 new weights whose first node sits sh = first - anchor slots into the per-cell window (sh = -1 .. 2
+// for a move of less than one cell): weights landing on slots 0 .. FW-1 go to out[], the one that may land
+// on slot -1 or FW (the particle crossed the cell face) is returned in e_lo / e_hi.
+template <int N>
+__device__ __forceinline__ void place_new_window(const double (&w)[N + 1], int sh, double (&out)[FastWin<N>::FW],
+                                                 double& e_lo, double& e_hi) {
+    constexpr int FW = FastWin<N>::FW;
+#pragma unroll
+    for (int a = 0; a < FW; ++a) {
+        double v = 0.0;
+#pragma unroll
+        for (int t = -1; t <= 2; ++t) {
+            const int k = a - t;                      // weight index that lands on slot a when sh == t
+            if (k >= 0 && k <= N) v = (sh == t) ? w[k] : v;
+        }
+        out[a] = v;
+    }
+    e_lo = (sh == -1) ? w[0] : 0.0;
+    e_hi = 0.0;
+#pragma unroll
+    for (int t = 0; t <= 2; ++t) {
+        const int k = FW - t;
+        if (k >= 0 && k <= N) e_hi = (sh == t) ? w[k] : e_hi;
+    }
+}
+
 // Shared stencil layout: word(x, y, z) = y + EY * z + EY * EZ * x  (y fastest, x slowest).  With
 // EY = EZ = 10 the strides are 1, 10 and 100 = 4 (mod 16) words, so the addresses one gather load
 // touches in a half-warp -- up to 3 adjacent cells in x, times the -1/0 stagger shift in every
@@ -191,9 +217,15 @@ __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
 namespace {
 
 constexpr int FLAG = 33;           // last double of every staging slot: record kind
-constexpr double REC_FAST = 0.0;   // fast record (FastRec layout), accumulated by phase B
-constexpr double REC_SLOW = 1.0;   // slow record (SlowRec layout), deposited by the whole warp
-constexpr double REC_NONE = 2.0;   // nothing to deposit (q = 0, or the particle raised PIC_EPHYS)
+constexpr double REC_FAST = 0.0;   // fast record (FastRec layout): old and new cell identical
+// 1 .. 6: fast record of a particle that crossed ONE cell face: 1 + 2 d + (1 if towards +d).  The part of
+// its Esirkepov window inside the cell's window is in the record; the one node layer outside it (S0 = 0,
+// DS = e there) is described by (e, prefix factor on the outer edge) in the chunk's extras area.
+constexpr double REC_SLOW = 8.0;   // slow record (SlowRec layout), deposited by the whole warp
+constexpr double REC_NONE = 7.0;   // nothing to deposit (q = 0, or the particle raised PIC_EPHYS)
+
+// extras of staging slot p (unskewed index): two doubles in the gap slot the skew leaves after every 8 slots
+__device__ __forceinline__ int ext_word(int p, int pitch) { return (9 * (p >> 3) + 8) * pitch + 2 * (p & 7); }
 
 // fp64 add to GLOBAL memory without a return value: REDG.E.ADD.F64 (fire-and-forget).  atomicAdd on a
 // pointer whose address space the compiler cannot prove emits a generic ATOM with a returned value
@@ -303,13 +335,18 @@ struct CellAcc {
             for (int a = 0; a < FW - 1; ++a) { jx[b][a] = 0.0; jy[a][b] = 0.0; jz[a][b] = 0.0; }
     }
     // one staged particle; s = this lane's plane.  Returns false for a record that is not fast.
-    __device__ __forceinline__ bool add(const double* __restrict__ r, int s) {
+    // ext = the slot's extras (e, outer prefix factor), read only for a face crosser; jx0, jy0, jz0 =
+    // global J pointers at the first node of this cell's window (for the crosser's overflow layer).
+    __device__ __forceinline__ bool add(const double* __restrict__ r, int s, const double* __restrict__ ext,
+                                        double* jx0, double* jy0, double* jz0, long long sy, long long sz) {
         using R = FastRec<N>;
         const double third = 1.0 / 3.0;
         double s0x[FW], dsx[FW], s0y[FW], dsy[FW], pdx[FW - 1], pdy[FW - 1], pdz[FW - 1];
+        double code;
         if constexpr (FW == 4) {
             const double2 tail = ld2(r, 32);                  // pdz[2], flag
-            if (tail.y != REC_FAST) return false;
+            if (tail.y >= REC_NONE) return false;
+            code = tail.y;
             double2 v;
             v = ld2(r, R::S0X); s0x[0] = v.x; s0x[1] = v.y; v = ld2(r, R::S0X + 2); s0x[2] = v.x; s0x[3] = v.y;
             v = ld2(r, R::DSX); dsx[0] = v.x; dsx[1] = v.y; v = ld2(r, R::DSX + 2); dsx[2] = v.x; dsx[3] = v.y;
@@ -321,7 +358,8 @@ struct CellAcc {
             v = ld2(r, 30); pdz[0] = v.x; pdz[1] = v.y;
             pdz[2] = tail.x;
         } else {
-            if (r[FLAG] != REC_FAST) return false;
+            code = r[FLAG];
+            if (code >= REC_NONE) return false;
 #pragma unroll
             for (int a = 0; a < FW; ++a) {
                 s0x[a] = r[R::S0X + a]; dsx[a] = r[R::DSX + a]; s0y[a] = r[R::S0Y + a]; dsy[a] = r[R::DSY + a];
@@ -333,23 +371,74 @@ struct CellAcc {
         const double az = s0z + 0.5 * dsz, bz = 0.5 * s0z + third * dsz;
         const double s0ys = r[R::S0Y + s], dsys = r[R::DSY + s];
         const double ay = s0ys + 0.5 * dsys, by = 0.5 * s0ys + third * dsys;
+        double tx[FW], ty[FW], tz[FW];   // cross-section factors of Jx (per b), Jy (per a), Jz (per a)
 #pragma unroll
         for (int b = 0; b < FW; ++b) {
-            const double t = s0y[b] * az + dsy[b] * bz;
+            tx[b] = s0y[b] * az + dsy[b] * bz;
 #pragma unroll
-            for (int a = 0; a < FW - 1; ++a) jx[b][a] = fma(pdx[a], t, jx[b][a]);
+            for (int a = 0; a < FW - 1; ++a) jx[b][a] = fma(pdx[a], tx[b], jx[b][a]);
         }
 #pragma unroll
         for (int a = 0; a < FW; ++a) {
-            const double t = s0x[a] * az + dsx[a] * bz;
+            ty[a] = s0x[a] * az + dsx[a] * bz;
 #pragma unroll
-            for (int b = 0; b < FW - 1; ++b) jy[b][a] = fma(pdy[b], t, jy[b][a]);
+            for (int b = 0; b < FW - 1; ++b) jy[b][a] = fma(pdy[b], ty[a], jy[b][a]);
         }
 #pragma unroll
         for (int a = 0; a < FW; ++a) {
-            const double t = s0x[a] * ay + dsx[a] * by;
+            tz[a] = s0x[a] * ay + dsx[a] * by;
 #pragma unroll
-            for (int c = 0; c < FW - 1; ++c) jz[c][a] = fma(pdz[c], t, jz[c][a]);
+            for (int c = 0; c < FW - 1; ++c) jz[c][a] = fma(pdz[c], tz[a], jz[c][a]);
+        }
+        if (code != REC_FAST) {
+            // ---- face crosser: the node layer just outside the window (S0 = 0, DS = e) ----------------
+            const double2 x = ld2(ext, 0);
+            const double e = x.x, pd_ov = x.y;
+            const int k = (int)code - 1, d = k >> 1, hi = k & 1;
+            const long long node = hi ? FW : -1;          // node slot of the layer
+            const long long edge = hi ? FW - 1 : -1;      // edge slot between the layer and the window
+            const double he = 0.5 * e, te = third * e;
+            if (d == 0) {
+                double* px = jx0 + edge + sz * s;
+#pragma unroll
+                for (int b = 0; b < FW; ++b) red_add(px + sy * b, pd_ov * tx[b]);
+                double* py = jy0 + node + sz * s;
+                const double ebz = e * bz;
+#pragma unroll
+                for (int b = 0; b < FW - 1; ++b) red_add(py + sy * b, pdy[b] * ebz);
+                double* pz = jz0 + node + sy * s;
+                const double eby = e * by;
+#pragma unroll
+                for (int c = 0; c < FW - 1; ++c) red_add(pz + sz * c, pdz[c] * eby);
+            } else if (d == 1) {
+                double* py = jy0 + sy * edge + sz * s;
+#pragma unroll
+                for (int a = 0; a < FW; ++a) red_add(py + a, pd_ov * ty[a]);
+                double* px = jx0 + sy * node + sz * s;
+                const double ebz = e * bz;
+#pragma unroll
+                for (int a = 0; a < FW - 1; ++a) red_add(px + a, pdx[a] * ebz);
+                if (s < FW - 1) {     // the layer's Jz row belongs to no lane: lane s takes plane c = s
+                    double* pz = jz0 + sy * node + sz * s;
+                    const double pc = r[R::PDZ + s];
+#pragma unroll
+                    for (int a = 0; a < FW; ++a) red_add(pz + a, pc * (s0x[a] * he + dsx[a] * te));
+                }
+            } else {
+                double* pz = jz0 + sy * s + sz * edge;
+#pragma unroll
+                for (int a = 0; a < FW; ++a) red_add(pz + a, pd_ov * tz[a]);
+                double* px = jx0 + sy * s + sz * node;      // the layer's Jx, Jy planes: lane s takes row b = s
+                const double t = s0ys * he + dsys * te;
+#pragma unroll
+                for (int a = 0; a < FW - 1; ++a) red_add(px + a, pdx[a] * t);
+                if (s < FW - 1) {
+                    double* py = jy0 + sy * s + sz * node;
+                    const double pb = r[R::PDY + s];
+#pragma unroll
+                    for (int a = 0; a < FW; ++a) red_add(py + a, pb * (s0x[a] * he + dsx[a] * te));
+                }
+            }
         }
         return true;
     }
@@ -472,6 +561,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
         const int cell_lo = off[bq], cell_hi = off[bq + 1];  // phase B: this lane's cell
         CellAcc<N> acc;
         acc.clear();
+        const long long win0 = g.idx(t0x + bq + FA, t0y + ry0 + FA, t0z + rz0 + FA);   // this lane's cell window
 
         for (int base = row_lo; base < row_hi; base += C::CHUNK) {
             // ---------------- phase A: lane <-> particle, 32 at a time ---------------------------
@@ -529,11 +619,11 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                     int lc = 0;
 #pragma unroll
                     for (int c = 1; c < C::TX; ++c) lc += (off[c] <= ip) ? 1 : 0;
-                    const bool same = __double2int_rd(xi1) == ci && __double2int_rd(et1) == cj &&
-                                      __double2int_rd(ze1) == ck;
                     const bool listed = in_tile && rx == lc && ry == ry0 && rz == rz0;
                     const bool deposits = !bad && qw != 0.0;
-                    const bool fast = deposits && same && listed;
+                    const int ncross = (__double2int_rd(xi1) != ci) + (__double2int_rd(et1) != cj) +
+                                       (__double2int_rd(ze1) != ck);
+                    const bool fast = deposits && listed && ncross <= 1;   // phase B handles one crossed face
                     is_slow = deposits && !fast;
                     if (in_tile) { if (is_slow) ++n_slow; else ++n_fast; }
                     if (fast) {
@@ -541,6 +631,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                         double fr[FLAG + 1];
 #pragma unroll
                         for (int k = 0; k <= FLAG; ++k) fr[k] = 0.0;
+                        double code = REC_FAST, ext_e = 0.0, ext_pd = 0.0;
 #pragma unroll
                         for (int d = 0; d < 3; ++d) {
                             const double a1 = (d == 0) ? xi1 : ((d == 1) ? et1 : ze1);
@@ -549,12 +640,13 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                             const double (&w0)[N + 1] = (d == 0) ? wxn : ((d == 1) ? wyn : wzn);
                             const double area = (d == 0) ? g.inv_dy * g.inv_dz
                                                          : ((d == 1) ? g.inv_dx * g.inv_dz : g.inv_dx * g.inv_dy);
-                            double w1[N + 1], s0[FW], s1[FW];
+                            double w1[N + 1], s0[FW], s1[FW], e_lo, e_hi;
                             const int f1 = shape_weights<N>(a1, w1);
                             to_fast_window<N>(w0, f0, cell + FA, s0);
-                            to_fast_window<N>(w1, f1, cell + FA, s1);
+                            place_new_window<N>(w1, f1 - (cell + FA), s1, e_lo, e_hi);
                             const double cq = (-qw * inv_dt) * area;
-                            double run = 0.0;
+                            double run = e_lo;            // the prefix starts at the lowest node of the union window
+                            const double pd_lo = cq * run;
 #pragma unroll
                             for (int a = 0; a < FW; ++a) {
                                 const double dd = s1[a] - s0[a];
@@ -563,11 +655,14 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                                 run += dd;
                                 if (a < FW - 1) fr[FR::PDX + (FW - 1) * d + a] = cq * run;
                             }
+                            if (e_lo != 0.0) { code = 1.0 + 2.0 * d; ext_e = e_lo; ext_pd = pd_lo; }
+                            if (e_hi != 0.0) { code = 2.0 + 2.0 * d; ext_e = e_hi; ext_pd = cq * run; }
                         }
-                        fr[FLAG] = REC_FAST;
+                        fr[FLAG] = code;
 #pragma unroll
                         for (int k = 0; k < (FR::LEN + 1) / 2; ++k) st2(rec, 2 * k, fr[2 * k], fr[2 * k + 1]);
-                        if ((FR::LEN + 1) / 2 <= FLAG / 2) st2(rec, FLAG - 1, 0.0, REC_FAST);
+                        if ((FR::LEN + 1) / 2 <= FLAG / 2) st2(rec, FLAG - 1, 0.0, code);
+                        if (code != REC_FAST) st2(stg, ext_word(sub + lane, C::PITCH), ext_e, ext_pd);
                     } else if (is_slow) {
                         slow_write<N>(rec, g, xi, et, ze, xi1, et1, ze1, qw, inv_dt);
                     } else {
@@ -588,15 +683,18 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                 const int lo = max(cell_lo, base), hi = min(cell_hi, base + C::CHUNK);
                 const int len = (bs < FW) ? hi - lo : 0;
                 const int maxlen = __reduce_max_sync(0xffffffffu, max(len, 0));
-                const double* r0 = stg;
 #pragma unroll 1
                 for (int t = 0; t < maxlen; ++t)
-                    if (t < len) acc.add(r0 + skew(lo + t - base) * C::PITCH, bs);
+                    if (t < len) {
+                        const int pslot = lo + t - base;
+                        acc.add(stg + skew(pslot) * C::PITCH, bs, stg + ext_word(pslot, C::PITCH), f.Jx + win0,
+                                f.Jy + win0, f.Jz + win0, g.sy, g.sz);
+                    }
             }
             __syncwarp();
         }
         // ---------------- flush the row's accumulators ---------------------------------------------
-        if (bs < FW) acc.flush(g, f, g.idx(t0x + bq + FA, t0y + ry0 + FA, t0z + rz0 + FA), bs, stg, lane);
+        if (bs < FW) acc.flush(g, f, win0, bs, stg, lane);
         __syncwarp();
     }
     // ---- flags and counters ----------------------------------------------------------------------
