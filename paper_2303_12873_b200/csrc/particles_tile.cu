@@ -234,6 +234,17 @@ __device__ __forceinline__ void red_add(double* p, double v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// pull one 32-particle sub-chunk of the SoA arrays towards the SM ahead of its use
+__device__ __forceinline__ void prefetch_particles(const Particles& p, int ip, int hi) {
+    if (ip < hi) {
+        prefetch_l1(p.x + ip); prefetch_l1(p.y + ip); prefetch_l1(p.z + ip);
+        prefetch_l1(p.ux + ip); prefetch_l1(p.uy + ip); prefetch_l1(p.uz + ip);
+        prefetch_l1(p.w + ip);
+    }
+}
+
 __device__ __forceinline__ double2 ld2(const double* r, int i) { return *reinterpret_cast<const double2*>(r + i); }
 __device__ __forceinline__ void st2(double* r, int i, double a, double b) {
     *reinterpret_cast<double2*>(r + i) = make_double2(a, b);
@@ -528,16 +539,31 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
     if (n_tile == 0) return;    // empty tile (block-uniform)
 
     // ---- stage the field stencil ----------------------------------------------------------------
+    // All of a thread's loads are issued before the first store (one L2/HBM round trip instead of one
+    // per loop trip: with one block per SM nothing else hides this latency).
     {
         const double* src[6] = {f.Ex, f.Ey, f.Ez, f.Bx, f.By, f.Bz};
-        for (int e = tid; e < C::ESZ; e += C::NT) {
+        constexpr int NIT = (C::ESZ + C::NT - 1) / C::NT;
+        double v[NIT][6];
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int e = tid + it * C::NT;
             const int ex = e % C::EX, ey = (e / C::EX) % C::EY, ez = e / (C::EX * C::EY);
             const int gx = t0x - C::GL + ex + NG, gy = t0y - C::GL + ey + NG, gz = t0z - C::GL + ez + NG;
-            const bool ok = gx >= 0 && gx < g.nx + 2 * NG && gy >= 0 && gy < g.py && gz >= 0 && gz < g.pz;
+            const bool ok = e < C::ESZ && gx >= 0 && gx < g.nx + 2 * NG && gy >= 0 && gy < g.py && gz >= 0 &&
+                            gz < g.pz;
             const long long o = gx + g.sy * gy + g.sz * gz;
-            const int w = tile_word<C>(ex, ey, ez);
 #pragma unroll
-            for (int cpt = 0; cpt < 6; ++cpt) Et[cpt * C::ESZ + w] = ok ? __ldg(src[cpt] + o) : 0.0;
+            for (int cpt = 0; cpt < 6; ++cpt) v[it][cpt] = ok ? __ldg(src[cpt] + o) : 0.0;
+        }
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int e = tid + it * C::NT;
+            if (e < C::ESZ) {
+                const int w = tile_word<C>(e % C::EX, (e / C::EX) % C::EY, e / (C::EX * C::EY));
+#pragma unroll
+                for (int cpt = 0; cpt < 6; ++cpt) Et[cpt * C::ESZ + w] = v[it][cpt];
+            }
         }
     }
     __syncthreads();
@@ -549,11 +575,19 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
     unsigned int n_fast = 0, n_slow = 0, n_glob = 0;
     bool bad_any = false;
 
+    int row_ahead = 0;
+    if (lane == 0) row_ahead = atomicAdd(next_row, 1);
+    row_ahead = __shfl_sync(0xffffffffu, row_ahead, 0);
     for (;;) {
-        int row = 0;
-        if (lane == 0) row = atomicAdd(next_row, 1);
-        row = __shfl_sync(0xffffffffu, row, 0);
+        const int row = row_ahead;
         if (row >= C::NROW) break;
+        if (lane == 0) row_ahead = atomicAdd(next_row, 1);     // the row after this one: prefetch its head
+        row_ahead = __shfl_sync(0xffffffffu, row_ahead, 0);
+        if (row_ahead < C::NROW) {
+            const int* offn = row_off + row_ahead * (C::TX + 1);
+            prefetch_particles(p, offn[0] + lane, offn[C::TX]);
+            prefetch_particles(p, offn[0] + 32 + lane, offn[C::TX]);
+        }
         const int* off = row_off + row * (C::TX + 1);
         const int row_lo = off[0], row_hi = off[C::TX];
         if (row_lo >= row_hi) continue;
@@ -569,6 +603,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
             for (int sub = 0; sub < C::CHUNK; sub += 32) {
                 const int ip = base + sub + lane;
                 if (base + sub >= row_hi) break;
+                prefetch_particles(p, ip + 64, row_hi);   // rows longer than the two sub-chunks prefetched a row ahead
                 double* rec = stg + skew(sub + lane) * C::PITCH;
                 bool is_slow = false;
                 if (ip < row_hi) {
