@@ -210,7 +210,9 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *   "force_path"     0 = automatic, 1 = always the global-atomic particle
  *                    kernel, 2 = always the fused per-tile kernel (requires a
  *                    prior pic_sort, else PIC_ESTATE at pic_step)
- *   "yee_tma"        1 (default) = TMA-staged Yee kernels, 0 = plain loads
+ *   "yee_tma"        bit 0 = B push, bit 1 = E push through the TMA-staged
+ *                    tile kernels; 3 (default) = both, 0 = plain one-thread-
+ *                    per-cell kernels (same arithmetic, bit-identical result)
  * Unknown name: PIC_EINVAL.
  */
 int pic_set_option(pic_ctx*, const char* name, long long value);

@@ -50,7 +50,8 @@ struct pic_ctx {
     int sticky = PIC_OK;
     unsigned long long launches = 0, steps = 0, sorts = 0;
     // options
-    int stage_timing = 0, force_path = 0, yee_tma = 1;
+    int stage_timing = 0, force_path = 0, yee_tma = 3;
+    YeeMaps yee_maps{};
     std::vector<cudaEvent_t> ev_pool;   // grows on demand; never waited on inside pic_step / pic_sort
     size_t ev_used = 0;
     std::vector<TimedSpan> spans;
@@ -285,6 +286,7 @@ int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, d
     // zero the status block, the fields and the scratch component (particles are written at load)
     cudaError_t e = cudaMemsetAsync(base, 0, L.tmp + L.comp_bytes, c->stream);
     if (e == cudaSuccess) e = (cudaError_t)tile_setup();
+    make_yee_maps(c->g, c->f, &c->yee_maps);   // on failure yee_maps.valid stays 0: plain Yee kernels
     if (e != cudaSuccess) {
         delete c;
         return PIC_ECUDA;
@@ -356,7 +358,8 @@ int pic_step(pic_ctx* c, int nsteps) {
     const bool timing = c->stage_timing != 0;
     const Grid& g = c->g;
     const size_t comp_bytes = (size_t)g.npad * sizeof(double);
-    const bool tma = c->yee_tma != 0;
+    const YeeMaps* tma_B = ((c->yee_tma & 1) && c->yee_maps.valid) ? &c->yee_maps : nullptr;
+    const YeeMaps* tma_E = ((c->yee_tma & 2) && c->yee_maps.valid) ? &c->yee_maps : nullptr;
     for (int it = 0; it < nsteps; ++it) {
         cudaEvent_t* ev = nullptr;
         if (timing) {
@@ -393,12 +396,12 @@ int pic_step(pic_ctx* c, int nsteps) {
         c->launches += 3;
         if (timing) cudaEventRecord(ev[3], c->stream);
         // steps 6-8
-        launch_push_B(g, c->f, 0.5 * g.dt, tma, c->stream);
+        launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
         if (timing) cudaEventRecord(ev[4], c->stream);
-        launch_push_E(g, c->f, g.dt, tma, c->stream);
+        launch_push_E(g, c->f, g.dt, tma_E, c->stream);
         if (timing) cudaEventRecord(ev[5], c->stream);
-        launch_push_B(g, c->f, 0.5 * g.dt, tma, c->stream);
-        c->launches += 3 * yee_num_launches(tma);
+        launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
+        c->launches += 3;
         c->steps += 1;
         if (timing) cudaEventRecord(ev[6], c->stream);
     }
@@ -565,7 +568,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     else if (!strcmp(name, "force_path")) {
         if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "force_path must be 0, 1 or 2");
         c->force_path = (int)value;
-    } else if (!strcmp(name, "yee_tma")) c->yee_tma = value != 0;
+    } else if (!strcmp(name, "yee_tma")) c->yee_tma = (int)value & 3;
     else return fail(c, PIC_EINVAL, "unknown option '%s'", name);
     return PIC_OK;
 }

@@ -53,10 +53,16 @@ struct DevStatus {
 };
 
 // ---- yee.cu ---------------------------------------------------------------
-void launch_push_B(const Grid& g, const Fields& f, double dth, bool tma, cudaStream_t st);
-void launch_push_E(const Grid& g, const Fields& f, double dt, bool tma, cudaStream_t st);
+// Six CUtensorMap objects (Ex Ey Ez Bx By Bz), kept opaque here so that only yee.cu needs <cuda.h>.
+struct YeeMaps {
+    alignas(64) unsigned char map[6 * 128];
+    int valid;
+};
+int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out);   // 0 = ok; else the plain kernels are used
+// maps == nullptr or !maps->valid: plain one-thread-per-cell kernels; else the TMA-staged tile kernels
+void launch_push_B(const Grid& g, const Fields& f, double dth, const YeeMaps* maps, cudaStream_t st);
+void launch_push_E(const Grid& g, const Fields& f, double dt, const YeeMaps* maps, cudaStream_t st);
 void launch_fill_guards(const Grid& g, double* F, cudaStream_t st);       // periodic images of one component
-int yee_num_launches(bool tma);
 
 // ---- particles_global.cu --------------------------------------------------
 // gather + Boris + move + Esirkepov with global fp64 atomics + wrap; any particle order.

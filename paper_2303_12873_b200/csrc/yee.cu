@@ -10,6 +10,16 @@
 // image of that cell, so no separate guard-exchange pass is needed: after a
 // push the updated component is valid on the whole padded array.
 // HBM-bound: 72 B/cell (B push), 96 B/cell (E push) algorithmic.
+//
+// Two implementations of each push:
+//   *_kernel      one thread per cell, every operand a global load (12 loads per cell; the +-1 rows in
+//                 y and z miss L1, so the kernel is L1/L2-throughput bound at ~40 % of the HBM roofline);
+//   *_tma_kernel  one block per 32 x 8 x 8 tile: the three curl operands (+ a one-cell halo) are staged
+//                 in shared memory by TMA (cp.async.bulk.tensor.3d, one thread, mbarrier
+//                 completion) while the threads fetch the component they update; the padded guard cells
+//                 mean a box never wraps, and boxes that poke out of the array are zero-filled.
+#include <cuda.h>
+
 #include "pic_internal.h"
 
 namespace pic {
@@ -67,18 +77,224 @@ __global__ void __launch_bounds__(128) push_E_kernel(Grid g, Fields f, double cd
     if (is_edge(g, i, j, k)) store_images3(g, f.Ex, f.Ey, f.Ez, i, j, k, ex, ey, ez);
 }
 
-void launch_push_B(const Grid& g, const Fields& f, double dth, bool /*tma*/, cudaStream_t st) {
-    dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
-    push_B_kernel<<<nb, bs, 0, st>>>(g, f, dth * g.inv_dx, dth * g.inv_dy, dth * g.inv_dz);
+// ---- TMA-staged variant ------------------------------------------------------------------------
+namespace {
+
+constexpr int YTX = 32, YTY = 8, YTZ = 8;                  // cells per block
+// Staged box: the tile plus one halo cell in y and z and, in x, 2 cells: with 8-byte elements the box corner
+// must sit on an EVEN x coordinate (TMA wants the first byte of a box row 16-byte aligned; an odd coordinate
+// raises "illegal instruction"), so the E push (backward differences) starts 2 cells below the tile, not 1.
+// Row = 34 or 36 doubles = 272 / 288 B: a multiple of 16 B as TMA requires.
+constexpr int YBY = YTY + 1, YBZ = YTZ + 1;
+template <int HX> struct YeeBox {
+    static constexpr int BX = YTX + HX;
+    static constexpr int SZ = BX * YBY * YBZ;
+    static constexpr int PAD = (SZ + 15) / 16 * 16;        // every TMA destination starts on a 128-byte boundary
+};
+constexpr int YNT = 256;
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned phase) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(phase) : "memory");
+}
+// one 3-D box of a padded component -> shared memory; (x, y, z) = padded element coordinates of its corner
+__device__ __forceinline__ void tma_load_box(double* dst, const CUtensorMap* map, unsigned long long* bar, int x,
+                                             int y, int z) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<unsigned long long>(map)), "r"(x), "r"(y), "r"(z),
+        "r"(smem_u32(bar)) : "memory");
 }
 
-void launch_push_E(const Grid& g, const Fields& f, double dt, bool /*tma*/, cudaStream_t st) {
-    dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
+template <int HX> struct YeeSmem {
+    alignas(128) double box[3][YeeBox<HX>::PAD];
+    alignas(8) unsigned long long bar;
+};
+
+// Box corner = (tile's first cell) - (shx, sh, sh): sh = 0 for forward differences (B push), 1 for backward
+// differences (E push, shx = 2 to stay on an even x coordinate).
+template <int HX>
+__device__ __forceinline__ void stage_boxes(YeeSmem<HX>& sm, const CUtensorMap* m0, const CUtensorMap* m1,
+                                            const CUtensorMap* m2, int t0x, int t0y, int t0z, int shx, int sh) {
+    if (threadIdx.x == 0) mbar_init(&sm.bar, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        mbar_expect_tx(&sm.bar, 3u * YeeBox<HX>::SZ * (unsigned)sizeof(double));
+        tma_load_box(sm.box[0], m0, &sm.bar, t0x + NG - shx, t0y + NG - sh, t0z + NG - sh);
+        tma_load_box(sm.box[1], m1, &sm.bar, t0x + NG - shx, t0y + NG - sh, t0z + NG - sh);
+        tma_load_box(sm.box[2], m2, &sm.bar, t0x + NG - shx, t0y + NG - sh, t0z + NG - sh);
+    }
+}
+
+}  // namespace
+
+__global__ void __launch_bounds__(YNT) push_B_tma_kernel(Grid g, Fields f, double cdx, double cdy, double cdz,
+                                                         const __grid_constant__ CUtensorMap mEx,
+                                                         const __grid_constant__ CUtensorMap mEy,
+                                                         const __grid_constant__ CUtensorMap mEz) {
+    extern __shared__ __align__(128) unsigned char yee_smem_raw[];
+    constexpr int YBX = YeeBox<2>::BX;
+    YeeSmem<2>& sm = *reinterpret_cast<YeeSmem<2>*>(yee_smem_raw);
+    const int t0x = blockIdx.x * YTX, t0y = blockIdx.y * YTY, t0z = blockIdx.z * YTZ;
+    stage_boxes<2>(sm, &mEx, &mEy, &mEz, t0x, t0y, t0z, 0, 0);
+    const int tx = threadIdx.x % YTX, ty = threadIdx.x / YTX;     // 32 x 8 threads, each walks the 8 z planes
+    const int i = t0x + tx, j = t0y + ty;
+    const bool in_xy = i < g.nx && j < g.ny;
+    double bx[YTZ], by[YTZ], bz[YTZ];
+#pragma unroll
+    for (int c = 0; c < YTZ; ++c) {
+        const bool ok = in_xy && t0z + c < g.nz;
+        const long long o = g.idx(i, j, t0z + c);
+        bx[c] = ok ? f.Bx[o] : 0.0;
+        by[c] = ok ? f.By[o] : 0.0;
+        bz[c] = ok ? f.Bz[o] : 0.0;
+    }
+    mbar_wait(&sm.bar, 0);
+    const double* Ex = sm.box[0] + tx + YBX * ty;
+    const double* Ey = sm.box[1] + tx + YBX * ty;
+    const double* Ez = sm.box[2] + tx + YBX * ty;
+#pragma unroll
+    for (int c = 0; c < YTZ; ++c) {
+        const int k = t0z + c;
+        if (!(in_xy && k < g.nz)) continue;
+        const int w = YBX * YBY * c;
+        const double ex = Ex[w], ey = Ey[w], ez = Ez[w];
+        const double nbx = bx[c] - (cdy * (Ez[w + YBX] - ez) - cdz * (Ey[w + YBX * YBY] - ey));
+        const double nby = by[c] - (cdz * (Ex[w + YBX * YBY] - ex) - cdx * (Ez[w + 1] - ez));
+        const double nbz = bz[c] - (cdx * (Ey[w + 1] - ey) - cdy * (Ex[w + YBX] - ex));
+        const long long o = g.idx(i, j, k);
+        f.Bx[o] = nbx;
+        f.By[o] = nby;
+        f.Bz[o] = nbz;
+        if (is_edge(g, i, j, k)) store_images3(g, f.Bx, f.By, f.Bz, i, j, k, nbx, nby, nbz);
+    }
+}
+
+__global__ void __launch_bounds__(YNT) push_E_tma_kernel(Grid g, Fields f, double cdx, double cdy, double cdz,
+                                                         double dt_eps0, const __grid_constant__ CUtensorMap mBx,
+                                                         const __grid_constant__ CUtensorMap mBy,
+                                                         const __grid_constant__ CUtensorMap mBz) {
+    extern __shared__ __align__(128) unsigned char yee_smem_raw[];
+    constexpr int YBX = YeeBox<4>::BX;
+    YeeSmem<4>& sm = *reinterpret_cast<YeeSmem<4>*>(yee_smem_raw);
+    const int t0x = blockIdx.x * YTX, t0y = blockIdx.y * YTY, t0z = blockIdx.z * YTZ;
+    stage_boxes<4>(sm, &mBx, &mBy, &mBz, t0x, t0y, t0z, 2, 1);
+    const int tx = threadIdx.x % YTX, ty = threadIdx.x / YTX;
+    const int i = t0x + tx, j = t0y + ty;
+    const bool in_xy = i < g.nx && j < g.ny;
+    double ex[YTZ], ey[YTZ], ez[YTZ], jx[YTZ], jy[YTZ], jz[YTZ];     // in flight while the TMA boxes land
+#pragma unroll
+    for (int c = 0; c < YTZ; ++c) {
+        const bool ok = in_xy && t0z + c < g.nz;
+        const long long o = g.idx(i, j, t0z + c);
+        ex[c] = ok ? f.Ex[o] : 0.0;
+        ey[c] = ok ? f.Ey[o] : 0.0;
+        ez[c] = ok ? f.Ez[o] : 0.0;
+        jx[c] = ok ? f.Jx[o] : 0.0;
+        jy[c] = ok ? f.Jy[o] : 0.0;
+        jz[c] = ok ? f.Jz[o] : 0.0;
+    }
+    mbar_wait(&sm.bar, 0);
+    const double* Bx = sm.box[0] + (tx + 2) + YBX * (ty + 1) + YBX * YBY;
+    const double* By = sm.box[1] + (tx + 2) + YBX * (ty + 1) + YBX * YBY;
+    const double* Bz = sm.box[2] + (tx + 2) + YBX * (ty + 1) + YBX * YBY;
+#pragma unroll
+    for (int c = 0; c < YTZ; ++c) {
+        const int k = t0z + c;
+        if (!(in_xy && k < g.nz)) continue;
+        const int w = YBX * YBY * c;
+        const double bx = Bx[w], by = By[w], bz = Bz[w];
+        const long long o = g.idx(i, j, k);
+        // same operation order as the plain kernel: (E + curl term) - dt/eps0 J
+        const double nex = (ex[c] + (cdy * (bz - Bz[w - YBX]) - cdz * (by - By[w - YBX * YBY]))) - dt_eps0 * jx[c];
+        const double ney = (ey[c] + (cdz * (bx - Bx[w - YBX * YBY]) - cdx * (bz - Bz[w - 1]))) - dt_eps0 * jy[c];
+        const double nez = (ez[c] + (cdx * (by - By[w - 1]) - cdy * (bx - Bx[w - YBX]))) - dt_eps0 * jz[c];
+        f.Ex[o] = nex;
+        f.Ey[o] = ney;
+        f.Ez[o] = nez;
+        if (is_edge(g, i, j, k)) store_images3(g, f.Ex, f.Ey, f.Ez, i, j, k, nex, ney, nez);
+    }
+}
+
+void launch_push_B(const Grid& g, const Fields& f, double dth, const YeeMaps* maps, cudaStream_t st) {
+    const double cdx = dth * g.inv_dx, cdy = dth * g.inv_dy, cdz = dth * g.inv_dz;
+    if (maps && maps->valid) {
+        dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ - 1) / YTZ);
+        const CUtensorMap* m = reinterpret_cast<const CUtensorMap*>(maps->map);
+        push_B_tma_kernel<<<nb, YNT, sizeof(YeeSmem<2>), st>>>(g, f, cdx, cdy, cdz, m[0], m[1], m[2]);
+    } else {
+        dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
+        push_B_kernel<<<nb, bs, 0, st>>>(g, f, cdx, cdy, cdz);
+    }
+}
+
+void launch_push_E(const Grid& g, const Fields& f, double dt, const YeeMaps* maps, cudaStream_t st) {
     const double c2dt = C_LIGHT * C_LIGHT * dt;
-    push_E_kernel<<<nb, bs, 0, st>>>(g, f, c2dt * g.inv_dx, c2dt * g.inv_dy, c2dt * g.inv_dz, dt / EPS0);
+    const double cdx = c2dt * g.inv_dx, cdy = c2dt * g.inv_dy, cdz = c2dt * g.inv_dz;
+    if (maps && maps->valid) {
+        dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ - 1) / YTZ);
+        const CUtensorMap* m = reinterpret_cast<const CUtensorMap*>(maps->map);
+        push_E_tma_kernel<<<nb, YNT, sizeof(YeeSmem<4>), st>>>(g, f, cdx, cdy, cdz, dt / EPS0, m[3], m[4], m[5]);
+    } else {
+        dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
+        push_E_kernel<<<nb, bs, 0, st>>>(g, f, cdx, cdy, cdz, dt / EPS0);
+    }
 }
 
-int yee_num_launches(bool) { return 1; }
+// Tensor maps of the six padded E,B components (rank 3, fp64, no swizzle, zero fill outside the array),
+// box = (YTX + 2) x YBY x YBZ for E (read by the B push), (YTX + 4) x YBY x YBZ for B.  The driver entry point is fetched through the runtime (no link-time libcuda).
+int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out) {
+    static_assert(sizeof(CUtensorMap) == 128 && sizeof(out->map) == 6 * 128, "YeeMaps storage");
+    out->valid = 0;
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                 const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return 1;
+    }
+    double* comp[6] = {f.Ex, f.Ey, f.Ez, f.Bx, f.By, f.Bz};
+    CUtensorMap* m = reinterpret_cast<CUtensorMap*>(out->map);
+    const cuuint64_t dims[3] = {(cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.px * 8, (cuuint64_t)g.px * (cuuint64_t)g.py * 8};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    for (int k = 0; k < 6; ++k) {
+        const cuuint32_t box[3] = {(cuuint32_t)(k < 3 ? YeeBox<2>::BX : YeeBox<4>::BX), YBY, YBZ};
+        CUresult r = ((EncodeFn)fn)(&m[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, comp[k], dims, strides, box, estr,
+                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return 2;
+    }
+    if (cudaFuncSetAttribute(push_B_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(YeeSmem<2>)) !=
+            cudaSuccess ||
+        cudaFuncSetAttribute(push_E_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(YeeSmem<4>)) !=
+            cudaSuccess) {
+        cudaGetLastError();
+        return 3;
+    }
+    out->valid = 1;
+    return 0;
+}
+
 
 // Periodic images of one component from its interior (used after pic_set_fields).
 __global__ void fill_guards_kernel(Grid g, double* F) {
