@@ -213,6 +213,10 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *   "yee_tma"        bit 0 = B push, bit 1 = E push through the TMA-staged
  *                    tile kernels; 3 (default) = both, 0 = plain one-thread-
  *                    per-cell kernels (same arithmetic, bit-identical result)
+ *   "tile_fresh"     1 (default) = a species that has not stepped since its
+ *                    last pic_sort runs the small-stencil, two-blocks-per-SM
+ *                    variant of the fused per-tile kernel; 0 = always the
+ *                    drift-tolerant variant (same arithmetic per particle)
  * Unknown name: PIC_EINVAL.
  */
 int pic_set_option(pic_ctx*, const char* name, long long value);

@@ -34,28 +34,46 @@ namespace pic {
 
 namespace {
 
-constexpr int DRIFT = 1;   // cells a particle may sit outside the tile and still gather from shared memory
-
 template <int N>
 struct FastWin {
     static constexpr int FW = (N == 1) ? 2 : 4;    // nodes of the per-cell window (old and new cell identical)
     static constexpr int FA = (N == 1) ? 0 : -1;   // first window node relative to the cell index
 };
 
-template <int TX_, int TY_, int TZ_, int NW_, int MINB_>
+// DRIFT = cells a particle may sit outside the tile and still gather from shared memory: 1 for a species
+// that has moved since its last pic_sort, 0 right after a sort (every particle is in its listed cell), which
+// shrinks the stencil from 14 x 10 x 10 to 12 x 8 x 8 nodes per component so that TWO blocks fit one SM
+// and one block's prologue (stencil staging: every warp of the block waits) overlaps the other's particles.
+template <int TX_, int TY_, int TZ_, int NW_, int MINB_, int DRIFT_>
 struct TileCfg {
-    static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NW = NW_, NT = 32 * NW_, MINB = MINB_;
+    static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NW = NW_, NT = 32 * NW_, MINB = MINB_, DRIFT = DRIFT_;
     static constexpr int NROW = TY * TZ;
     // gather stencil: nodes i-2 .. i+2 of a particle in cell i (every order, every staggering)
     static constexpr int GL = 2 + DRIFT;
     static constexpr int EX = TX + 2 * GL, EY = TY + 2 * GL, EZ = TZ + 2 * GL;
-    static constexpr int ESZ = EX * EY * EZ;
+    static constexpr int ESZ = EX * EY * EZ;      // nodes per component
+    // Shared layout: word(x, y, z) = y + SZ z + SX x (y fastest, x slowest).  The addresses one gather load
+    // touches in a half-warp -- a few adjacent cells in x, times the -1/0 stagger shift in every dimension --
+    // must fall into 16 different 8-byte banks: (SZ, SX) = (10, 4) or (8, 2) mod 16 does that.
+    static constexpr int SZ = EY;
+    static constexpr int SXR = (SZ % 16 == 10) ? 4 : 2;
+    static constexpr int SX = EZ * SZ + ((SXR - (EZ * SZ) % 16) + 16) % 16;
+    static_assert(SZ % 16 == 10 || SZ % 16 == 8, "no conflict-free stride for this tile height");
+    // One component occupies FP words; components that are nodal in x (Ey, Ez, Bx) never read x-slab 0
+    // (their lowest node is i-1), so that slab is not stored: their base is shifted back by one slab.
+    static constexpr int FP = (EX - 1) * SX + (EZ - 1) * SZ + EY;
+    static constexpr int TOT = 6 * FP - 3 * SX + ((6 * FP - 3 * SX) & 1);     // even: staging stays 16-byte aligned
+    __host__ __device__ static constexpr bool trimmed(int k) { return k >= 1 && k <= 3; }
+    __host__ __device__ static constexpr int comp_base(int k) {   // word of (x = 0, y = 0, z = 0), virtual for k = 1..3
+        return k == 0 ? 0 : (k == 1 ? FP - SX : (k == 2 ? 2 * FP - 2 * SX : (k == 3 ? 3 * FP - 3 * SX
+                      : (k == 4 ? 4 * FP - 3 * SX : 5 * FP - 3 * SX))));
+    }
     // per-warp staging: CHUNK skewed slots of PITCH doubles (PITCH/2 odd and the skew make the eight
     // 16-byte words a phase-B warp load touches fall into eight different 16-byte bank groups)
     static constexpr int CHUNK = 64, PITCH = 34, NSLOT = CHUNK + CHUNK / 8;
     static constexpr int STG_W = PITCH * NSLOT;
     static constexpr int NOFF = NROW * (TX + 1);
-    static constexpr size_t SMEM = sizeof(double) * (6 * (size_t)ESZ + (size_t)NW * STG_W) + sizeof(int) * (NOFF + 4);
+    static constexpr size_t SMEM = sizeof(double) * ((size_t)TOT + (size_t)NW * STG_W) + sizeof(int) * (NOFF + 4);
     static_assert(TX == 8, "phase B maps 8 cells x 4 planes onto a warp");
 };
 
@@ -130,13 +148,10 @@ __device__ __forceinline__ void place_new_window(const double (&w)[N + 1], int s
     }
 }
 
-// Shared stencil layout: word(x, y, z) = y + EY * z + EY * EZ * x  (y fastest, x slowest).  With
-// EY = EZ = 10 the strides are 1, 10 and 100 = 4 (mod 16) words, so the addresses one gather load
-// touches in a half-warp -- up to 3 adjacent cells in x, times the -1/0 stagger shift in every
-// dimension -- fall into 16 different 8-byte banks: no bank conflicts (the x-fastest layout had
-// 1.4x-1.7x wavefronts on the components staggered in y).
+// Shared stencil layout (TileCfg): word(x, y, z) = y + SZ z + SX x, conflict-free strides (the x-fastest
+// layout had 1.4x-1.7x wavefronts on the components staggered in y).
 template <class C>
-__device__ __forceinline__ int tile_word(int x, int y, int z) { return y + C::EY * (z + C::EZ * x); }
+__device__ __forceinline__ int tile_word(int x, int y, int z) { return y + C::SZ * z + C::SX * x; }
 
 // One z-plane of one component from the shared stencil: sum_b wy[b] sum_a wx[a] F[a,b].
 template <int N, class C>
@@ -147,7 +162,7 @@ __device__ __forceinline__ double gather_plane(const double* __restrict__ base, 
     for (int b = 0; b <= N; ++b) {
         double accx = 0.0;
 #pragma unroll
-        for (int a = 0; a <= N; ++a) accx = fma(wx[a], base[b + C::EY * C::EZ * a], accx);
+        for (int a = 0; a <= N; ++a) accx = fma(wx[a], base[b + C::SX * a], accx);
         accy = fma(wy[b], accx, accy);
     }
     return accy;
@@ -163,17 +178,17 @@ __device__ __forceinline__ void gather6_tile(const double* __restrict__ Et, int 
                                              const double (&wyn)[N + 1], double (&wzn)[N + 1],
                                              const double (&wxs)[N + 1], const double (&wys)[N + 1],
                                              double (&wzs)[N + 1], double (&eb)[6]) {
-    const int o_ex = 0 * C::ESZ + tile_word<C>(fxs, gyn, gzn);
-    const int o_ey = 1 * C::ESZ + tile_word<C>(gxn, fys, gzn);
-    const int o_ez = 2 * C::ESZ + tile_word<C>(gxn, gyn, fzs);
-    const int o_bx = 3 * C::ESZ + tile_word<C>(gxn, fys, fzs);
-    const int o_by = 4 * C::ESZ + tile_word<C>(fxs, gyn, fzs);
-    const int o_bz = 5 * C::ESZ + tile_word<C>(fxs, fys, gzn);
+    const int o_ex = C::comp_base(0) + tile_word<C>(fxs, gyn, gzn);
+    const int o_ey = C::comp_base(1) + tile_word<C>(gxn, fys, gzn);
+    const int o_ez = C::comp_base(2) + tile_word<C>(gxn, gyn, fzs);
+    const int o_bx = C::comp_base(3) + tile_word<C>(gxn, fys, fzs);
+    const int o_by = C::comp_base(4) + tile_word<C>(fxs, gyn, fzs);
+    const int o_bz = C::comp_base(5) + tile_word<C>(fxs, fys, gzn);
 #pragma unroll
     for (int k = 0; k < 6; ++k) eb[k] = 0.0;
     const double* pl = Et;
 #pragma unroll 1
-    for (int c = 0; c <= N; ++c, pl += C::EY) {
+    for (int c = 0; c <= N; ++c, pl += C::SZ) {
         const double zn = wzn[0], zs = wzs[0];
         eb[0] = fma(zn, gather_plane<N, C>(pl + o_ex, wxs, wyn), eb[0]);
         eb[1] = fma(zn, gather_plane<N, C>(pl + o_ey, wxn, wys), eb[1]);
@@ -205,6 +220,7 @@ __device__ __noinline__ void gather_global6(const Grid& g, const Fields& f, doub
 }
 
 // tile-relative cell index with the periodic image nearest to the tile
+template <int DRIFT>
 __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
     int r = i - t0;
     if (r < -DRIFT) r += n;
@@ -506,12 +522,12 @@ template <int N, class C>
 __global__ void __launch_bounds__(C::NT, C::MINB)
 particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const unsigned int* __restrict__ cell_offset,
                       int ntx, int nty, DevStatus* status) {
-    constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA;
+    constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA, DRIFT = C::DRIFT;
     using FR = FastRec<N>;
     static_assert(CellAcc<N>::NACC * 32 <= C::STG_W, "flush buffer does not fit the staging area");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* Et = reinterpret_cast<double*>(smem_raw);            // 6 * ESZ: Ex Ey Ez Bx By Bz
-    double* stg_all = Et + 6 * C::ESZ;                           // NW * STG_W
+    double* Et = reinterpret_cast<double*>(smem_raw);            // TOT words: Ex Ey Ez Bx By Bz
+    double* stg_all = Et + C::TOT;                               // NW * STG_W
     int* row_off = reinterpret_cast<int*>(stg_all + C::NW * C::STG_W);   // NROW x (TX+1) container indices
     int* next_row = row_off + C::NOFF;
 
@@ -540,7 +556,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
 
     // ---- stage the field stencil ----------------------------------------------------------------
     // All of a thread's loads are issued before the first store (one L2/HBM round trip instead of one
-    // per loop trip: with one block per SM nothing else hides this latency).
+    // per loop trip).
     {
         const double* src[6] = {f.Ex, f.Ey, f.Ez, f.Bx, f.By, f.Bz};
         constexpr int NIT = (C::ESZ + C::NT - 1) / C::NT;
@@ -562,7 +578,8 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
             if (e < C::ESZ) {
                 const int w = tile_word<C>(e % C::EX, (e / C::EX) % C::EY, e / (C::EX * C::EY));
 #pragma unroll
-                for (int cpt = 0; cpt < 6; ++cpt) Et[cpt * C::ESZ + w] = v[it][cpt];
+                for (int cpt = 0; cpt < 6; ++cpt)
+                    if (!(C::trimmed(cpt) && e % C::EX == 0)) Et[C::comp_base(cpt) + w] = v[it][cpt];
             }
         }
     }
@@ -613,8 +630,8 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                     const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy,
                                  ze = (z - g.zmin) * g.inv_dz;
                     const int ci = __double2int_rd(xi), cj = __double2int_rd(et), ck = __double2int_rd(ze);
-                    const int rx = rel_cell(ci, t0x, C::TX, g.nx), ry = rel_cell(cj, t0y, C::TY, g.ny),
-                              rz = rel_cell(ck, t0z, C::TZ, g.nz);
+                    const int rx = rel_cell<DRIFT>(ci, t0x, C::TX, g.nx), ry = rel_cell<DRIFT>(cj, t0y, C::TY, g.ny),
+                              rz = rel_cell<DRIFT>(ck, t0z, C::TZ, g.nz);
                     const bool in_tile = rx >= -DRIFT && rx <= C::TX - 1 + DRIFT && t0x + rx <= g.nx - 1 + DRIFT &&
                                          ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
                                          rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
@@ -744,9 +761,14 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
     }
 }
 
-using Cfg = TileCfg<8, 4, 4, 8, 1>;
+// CfgDrift: a species that has moved since its last sort (particles up to one cell outside their listed
+// cell still gather from shared memory); one block of 8 warps per SM.
+// CfgFresh: right after pic_sort; two blocks of 4 warps per SM (2 x 112.6 KB of shared memory).
+using CfgDrift = TileCfg<8, 4, 4, 8, 1, 1>;
+using CfgFresh = TileCfg<8, 4, 4, 4, 2, 0>;
+static_assert(2 * (CfgFresh::SMEM + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
 
-template <int N>
+template <int N, class Cfg>
 void launch_tile(const Grid& g, const Fields& f, const Particles& p, double q, double h,
                  const unsigned int* cell_offset, DevStatus* status, cudaStream_t st) {
     const int ntx = (g.nx + Cfg::TX - 1) / Cfg::TX, nty = (g.ny + Cfg::TY - 1) / Cfg::TY,
@@ -756,27 +778,42 @@ void launch_tile(const Grid& g, const Fields& f, const Particles& p, double q, d
                                                                            status);
 }
 
+template <int N, class Cfg>
+cudaError_t setup_one() {
+    cudaError_t e = cudaFuncSetAttribute(particles_tile_kernel<N, Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)Cfg::SMEM);
+    if (e == cudaSuccess && Cfg::MINB > 1)
+        e = cudaFuncSetAttribute(particles_tile_kernel<N, Cfg>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 (int)cudaSharedmemCarveoutMaxShared);
+    return e;
+}
+
 }  // namespace
 
 int tile_setup() {
-    cudaError_t e = cudaFuncSetAttribute(particles_tile_kernel<1, Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)Cfg::SMEM);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(particles_tile_kernel<2, Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)Cfg::SMEM);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(particles_tile_kernel<3, Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)Cfg::SMEM);
+    cudaError_t e = setup_one<1, CfgDrift>();
+    if (e == cudaSuccess) e = setup_one<2, CfgDrift>();
+    if (e == cudaSuccess) e = setup_one<3, CfgDrift>();
+    if (e == cudaSuccess) e = setup_one<1, CfgFresh>();
+    if (e == cudaSuccess) e = setup_one<2, CfgFresh>();
+    if (e == cudaSuccess) e = setup_one<3, CfgFresh>();
     return (int)e;
 }
 
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, long long n, double q, double m,
-                          int order, const unsigned int* cell_offset, DevStatus* status, cudaStream_t st) {
+                          int order, const unsigned int* cell_offset, bool fresh, DevStatus* status,
+                          cudaStream_t st) {
     if (n <= 0) return 0;
     const double h = q * g.dt / (2.0 * m);
-    if (order == 1) launch_tile<1>(g, f, p, q, h, cell_offset, status, st);
-    else if (order == 2) launch_tile<2>(g, f, p, q, h, cell_offset, status, st);
-    else launch_tile<3>(g, f, p, q, h, cell_offset, status, st);
+    if (fresh) {
+        if (order == 1) launch_tile<1, CfgFresh>(g, f, p, q, h, cell_offset, status, st);
+        else if (order == 2) launch_tile<2, CfgFresh>(g, f, p, q, h, cell_offset, status, st);
+        else launch_tile<3, CfgFresh>(g, f, p, q, h, cell_offset, status, st);
+    } else {
+        if (order == 1) launch_tile<1, CfgDrift>(g, f, p, q, h, cell_offset, status, st);
+        else if (order == 2) launch_tile<2, CfgDrift>(g, f, p, q, h, cell_offset, status, st);
+        else launch_tile<3, CfgDrift>(g, f, p, q, h, cell_offset, status, st);
+    }
     return 1;
 }
 

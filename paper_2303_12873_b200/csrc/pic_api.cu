@@ -50,7 +50,7 @@ struct pic_ctx {
     int sticky = PIC_OK;
     unsigned long long launches = 0, steps = 0, sorts = 0;
     // options
-    int stage_timing = 0, force_path = 0, yee_tma = 3;
+    int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1;
     YeeMaps yee_maps{};
     std::vector<cudaEvent_t> ev_pool;   // grows on demand; never waited on inside pic_step / pic_sort
     size_t ev_used = 0;
@@ -380,7 +380,8 @@ int pic_step(pic_ctx* c, int nsteps) {
             if (!S.loaded || S.n == 0) continue;
             const Particles& P = S.buf[S.cur];
             if (use_tile_path(c, S)) {
-                c->launches += launch_particles_tile(g, c->f, P, S.n, S.q, S.m, c->order, S.cell_offset, c->status,
+                c->launches += launch_particles_tile(g, c->f, P, S.n, S.q, S.m, c->order, S.cell_offset,
+                                                     S.steps_since_sort == 0 && c->tile_fresh != 0, c->status,
                                                      c->stream);
             } else {
                 launch_particles_global(g, c->f, P, S.n, S.q, S.m, c->order, c->status, c->stream);
@@ -569,6 +570,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
         if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "force_path must be 0, 1 or 2");
         c->force_path = (int)value;
     } else if (!strcmp(name, "yee_tma")) c->yee_tma = (int)value & 3;
+    else if (!strcmp(name, "tile_fresh")) c->tile_fresh = value != 0;
     else return fail(c, PIC_EINVAL, "unknown option '%s'", name);
     return PIC_OK;
 }

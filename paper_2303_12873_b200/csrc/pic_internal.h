@@ -92,8 +92,10 @@ struct TileScratch {
     void* ptr;
     size_t bytes;
 };
+// fresh = no step since the species' last sort (every particle sits in its listed cell): smaller stencil, 2 blocks/SM
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, long long n, double q, double m,
-                          int order, const unsigned int* cell_offset, DevStatus* status, cudaStream_t st);  // kernels launched
+                          int order, const unsigned int* cell_offset, bool fresh, DevStatus* status,
+                          cudaStream_t st);  // kernels launched
 int tile_setup();   // one-time cudaFuncSetAttribute calls; returns cudaError_t as int
 
 }  // namespace pic

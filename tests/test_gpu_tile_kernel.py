@@ -158,3 +158,26 @@ def test_full_size_config2_sampled_parity_and_continuity(ora, Sim):
     # (d) everything went through the fused kernel; only cell crossers took its slow path
     c = g.counters()
     assert c["global"] == 0 and c["fast"] + c["slow"] == N and c["slow"] < 0.12 * N
+
+
+@pytest.mark.parametrize("order", [1, 2, 3])
+@pytest.mark.parametrize("fresh", [0, 1])
+def test_fresh_and_drift_variants_of_the_tile_kernel(ora, Sim, order, fresh):
+    """Right after pic_sort the tile kernel runs its small-stencil, two-blocks-per-SM variant (option
+    tile_fresh = 1, the default); tile_fresh = 0 forces the drift-tolerant variant.  Same arithmetic per
+    particle, so both meet the 1-step bounds; grid sizes ragged against the 8 x 4 x 4 tile, 0.15 c so that
+    every face of a tile is crossed, random fields on all six staggerings."""
+    wl = W.uniform_plasma(19, 10, 7, ppc=9, u_th=0.15, order=order, seed=500 + order, dx=0.4e-6, dy=0.5e-6,
+                          dz=0.3e-6)
+    wl.fields = _rand_fields(wl, 23 + order)
+    o, g = make_pair(ora, Sim, wl, sort_first=True, force_path=2)
+    g.set_option("tile_fresh", fresh)
+    o.step(1)
+    g.step(1)
+    check_step_parity(o, g, wl, "fresh=%d order %d" % (fresh, order))
+    c = g.counters()
+    assert c["global"] == 0 and c["fast"] + c["slow"] == wl.nparticles
+    g.sort()
+    o.step(1)
+    g.step(1)
+    check_step_parity(o, g, wl, "fresh=%d order %d step 2" % (fresh, order))
