@@ -469,48 +469,47 @@ struct CellAcc {
         }
         return true;
     }
-    // Add to the padded global arrays.  o = offset of the window's first node, s = this lane's plane,
-    // buf = NACC x 32 doubles of warp-private shared memory (lane-interleaved).  The accumulators are
-    // spilled there once so that the RED loops can stay rolled (short code, I-cache resident).
-    __device__ __forceinline__ void flush(const Grid& g, const Fields& f, long long o, int s, double* buf,
-                                          int lane) const {
-        double* mine = buf + lane;
+    // One x-line of window values v[a] (node or edge q + FA + a of the cell q = lane >> 2) from all eight cells
+    // of the row: the windows of neighbouring cells overlap in all but one node, so the lanes first add up,
+    // with shuffles, everything that lands on the same global node -- lane q ends up with the total for
+    // node q (a = A0 = -FA of its own window) -- and then issue ONE RED per distinct node (10 or 11 per line
+    // instead of 24 or 32).  p0 = address of this lane's node q on the line.  Called by all 32 lanes.
+    template <int NA, int A0>
+    static __device__ __forceinline__ void flush_line(const double (&v)[NA], double* p0, int lane, bool active) {
+        const int q = lane >> 2;
+        double m = v[A0];
 #pragma unroll
-        for (int b = 0; b < FW; ++b)
+        for (int a = 0; a < NA; ++a) {
+            if (a == A0) continue;
+            const int dq = A0 - a;                      // v[a] of cell q + dq lands on node q
+            const double t = __shfl_sync(0xffffffffu, v[a], (lane + 4 * dq) & 31);
+            if (q + dq >= 0 && q + dq <= 7) m += t;
+        }
+        if (active && m != 0.0) red_add(p0, m);
+        // nodes outside 0 .. 7: -1 (cell 0, a = 0) and 8 (cell 7, a = A0 + 1; cell 6, a = A0 + 2) in one
+        // RED instruction, 9 (cell 7, a = A0 + 2) in another
+        double e = 0.0;
+        if constexpr (A0 + 2 < NA) e = __shfl_sync(0xffffffffu, v[A0 + 2], (lane - 4) & 31);
+        if constexpr (A0 + 1 < NA) e += v[A0 + 1];
+        if constexpr (A0 >= 1) e = (q == 0) ? v[0] : e;
+        if (active && (q == 7 || (A0 >= 1 && q == 0)) && e != 0.0) red_add(q == 0 ? p0 - 1 : p0 + 1, e);
+        if constexpr (A0 + 2 < NA)
+            if (active && q == 7 && v[A0 + 2] != 0.0) red_add(p0 + 2, v[A0 + 2]);
+    }
+    // Add the row's accumulators to the padded global arrays.  o = offset of this lane's window's first node,
+    // s = this lane's plane.  Called by all 32 lanes (lanes with s >= FW hold zeros and only shuffle).
+    __device__ __forceinline__ void flush(const Grid& g, const Fields& f, long long o, int s, int lane) const {
+        constexpr int A0 = -FastWin<N>::FA;
+        const bool active = s < FW;
+        double* px = f.Jx + o + g.sz * s + A0;
 #pragma unroll
-            for (int a = 0; a < FW - 1; ++a) mine[32 * (b * (FW - 1) + a)] = jx[b][a];
+        for (int b = 0; b < FW; ++b) flush_line<FW - 1, A0>(jx[b], px + g.sy * b, lane, active);
+        double* py = f.Jy + o + g.sz * s + A0;
 #pragma unroll
-        for (int b = 0; b < FW - 1; ++b)
+        for (int b = 0; b < FW - 1; ++b) flush_line<FW, A0>(jy[b], py + g.sy * b, lane, active);
+        double* pz = f.Jz + o + g.sy * s + A0;
 #pragma unroll
-            for (int a = 0; a < FW; ++a) {
-                mine[32 * (FW * (FW - 1) + b * FW + a)] = jy[b][a];
-                mine[32 * (2 * FW * (FW - 1) + b * FW + a)] = jz[b][a];
-            }
-        double* pr = f.Jx + o + g.sz * s;
-        const double* src = mine;
-#pragma unroll 1
-        for (int b = 0; b < FW; ++b, pr += g.sy, src += 32 * (FW - 1))
-#pragma unroll
-            for (int a = 0; a < FW - 1; ++a) {
-                const double v = src[32 * a];
-                if (v != 0.0) red_add(pr + a, v);
-            }
-        pr = f.Jy + o + g.sz * s;
-#pragma unroll 1
-        for (int b = 0; b < FW - 1; ++b, pr += g.sy, src += 32 * FW)
-#pragma unroll
-            for (int a = 0; a < FW; ++a) {
-                const double v = src[32 * a];
-                if (v != 0.0) red_add(pr + a, v);
-            }
-        pr = f.Jz + o + g.sy * s;
-#pragma unroll 1
-        for (int c = 0; c < FW - 1; ++c, pr += g.sz, src += 32 * FW)
-#pragma unroll
-            for (int a = 0; a < FW; ++a) {
-                const double v = src[32 * a];
-                if (v != 0.0) red_add(pr + a, v);
-            }
+        for (int c = 0; c < FW - 1; ++c) flush_line<FW, A0>(jz[c], pz + g.sz * c, lane, active);
     }
 };
 
@@ -524,7 +523,6 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                       int ntx, int nty, DevStatus* status) {
     constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA, DRIFT = C::DRIFT;
     using FR = FastRec<N>;
-    static_assert(CellAcc<N>::NACC * 32 <= C::STG_W, "flush buffer does not fit the staging area");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* Et = reinterpret_cast<double*>(smem_raw);            // TOT words: Ex Ey Ez Bx By Bz
     double* stg_all = Et + C::TOT;                               // NW * STG_W
@@ -746,8 +744,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
             __syncwarp();
         }
         // ---------------- flush the row's accumulators ---------------------------------------------
-        if (bs < FW) acc.flush(g, f, win0, bs, stg, lane);
-        __syncwarp();
+        acc.flush(g, f, win0, bs, lane);
     }
     // ---- flags and counters ----------------------------------------------------------------------
     if (bad_any) status->ephys = 1;
