@@ -56,14 +56,15 @@ YEE_BYTES_PER_CELL = 240.0
 # fp64-pipe roofline of the fused kernel.  Instructions per particle = DFMA + DMUL + DADD
 # thread instructions executed per particle by the committed kernel (ncu, profiles/); order 3 measured,
 # orders 1 and 2 scaled by the gather/deposit operation counts.
-FP64_INSTR_PER_PARTICLE = {1: 400.0, 2: 750.0, 3: 1116.0}
+FP64_INSTR_PER_PARTICLE = {1: 400.0, 2: 750.0, 3: 1094.0}
 FP64_LANES_PER_SM = 64
 N_SM = 148
 SM_MAX_MHZ = 1965.0
-# shared-memory bytes the kernel moves per particle at order 3 (gather 384 x 8 B, staging, phase B)
-SMEM_BYTES_PER_PARTICLE = {1: 1100.0, 2: 2600.0, 3: 5100.0}
+# shared-memory bytes the kernel moves per particle: order 3 = 41.1 wavefronts x 128 B (ncu, profiles/r01_v4);
+# orders 1 and 2 scaled by the gather/deposit operand counts
+SMEM_BYTES_PER_PARTICLE = {1: 1100.0, 2: 2700.0, 3: 5270.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch at the default workload (profiles/)
-TRAFFIC_BYTES_PER_LAUNCH = 17.90e9
+TRAFFIC_BYTES_PER_LAUNCH = 17.46e9
 
 
 def _peaks():
@@ -299,6 +300,13 @@ def run_ours(args):
               "sorts_in_timed_region": int(st["sorts"]),
               "yee_cell_updates_per_s": ncell / (yee_ms * 1e-3) if yee_ms > 0 else None,
               "yee_gbs": YEE_BYTES_PER_CELL * ncell / (yee_ms * 1e-3) / 1e9 if yee_ms > 0 else None}
+    roofline_yee = None
+    if yee_ms > 0:
+        yee_gbs = YEE_BYTES_PER_CELL * ncell / (yee_ms * 1e-3) / 1e9
+        roofline_yee = {"bound": "hbm", "kernel": "push_B_tma_kernel x2 + push_E_tma_kernel", "achieved": yee_gbs,
+                        "peak": hbm_peak, "peak_kind": hbm_kind, "unit": "GB/s", "frac": yee_gbs / hbm_peak,
+                        "algorithmic_bytes_per_step": YEE_BYTES_PER_CELL * ncell,
+                        "cell_updates_per_s": ncell / (yee_ms * 1e-3)}
     paths = {k: c1[k] - c0[k] for k in ("fast", "slow", "global")}
 
     # ---- end to end through the C ABI with pinned HOST buffers (rank-local; max over ranks) ----
@@ -357,7 +365,8 @@ def run_ours(args):
                            (BYTES_PER_PARTICLE * npart + 9 * 8 * ncell) / 1e9),
                        "generation_s": round(t_gen, 1)},
             "cell_updates_per_s": world * ncell * args.steps / (ms_total * 1e-3),
-            "roofline": roofline, "roofline_hbm": roofline_hbm, "roofline_smem": roofline_smem, "stages": stages, "particle_paths": paths,
+            "roofline": roofline, "roofline_hbm": roofline_hbm, "roofline_smem": roofline_smem,
+            "roofline_yee": roofline_yee, "stages": stages, "particle_paths": paths,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(c1["launches"] - c0["launches"]),
             "clocks": clk}
     print(json.dumps(line))
