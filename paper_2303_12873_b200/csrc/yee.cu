@@ -14,7 +14,7 @@
 // Two implementations of each push:
 //   *_kernel      one thread per cell, every operand a global load (12 loads per cell; the +-1 rows in
 //                 y and z miss L1, so the kernel is L1/L2-throughput bound at ~40 % of the HBM roofline);
-//   *_tma_kernel  one block per 32 x 8 x 8 tile: the three curl operands (+ a one-cell halo) are staged
+//   *_tma_kernel  one block per 32 x 8 x 4 (B push) or 32 x 8 x 8 (E push) tile: the three curl operands (+ a one-cell halo) are staged
 //                 in shared memory by TMA (cp.async.bulk.tensor.3d, one thread, mbarrier
 //                 completion) while the threads fetch the component they update; the padded guard cells
 //                 mean a box never wraps, and boxes that poke out of the array are zero-filled.
@@ -80,15 +80,16 @@ __global__ void __launch_bounds__(128) push_E_kernel(Grid g, Fields f, double cd
 // ---- TMA-staged variant ------------------------------------------------------------------------
 namespace {
 
-constexpr int YTX = 32, YTY = 8, YTZ = 8;                  // cells per block
+constexpr int YTX = 32, YTY = 8;                           // cells per block in x, y (one thread each)
+constexpr int YTZ_B = 4, YTZ_E = 8;                        // z planes a thread walks (measured best: 256^3, profiles/r01_v4)                  // cells per block
 // Staged box: the tile plus one halo cell in y and z and, in x, 2 cells: with 8-byte elements the box corner
 // must sit on an EVEN x coordinate (TMA wants the first byte of a box row 16-byte aligned; an odd coordinate
 // raises "illegal instruction"), so the E push (backward differences) starts 2 cells below the tile, not 1.
 // Row = 34 or 36 doubles = 272 / 288 B: a multiple of 16 B as TMA requires.
-constexpr int YBY = YTY + 1, YBZ = YTZ + 1;
-template <int HX> struct YeeBox {
-    static constexpr int BX = YTX + HX;
-    static constexpr int SZ = BX * YBY * YBZ;
+constexpr int YBY = YTY + 1;
+template <int HX, int TZ> struct YeeBox {
+    static constexpr int BX = YTX + HX, BZ = TZ + 1;
+    static constexpr int SZ = BX * YBY * BZ;
     static constexpr int PAD = (SZ + 15) / 16 * 16;        // every TMA destination starts on a 128-byte boundary
 };
 constexpr int YNT = 256;
@@ -122,20 +123,20 @@ __device__ __forceinline__ void tma_load_box(double* dst, const CUtensorMap* map
         "r"(smem_u32(bar)) : "memory");
 }
 
-template <int HX> struct YeeSmem {
-    alignas(128) double box[3][YeeBox<HX>::PAD];
+template <int HX, int TZ> struct YeeSmem {
+    alignas(128) double box[3][YeeBox<HX, TZ>::PAD];
     alignas(8) unsigned long long bar;
 };
 
 // Box corner = (tile's first cell) - (shx, sh, sh): sh = 0 for forward differences (B push), 1 for backward
 // differences (E push, shx = 2 to stay on an even x coordinate).
-template <int HX>
-__device__ __forceinline__ void stage_boxes(YeeSmem<HX>& sm, const CUtensorMap* m0, const CUtensorMap* m1,
+template <int HX, int TZ>
+__device__ __forceinline__ void stage_boxes(YeeSmem<HX, TZ>& sm, const CUtensorMap* m0, const CUtensorMap* m1,
                                             const CUtensorMap* m2, int t0x, int t0y, int t0z, int shx, int sh) {
     if (threadIdx.x == 0) mbar_init(&sm.bar, 1);
     __syncthreads();
     if (threadIdx.x == 0) {
-        mbar_expect_tx(&sm.bar, 3u * YeeBox<HX>::SZ * (unsigned)sizeof(double));
+        mbar_expect_tx(&sm.bar, 3u * YeeBox<HX, TZ>::SZ * (unsigned)sizeof(double));
         tma_load_box(sm.box[0], m0, &sm.bar, t0x + NG - shx, t0y + NG - sh, t0z + NG - sh);
         tma_load_box(sm.box[1], m1, &sm.bar, t0x + NG - shx, t0y + NG - sh, t0z + NG - sh);
         tma_load_box(sm.box[2], m2, &sm.bar, t0x + NG - shx, t0y + NG - sh, t0z + NG - sh);
@@ -144,15 +145,16 @@ __device__ __forceinline__ void stage_boxes(YeeSmem<HX>& sm, const CUtensorMap* 
 
 }  // namespace
 
+template <int YTZ>
 __global__ void __launch_bounds__(YNT) push_B_tma_kernel(Grid g, Fields f, double cdx, double cdy, double cdz,
                                                          const __grid_constant__ CUtensorMap mEx,
                                                          const __grid_constant__ CUtensorMap mEy,
                                                          const __grid_constant__ CUtensorMap mEz) {
     extern __shared__ __align__(128) unsigned char yee_smem_raw[];
-    constexpr int YBX = YeeBox<2>::BX;
-    YeeSmem<2>& sm = *reinterpret_cast<YeeSmem<2>*>(yee_smem_raw);
+    constexpr int YBX = YeeBox<2, YTZ>::BX;
+    YeeSmem<2, YTZ>& sm = *reinterpret_cast<YeeSmem<2, YTZ>*>(yee_smem_raw);
     const int t0x = blockIdx.x * YTX, t0y = blockIdx.y * YTY, t0z = blockIdx.z * YTZ;
-    stage_boxes<2>(sm, &mEx, &mEy, &mEz, t0x, t0y, t0z, 0, 0);
+    stage_boxes<2, YTZ>(sm, &mEx, &mEy, &mEz, t0x, t0y, t0z, 0, 0);
     const int tx = threadIdx.x % YTX, ty = threadIdx.x / YTX;     // 32 x 8 threads, each walks the 8 z planes
     const int i = t0x + tx, j = t0y + ty;
     const bool in_xy = i < g.nx && j < g.ny;
@@ -186,15 +188,16 @@ __global__ void __launch_bounds__(YNT) push_B_tma_kernel(Grid g, Fields f, doubl
     }
 }
 
+template <int YTZ>
 __global__ void __launch_bounds__(YNT) push_E_tma_kernel(Grid g, Fields f, double cdx, double cdy, double cdz,
                                                          double dt_eps0, const __grid_constant__ CUtensorMap mBx,
                                                          const __grid_constant__ CUtensorMap mBy,
                                                          const __grid_constant__ CUtensorMap mBz) {
     extern __shared__ __align__(128) unsigned char yee_smem_raw[];
-    constexpr int YBX = YeeBox<4>::BX;
-    YeeSmem<4>& sm = *reinterpret_cast<YeeSmem<4>*>(yee_smem_raw);
+    constexpr int YBX = YeeBox<4, YTZ>::BX;
+    YeeSmem<4, YTZ>& sm = *reinterpret_cast<YeeSmem<4, YTZ>*>(yee_smem_raw);
     const int t0x = blockIdx.x * YTX, t0y = blockIdx.y * YTY, t0z = blockIdx.z * YTZ;
-    stage_boxes<4>(sm, &mBx, &mBy, &mBz, t0x, t0y, t0z, 2, 1);
+    stage_boxes<4, YTZ>(sm, &mBx, &mBy, &mBz, t0x, t0y, t0z, 2, 1);
     const int tx = threadIdx.x % YTX, ty = threadIdx.x / YTX;
     const int i = t0x + tx, j = t0y + ty;
     const bool in_xy = i < g.nx && j < g.ny;
@@ -235,9 +238,9 @@ __global__ void __launch_bounds__(YNT) push_E_tma_kernel(Grid g, Fields f, doubl
 void launch_push_B(const Grid& g, const Fields& f, double dth, const YeeMaps* maps, cudaStream_t st) {
     const double cdx = dth * g.inv_dx, cdy = dth * g.inv_dy, cdz = dth * g.inv_dz;
     if (maps && maps->valid) {
-        dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ - 1) / YTZ);
+        dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ_B - 1) / YTZ_B);
         const CUtensorMap* m = reinterpret_cast<const CUtensorMap*>(maps->map);
-        push_B_tma_kernel<<<nb, YNT, sizeof(YeeSmem<2>), st>>>(g, f, cdx, cdy, cdz, m[0], m[1], m[2]);
+        push_B_tma_kernel<YTZ_B><<<nb, YNT, sizeof(YeeSmem<2, YTZ_B>), st>>>(g, f, cdx, cdy, cdz, m[0], m[1], m[2]);
     } else {
         dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
         push_B_kernel<<<nb, bs, 0, st>>>(g, f, cdx, cdy, cdz);
@@ -248,9 +251,9 @@ void launch_push_E(const Grid& g, const Fields& f, double dt, const YeeMaps* map
     const double c2dt = C_LIGHT * C_LIGHT * dt;
     const double cdx = c2dt * g.inv_dx, cdy = c2dt * g.inv_dy, cdz = c2dt * g.inv_dz;
     if (maps && maps->valid) {
-        dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ - 1) / YTZ);
+        dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ_E - 1) / YTZ_E);
         const CUtensorMap* m = reinterpret_cast<const CUtensorMap*>(maps->map);
-        push_E_tma_kernel<<<nb, YNT, sizeof(YeeSmem<4>), st>>>(g, f, cdx, cdy, cdz, dt / EPS0, m[3], m[4], m[5]);
+        push_E_tma_kernel<YTZ_E><<<nb, YNT, sizeof(YeeSmem<4, YTZ_E>), st>>>(g, f, cdx, cdy, cdz, dt / EPS0, m[3], m[4], m[5]);
     } else {
         dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
         push_E_kernel<<<nb, bs, 0, st>>>(g, f, cdx, cdy, cdz, dt / EPS0);
@@ -258,7 +261,7 @@ void launch_push_E(const Grid& g, const Fields& f, double dt, const YeeMaps* map
 }
 
 // Tensor maps of the six padded E,B components (rank 3, fp64, no swizzle, zero fill outside the array),
-// box = (YTX + 2) x YBY x YBZ for E (read by the B push), (YTX + 4) x YBY x YBZ for B.  The driver entry point is fetched through the runtime (no link-time libcuda).
+// box = (YTX + 2) x YBY x (YTZ_B + 1) for E (read by the B push), (YTX + 4) x YBY x (YTZ_E + 1) for B.  The driver entry point is fetched through the runtime (no link-time libcuda).
 int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out) {
     static_assert(sizeof(CUtensorMap) == 128 && sizeof(out->map) == 6 * 128, "YeeMaps storage");
     out->valid = 0;
@@ -278,15 +281,18 @@ int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out) {
     const cuuint64_t strides[2] = {(cuuint64_t)g.px * 8, (cuuint64_t)g.px * (cuuint64_t)g.py * 8};
     const cuuint32_t estr[3] = {1, 1, 1};
     for (int k = 0; k < 6; ++k) {
-        const cuuint32_t box[3] = {(cuuint32_t)(k < 3 ? YeeBox<2>::BX : YeeBox<4>::BX), YBY, YBZ};
+        const cuuint32_t box[3] = {(cuuint32_t)(k < 3 ? YeeBox<2, YTZ_B>::BX : YeeBox<4, YTZ_E>::BX), YBY,
+                                   (cuuint32_t)(k < 3 ? YeeBox<2, YTZ_B>::BZ : YeeBox<4, YTZ_E>::BZ)};
         CUresult r = ((EncodeFn)fn)(&m[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, comp[k], dims, strides, box, estr,
                                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return 2;
     }
-    if (cudaFuncSetAttribute(push_B_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(YeeSmem<2>)) !=
+    if (cudaFuncSetAttribute(push_B_tma_kernel<YTZ_B>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(YeeSmem<2, YTZ_B>)) !=
             cudaSuccess ||
-        cudaFuncSetAttribute(push_E_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(YeeSmem<4>)) !=
+        cudaFuncSetAttribute(push_E_tma_kernel<YTZ_E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(YeeSmem<4, YTZ_E>)) !=
             cudaSuccess) {
         cudaGetLastError();
         return 3;
