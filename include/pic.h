@@ -217,6 +217,13 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    last pic_sort runs the small-stencil, two-blocks-per-SM
  *                    variant of the fused per-tile kernel; 0 = always the
  *                    drift-tolerant variant (same arithmetic per particle)
+ *   "sort_deferred"  1 (default) = pic_sort writes only the permutation (4 B per
+ *                    particle); the particle data are moved by the next fused
+ *                    per-tile kernel, which reads its inputs through the
+ *                    permutation and writes its outputs in sorted order (any
+ *                    other reader -- pic_get_particles, the global-atomic
+ *                    kernel -- triggers the move first); 0 = pic_sort moves
+ *                    the data itself.  Same result either way.
  * Unknown name: PIC_EINVAL.
  */
 int pic_set_option(pic_ctx*, const char* name, long long value);

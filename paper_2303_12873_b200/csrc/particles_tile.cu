@@ -253,8 +253,16 @@ __device__ __forceinline__ void red_add(double* p, double v) {
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // pull one 32-particle sub-chunk of the SoA arrays towards the SM ahead of its use
-__device__ __forceinline__ void prefetch_particles(const Particles& p, int ip, int hi) {
+// (delta = where the sorted position's data sits in the source buffer relative to the position itself:
+// 0 in place, else the shift of the row's first particle under the deferred-sort permutation)
+__device__ __forceinline__ void prefetch_particles(const Particles& p, const unsigned int* perm, int ip, int hi,
+                                                   int delta) {
     if (ip < hi) {
+        if (perm != nullptr) {
+            prefetch_l1(perm + ip);
+            prefetch_l1(p.id + ip + delta);
+        }
+        ip += delta;
         prefetch_l1(p.x + ip); prefetch_l1(p.y + ip); prefetch_l1(p.z + ip);
         prefetch_l1(p.ux + ip); prefetch_l1(p.uy + ip); prefetch_l1(p.uz + ip);
         prefetch_l1(p.w + ip);
@@ -519,8 +527,8 @@ namespace {
 
 template <int N, class C>
 __global__ void __launch_bounds__(C::NT, C::MINB)
-particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const unsigned int* __restrict__ cell_offset,
-                      int ntx, int nty, DevStatus* status) {
+particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigned int* __restrict__ perm, double q,
+                      double h, const unsigned int* __restrict__ cell_offset, int ntx, int nty, DevStatus* status) {
     constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA, DRIFT = C::DRIFT;
     using FR = FastRec<N>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -528,6 +536,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
     double* stg_all = Et + C::TOT;                               // NW * STG_W
     int* row_off = reinterpret_cast<int*>(stg_all + C::NW * C::STG_W);   // NROW x (TX+1) container indices
     int* next_row = row_off + C::NOFF;
+    __shared__ int row_delta[C::NROW];     // deferred sort: perm[first particle of the row] - its sorted position
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     int b = blockIdx.x;
@@ -546,7 +555,12 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
         row_off[e] = v;
     }
     if (tid == 0) *next_row = 0;
+    if (tid < C::NROW) row_delta[tid] = 0;
     __syncthreads();
+    if (perm != nullptr && tid < C::NROW) {
+        const int lo = row_off[tid * (C::TX + 1)], hi = row_off[tid * (C::TX + 1) + C::TX];
+        if (lo < hi) row_delta[tid] = (int)perm[lo] - lo;     // read by the row's warp long after the stencil barrier
+    }
     int n_tile = 0;
 #pragma unroll 4
     for (int r = 0; r < C::NROW; ++r) n_tile += row_off[r * (C::TX + 1) + C::TX] - row_off[r * (C::TX + 1)];
@@ -600,13 +614,15 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
         row_ahead = __shfl_sync(0xffffffffu, row_ahead, 0);
         if (row_ahead < C::NROW) {
             const int* offn = row_off + row_ahead * (C::TX + 1);
-            prefetch_particles(p, offn[0] + lane, offn[C::TX]);
-            prefetch_particles(p, offn[0] + 32 + lane, offn[C::TX]);
+            const int dl = row_delta[row_ahead];
+            prefetch_particles(p, perm, offn[0] + lane, offn[C::TX], dl);
+            prefetch_particles(p, perm, offn[0] + 32 + lane, offn[C::TX], dl);
         }
         const int* off = row_off + row * (C::TX + 1);
         const int row_lo = off[0], row_hi = off[C::TX];
         if (row_lo >= row_hi) continue;
         const int ry0 = row % C::TY, rz0 = row / C::TY;     // the row's tile-relative (y, z) cell
+        const int delta = row_delta[row];
         const int cell_lo = off[bq], cell_hi = off[bq + 1];  // phase B: this lane's cell
         CellAcc<N> acc;
         acc.clear();
@@ -618,13 +634,19 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
             for (int sub = 0; sub < C::CHUNK; sub += 32) {
                 const int ip = base + sub + lane;
                 if (base + sub >= row_hi) break;
-                prefetch_particles(p, ip + 64, row_hi);   // rows longer than the two sub-chunks prefetched a row ahead
+                prefetch_particles(p, perm, ip + 64, row_hi, delta);   // rows longer than the two sub-chunks prefetched a row ahead
                 double* rec = stg + skew(sub + lane) * C::PITCH;
                 bool is_slow = false;
                 if (ip < row_hi) {
-                    const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
-                    double ux = p.ux[ip], uy = p.uy[ip], uz = p.uz[ip];
-                    const double qw = q * p.w[ip];
+                    const int is = (perm != nullptr) ? (int)perm[ip] : ip;     // where this particle's data sits
+                    const double x = p.x[is], y = p.y[is], z = p.z[is];
+                    double ux = p.ux[is], uy = p.uy[is], uz = p.uz[is];
+                    const double wgt = p.w[is];
+                    const double qw = q * wgt;
+                    if (perm != nullptr) {          // deferred sort: the other buffer gets every array, in sorted order
+                        po.w[ip] = wgt;
+                        po.id[ip] = p.id[is];
+                    }
                     const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy,
                                  ze = (z - g.zmin) * g.inv_dz;
                     const int ci = __double2int_rd(xi), cj = __double2int_rd(et), ck = __double2int_rd(ze);
@@ -659,12 +681,12 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
                     const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
                                      !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
                     bad_any = bad_any || bad;
-                    p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
-                    p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
-                    p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
-                    p.ux[ip] = ux;
-                    p.uy[ip] = uy;
-                    p.uz[ip] = uz;
+                    po.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
+                    po.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
+                    po.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
+                    po.ux[ip] = ux;
+                    po.uy[ip] = uy;
+                    po.uz[ip] = uz;
                     // ---- classify: fast = stayed inside the cell the sort listed it in -------------
                     int lc = 0;
 #pragma unroll
@@ -763,16 +785,16 @@ particles_tile_kernel(Grid g, Fields f, Particles p, double q, double h, const u
 // CfgFresh: right after pic_sort; two blocks of 4 warps per SM (2 x 112.6 KB of shared memory).
 using CfgDrift = TileCfg<8, 4, 4, 8, 1, 1>;
 using CfgFresh = TileCfg<8, 4, 4, 4, 2, 0>;
-static_assert(2 * (CfgFresh::SMEM + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
+static_assert(2 * (CfgFresh::SMEM + 64 + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
 
 template <int N, class Cfg>
-void launch_tile(const Grid& g, const Fields& f, const Particles& p, double q, double h,
-                 const unsigned int* cell_offset, DevStatus* status, cudaStream_t st) {
+void launch_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po, const unsigned int* perm,
+                 double q, double h, const unsigned int* cell_offset, DevStatus* status, cudaStream_t st) {
     const int ntx = (g.nx + Cfg::TX - 1) / Cfg::TX, nty = (g.ny + Cfg::TY - 1) / Cfg::TY,
               ntz = (g.nz + Cfg::TZ - 1) / Cfg::TZ;
     const long long nb = (long long)ntx * nty * ntz;
-    particles_tile_kernel<N, Cfg><<<(unsigned)nb, Cfg::NT, Cfg::SMEM, st>>>(g, f, p, q, h, cell_offset, ntx, nty,
-                                                                           status);
+    particles_tile_kernel<N, Cfg><<<(unsigned)nb, Cfg::NT, Cfg::SMEM, st>>>(g, f, p, po, perm, q, h, cell_offset, ntx,
+                                                                           nty, status);
 }
 
 template <int N, class Cfg>
@@ -797,19 +819,19 @@ int tile_setup() {
     return (int)e;
 }
 
-int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, long long n, double q, double m,
-                          int order, const unsigned int* cell_offset, bool fresh, DevStatus* status,
-                          cudaStream_t st) {
+int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po,
+                          const unsigned int* perm, long long n, double q, double m, int order,
+                          const unsigned int* cell_offset, bool fresh, DevStatus* status, cudaStream_t st) {
     if (n <= 0) return 0;
     const double h = q * g.dt / (2.0 * m);
     if (fresh) {
-        if (order == 1) launch_tile<1, CfgFresh>(g, f, p, q, h, cell_offset, status, st);
-        else if (order == 2) launch_tile<2, CfgFresh>(g, f, p, q, h, cell_offset, status, st);
-        else launch_tile<3, CfgFresh>(g, f, p, q, h, cell_offset, status, st);
+        if (order == 1) launch_tile<1, CfgFresh>(g, f, p, po, perm, q, h, cell_offset, status, st);
+        else if (order == 2) launch_tile<2, CfgFresh>(g, f, p, po, perm, q, h, cell_offset, status, st);
+        else launch_tile<3, CfgFresh>(g, f, p, po, perm, q, h, cell_offset, status, st);
     } else {
-        if (order == 1) launch_tile<1, CfgDrift>(g, f, p, q, h, cell_offset, status, st);
-        else if (order == 2) launch_tile<2, CfgDrift>(g, f, p, q, h, cell_offset, status, st);
-        else launch_tile<3, CfgDrift>(g, f, p, q, h, cell_offset, status, st);
+        if (order == 1) launch_tile<1, CfgDrift>(g, f, p, po, perm, q, h, cell_offset, status, st);
+        else if (order == 2) launch_tile<2, CfgDrift>(g, f, p, po, perm, q, h, cell_offset, status, st);
+        else launch_tile<3, CfgDrift>(g, f, p, po, perm, q, h, cell_offset, status, st);
     }
     return 1;
 }

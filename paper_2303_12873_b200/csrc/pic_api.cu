@@ -24,6 +24,10 @@ struct Species {
     int cur = 0;                // which of the two SoA buffers is live
     Particles buf[2];
     unsigned int* cell_offset = nullptr;
+    // Deferred sort: pic_sort wrote only perm[] (sorted position -> index in buf[cur]); the data is permuted by
+    // the next fused particle kernel (which writes buf[cur ^ 1]) or by materialize() for any other reader.
+    unsigned int* perm = nullptr;
+    bool perm_pending = false;
 };
 
 constexpr int NSTAGE = PIC_NSTAGES;
@@ -50,7 +54,7 @@ struct pic_ctx {
     int sticky = PIC_OK;
     unsigned long long launches = 0, steps = 0, sorts = 0;
     // options
-    int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1;
+    int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1;
     YeeMaps yee_maps{};
     std::vector<cudaEvent_t> ev_pool;   // grows on demand; never waited on inside pic_step / pic_sort
     size_t ev_used = 0;
@@ -85,7 +89,8 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 int padded_pitch(int nx) { return (nx + 2 * NG + 1) & ~1; }   // even: rows stay 16-byte aligned (TMA)
 
 struct Layout {
-    size_t status, fields, tmp, species[MAX_SPECIES], cell_offset[MAX_SPECIES], key, rank, block_sums, total;
+    size_t status, fields, tmp, species[MAX_SPECIES], cell_offset[MAX_SPECIES], perm[MAX_SPECIES], key, rank, block_sums,
+        total;
     size_t comp_bytes, np_bytes[MAX_SPECIES];
 };
 
@@ -102,6 +107,7 @@ int make_layout(int nx, int ny, int nz, int nspecies, const long long* np_max, L
         L->np_bytes[s] = align_up((size_t)np_max[s] * sizeof(double));
         L->species[s] = off; off += 2 * 8 * L->np_bytes[s];
         L->cell_offset[s] = off; off += align_up((ncell + 1) * sizeof(unsigned int));
+        L->perm[s] = off; off += align_up((size_t)np_max[s] * sizeof(unsigned int));
         if (np_max[s] > npm) npm = np_max[s];
     }
     L->key = off; off += align_up((size_t)npm * sizeof(unsigned int));
@@ -211,6 +217,15 @@ bool use_tile_path(const pic_ctx* c, const Species& s) {
     return s.sorted;
 }
 
+// Carry out a deferred sort for a reader other than the fused per-tile kernel.
+void materialize(pic_ctx* c, Species& S) {
+    if (!S.perm_pending) return;
+    launch_apply_perm(S.buf[S.cur], S.buf[S.cur ^ 1], S.n, S.perm, c->stream);
+    if (S.n > 0) c->launches += 1;
+    S.cur ^= 1;
+    S.perm_pending = false;
+}
+
 }  // namespace
 
 extern "C" {
@@ -277,6 +292,7 @@ int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, d
             S.buf[b].id = (unsigned long long*)(pb + (size_t)7 * L.np_bytes[s]);
         }
         S.cell_offset = (unsigned int*)(base + L.cell_offset[s]);
+        S.perm = (unsigned int*)(base + L.perm[s]);
     }
     c->sort_scratch.key = (unsigned int*)(base + L.key);
     c->sort_scratch.rank = (unsigned int*)(base + L.rank);
@@ -319,6 +335,7 @@ int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n,
     Species& S = c->sp[species];
     if (n > S.np_max) return fail(c, PIC_ENOMEM, "n = %lld exceeds np_max = %lld", n, S.np_max);
     S.cur = 0;
+    S.perm_pending = false;
     Particles& P = S.buf[0];
     const double* src[7] = {x, y, z, ux, uy, uz, w};
     double* dst[7] = {P.x, P.y, P.z, P.ux, P.uy, P.uz, P.w};
@@ -378,13 +395,21 @@ int pic_step(pic_ctx* c, int nsteps) {
         for (int s = 0; s < c->nspecies; ++s) {
             Species& S = c->sp[s];
             if (!S.loaded || S.n == 0) continue;
-            const Particles& P = S.buf[S.cur];
             if (use_tile_path(c, S)) {
-                c->launches += launch_particles_tile(g, c->f, P, S.n, S.q, S.m, c->order, S.cell_offset,
-                                                     S.steps_since_sort == 0 && c->tile_fresh != 0, c->status,
-                                                     c->stream);
+                // a deferred sort is carried out here: inputs read through perm, outputs to the other buffer
+                const bool deferred = S.perm_pending;
+                const Particles& P = S.buf[S.cur];
+                const Particles& PO = deferred ? S.buf[S.cur ^ 1] : P;
+                c->launches += launch_particles_tile(g, c->f, P, PO, deferred ? S.perm : nullptr, S.n, S.q, S.m, c->order,
+                                                     S.cell_offset, S.steps_since_sort == 0 && c->tile_fresh != 0,
+                                                     c->status, c->stream);
+                if (deferred) {
+                    S.cur ^= 1;
+                    S.perm_pending = false;
+                }
             } else {
-                launch_particles_global(g, c->f, P, S.n, S.q, S.m, c->order, c->status, c->stream);
+                materialize(c, S);
+                launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->status, c->stream);
                 c->launches += 1;
             }
             S.steps_since_sort += 1;
@@ -428,9 +453,12 @@ int pic_sort(pic_ctx* c) {
     for (int s = 0; s < c->nspecies; ++s) {
         Species& S = c->sp[s];
         if (!S.loaded) continue;
-        c->launches += launch_sort(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, S.cell_offset, c->sort_scratch,
-                                   c->stream);
-        S.cur ^= 1;
+        // (a still pending deferred sort is simply superseded: the keys are taken from the unsorted buffer)
+        const bool deferred = c->sort_deferred != 0 && c->force_path != 1;
+        c->launches += launch_sort(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, S.cell_offset,
+                                   deferred ? S.perm : nullptr, c->sort_scratch, c->stream);
+        if (deferred) S.perm_pending = S.n > 0;
+        else { S.cur ^= 1; S.perm_pending = false; }
         S.sorted = true;
         S.steps_since_sort = 0;
     }
@@ -462,6 +490,7 @@ int pic_get_particles(pic_ctx* c, int species, long long* n, double* x, double* 
     Species& S = c->sp[species];
     if (!S.loaded) return fail(c, PIC_ESTATE, "species %d was never loaded", species);
     if (n) *n = S.n;
+    materialize(c, S);
     const Particles& P = S.buf[S.cur];
     const cudaMemcpyKind kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     void* dst[8] = {x, y, z, ux, uy, uz, w, id};
@@ -571,6 +600,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
         c->force_path = (int)value;
     } else if (!strcmp(name, "yee_tma")) c->yee_tma = (int)value & 3;
     else if (!strcmp(name, "tile_fresh")) c->tile_fresh = value != 0;
+    else if (!strcmp(name, "sort_deferred")) c->sort_deferred = value != 0;
     else return fail(c, PIC_EINVAL, "unknown option '%s'", name);
     return PIC_OK;
 }

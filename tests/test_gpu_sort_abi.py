@@ -167,3 +167,41 @@ def test_error_codes(B):
     with pytest.raises(B.PicError) as e:
         g.sync()
     assert e.value.code == B.PIC_EPHYS
+
+
+@pytest.mark.parametrize("deferred", [0, 1])
+def test_deferred_and_immediate_sort_give_the_same_state(ora, B, deferred):
+    """sort_deferred = 1 (default): pic_sort writes only the permutation and the next fused per-tile kernel (or
+    pic_get_particles, or the global-atomic kernel) moves the data; 0: pic_sort moves it.  Every reader must
+    see the sorted container either way: sort -> get, sort -> step -> get, sort -> sort -> step, sort ->
+    rho -> step on the global path, and the physics stays within the 1-step bounds of the oracle."""
+    from parity_util import check_step_parity
+    wl = W.uniform_plasma(13, 9, 6, ppc=7, u_th=0.2, order=3, seed=71, shuffle=True, protons=True)
+    o, g = make_pair(ora, B.Sim, wl)
+    g.set_option("sort_deferred", deferred)
+    before = [g.get_particles(s) for s in range(2)]
+    g.sort()
+    rho = g.deposit_rho(0)                        # reads the (possibly not yet moved) container: order-free
+    assert np.abs(rho - o.deposit_rho(0)).max() <= 1e-12 * np.abs(rho).max()
+    g.sort()                                       # supersedes a pending permutation
+    for s in range(2):
+        after = g.get_particles(s)                 # forces the move
+        key = ora.cell_keys(o.g, after["x"], after["y"], after["z"])
+        assert (np.diff(key) >= 0).all()
+        a, b = by_id(after), by_id(before[s])
+        for k in ("x", "y", "z", "ux", "uy", "uz", "w"):
+            assert np.array_equal(a[k], b[k]), k
+    g.sort()
+    o.step(1); g.step(1)                           # tile kernel consumes the permutation
+    check_step_parity(o, g, wl, "deferred=%d step 1" % deferred)
+    for s in range(2):                             # outputs were written in sorted order of the OLD positions
+        off = g.get_cell_offsets(s).astype(np.int64)
+        assert off[-1] == wl.species[s].n
+    g.sort()
+    g.set_option("force_path", 1)                  # global-atomic kernel: materialises the pending permutation
+    o.step(1); g.step(1)
+    check_step_parity(o, g, wl, "deferred=%d step 2 (global path)" % deferred)
+    g.set_option("force_path", 0)
+    g.sort()
+    o.step(2); g.step(2)                           # one permuted step, one in-place (drift variant) step
+    check_step_parity(o, g, wl, "deferred=%d steps 3-4" % deferred)
