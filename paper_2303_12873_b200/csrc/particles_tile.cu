@@ -44,7 +44,7 @@ struct FastWin {
 // that has moved since its last pic_sort, 0 right after a sort (every particle is in its listed cell), which
 // shrinks the stencil from 14 x 10 x 10 to 12 x 8 x 8 nodes per component so that TWO blocks fit one SM
 // and one block's prologue (stencil staging: every warp of the block waits) overlaps the other's particles.
-template <int TX_, int TY_, int TZ_, int NW_, int MINB_, int DRIFT_>
+template <int TX_, int TY_, int TZ_, int NW_, int MINB_, int DRIFT_, int CHUNK_>
 struct TileCfg {
     static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NW = NW_, NT = 32 * NW_, MINB = MINB_, DRIFT = DRIFT_;
     static constexpr int NROW = TY * TZ;
@@ -69,9 +69,11 @@ struct TileCfg {
                       : (k == 4 ? 4 * FP - 3 * SX : 5 * FP - 3 * SX))));
     }
     // per-warp staging: CHUNK skewed slots of PITCH doubles (PITCH/2 odd and the skew make the eight
-    // 16-byte words a phase-B warp load touches fall into eight different 16-byte bank groups)
-    static constexpr int CHUNK = 64, PITCH = 34, NSLOT = CHUNK + CHUNK / 8;
-    static constexpr int STG_W = PITCH * NSLOT;
+    // 16-byte words a phase-B warp load touches fall into eight different 16-byte bank groups), then the
+    // scratch record of the slow path.  CHUNK = 80: a row of 8 cells x 8 ppc (64 +- 8 particles) is ONE chunk.
+    static constexpr int CHUNK = CHUNK_, PITCH = 26, NSLOT = CHUNK + (CHUNK + 7) / 8, SLOW_W = 32;
+    static constexpr int STG_W = PITCH * NSLOT + SLOW_W;
+    static_assert(CHUNK % 8 == 0 && STG_W % 2 == 0, "staging layout");
     static constexpr int NOFF = NROW * (TX + 1);
     static constexpr size_t SMEM = sizeof(double) * ((size_t)TOT + (size_t)NW * STG_W) + sizeof(int) * (NOFF + 4);
     static_assert(TX == 8, "phase B maps 8 cells x 4 planes onto a warp");
@@ -232,12 +234,13 @@ __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
 
 namespace {
 
-constexpr int FLAG = 33;           // last double of every staging slot: record kind
+constexpr int FLAG = 25;           // last double of every staging slot: record kind
+constexpr int RCQ = 24;            // fast record: -q w / dt (shares a 16-byte word with the flag)
 constexpr double REC_FAST = 0.0;   // fast record (FastRec layout): old and new cell identical
 // 1 .. 6: fast record of a particle that crossed ONE cell face: 1 + 2 d + (1 if towards +d).  The part of
 // its Esirkepov window inside the cell's window is in the record; the one node layer outside it (S0 = 0,
 // DS = e there) is described by (e, prefix factor on the outer edge) in the chunk's extras area.
-constexpr double REC_SLOW = 8.0;   // slow record (SlowRec layout), deposited by the whole warp
+constexpr double REC_SLOW = 8.0;   // slow particle: the slot holds xi0 eta0 zeta0 xi1 eta1 zeta1 qw; deposited by the whole warp
 constexpr double REC_NONE = 7.0;   // nothing to deposit (q = 0, or the particle raised PIC_EPHYS)
 
 // extras of staging slot p (unskewed index): two doubles in the gap slot the skew leaves after every 8 slots
@@ -281,32 +284,33 @@ struct SlowRec {
     // per dimension d: s0 at 2 W d, ds at 2 W d + W;  then -q w / dt and the window's first padded offset
     static constexpr int S0X = 0, DSX = W, S0Y = 2 * W, DSY = 3 * W, S0Z = 4 * W, DSZ = 5 * W, CQ = 6 * W,
                          ORG = 6 * W + 1;
-    static_assert(ORG < FLAG, "slow record overlaps the flag");
+    static_assert(ORG < 32, "slow record larger than the scratch area");
 };
 
-// Written by the owning lane (all slow lanes of a chunk in parallel, each into its own slot).
+// The staging slot of a slow particle holds only (xi0, eta0, zeta0, xi1, eta1, zeta1, q w).  Lanes 0..2 expand
+// it, one dimension each, into the SlowRec of the warp's scratch area.  Called by all 32 lanes.
 template <int N>
-__device__ __forceinline__ void slow_write(double* rec, const Grid& g, double xi0, double et0, double ze0,
-                                           double xi1, double et1, double ze1, double qw, double inv_dt) {
+__device__ __forceinline__ void slow_build(const double* slot, double* rec, const Grid& g, double inv_dt, int lane) {
     using R = SlowRec<N>;
     constexpr int W = R::W;
     long long o = 0;
-#pragma unroll 1
-    for (int d = 0; d < 3; ++d) {
-        const double a0 = (d == 0) ? xi0 : ((d == 1) ? et0 : ze0);
-        const double a1 = (d == 0) ? xi1 : ((d == 1) ? et1 : ze1);
+    if (lane < 3) {
+        const int d = lane;
         const long long stride = (d == 0) ? 1 : ((d == 1) ? g.sy : g.sz);
         double s0[W], ds[W];
         bool bad = false;
-        const int n0 = shapes_pair<N>(a0, a1, s0, ds, bad);
+        const int n0 = shapes_pair<N>(slot[d], slot[3 + d], s0, ds, bad);
         double* r = rec + 2 * W * d;
 #pragma unroll
         for (int a = 0; a < W; ++a) { r[a] = s0[a]; r[W + a] = ds[a]; }
-        o += stride * (long long)(n0 + NG);     // window nodes stay inside the guard shell
+        o = stride * (long long)(n0 + NG);     // window nodes stay inside the guard shell
     }
-    rec[R::CQ] = -qw * inv_dt;
-    rec[R::ORG] = __longlong_as_double(o);
-    rec[FLAG] = REC_SLOW;
+    const long long o1 = __shfl_down_sync(0xffffffffu, o, 1), o2 = __shfl_down_sync(0xffffffffu, o, 2);
+    if (lane == 0) {
+        rec[R::CQ] = -slot[6] * inv_dt;
+        rec[R::ORG] = __longlong_as_double(o + o1 + o2);
+    }
+    __syncwarp();
 }
 
 // Called by all 32 lanes: lane <-> one (u,v) pair of the window's cross-section; W-1 points along the
@@ -346,15 +350,24 @@ __device__ __forceinline__ void slow_deposit(const double* rec, const Grid& g, c
 }
 
 // ---- fast path: per-(cell, plane) register accumulators --------------------------------------
-// Staging slot layout (FW = window nodes): s0x dsx s0y dsy s0z dsz (FW each), then pdx pdy pdz
-// (FW-1 each) with pd_d[a] = cq_d * sum_{a' <= a} ds_d[a'].  At FW = 4: 33 doubles + the flag.
+// Staging slot layout (FW = window nodes): s0x dsx s0y dsy s0z dsz (FW each), then at RCQ the factor
+// -q w / dt and at FLAG the record code.  The prefix-summed current factors
+// pd_d[a] = cq_d * sum_{a' <= a} ds_d[a'] are rebuilt by the phase-B lanes (18 fp64 operations) instead of
+// being staged (9 more doubles per particle through the shared-memory pipe, which is what binds the kernel).
 template <int N>
 struct FastRec {
     static constexpr int FW = FastWin<N>::FW;
-    static constexpr int S0X = 0, DSX = FW, S0Y = 2 * FW, DSY = 3 * FW, S0Z = 4 * FW, DSZ = 5 * FW, PDX = 6 * FW,
-                         PDY = 6 * FW + (FW - 1), PDZ = 6 * FW + 2 * (FW - 1), LEN = 6 * FW + 3 * (FW - 1);
-    static_assert(LEN <= FLAG, "fast record overlaps the flag");
+    static constexpr int S0X = 0, DSX = FW, S0Y = 2 * FW, DSY = 3 * FW, S0Z = 4 * FW, DSZ = 5 * FW, LEN = 6 * FW;
+    static_assert(LEN <= RCQ, "fast record overlaps its tail");
 };
+
+template <int K>
+__device__ __forceinline__ double pick(const double (&v)[K], int s) {
+    double r = v[0];
+#pragma unroll
+    for (int k = 1; k < K; ++k) r = (s == k) ? v[k] : r;
+    return r;
+}
 
 template <int N>
 struct CellAcc {
@@ -373,38 +386,45 @@ struct CellAcc {
     // ext = the slot's extras (e, outer prefix factor), read only for a face crosser; jx0, jy0, jz0 =
     // global J pointers at the first node of this cell's window (for the crosser's overflow layer).
     __device__ __forceinline__ bool add(const double* __restrict__ r, int s, const double* __restrict__ ext,
-                                        double* jx0, double* jy0, double* jz0, long long sy, long long sz) {
+                                        double* jx0, double* jy0, double* jz0, long long sy, long long sz,
+                                        double area_x, double area_y, double area_z) {
         using R = FastRec<N>;
         const double third = 1.0 / 3.0;
-        double s0x[FW], dsx[FW], s0y[FW], dsy[FW], pdx[FW - 1], pdy[FW - 1], pdz[FW - 1];
-        double code;
-        if constexpr (FW == 4) {
-            const double2 tail = ld2(r, 32);                  // pdz[2], flag
-            if (tail.y >= REC_NONE) return false;
-            code = tail.y;
+        const double2 tail = ld2(r, RCQ);                     // -q w / dt, code
+        if (tail.y >= REC_NONE) return false;
+        const double code = tail.y;
+        double s0x[FW], dsx[FW], s0y[FW], dsy[FW], dsz[FW], pdx[FW - 1], pdy[FW - 1], pdz[FW - 1];
+#pragma unroll
+        for (int a = 0; a < FW; a += 2) {
             double2 v;
-            v = ld2(r, R::S0X); s0x[0] = v.x; s0x[1] = v.y; v = ld2(r, R::S0X + 2); s0x[2] = v.x; s0x[3] = v.y;
-            v = ld2(r, R::DSX); dsx[0] = v.x; dsx[1] = v.y; v = ld2(r, R::DSX + 2); dsx[2] = v.x; dsx[3] = v.y;
-            v = ld2(r, R::S0Y); s0y[0] = v.x; s0y[1] = v.y; v = ld2(r, R::S0Y + 2); s0y[2] = v.x; s0y[3] = v.y;
-            v = ld2(r, R::DSY); dsy[0] = v.x; dsy[1] = v.y; v = ld2(r, R::DSY + 2); dsy[2] = v.x; dsy[3] = v.y;
-            v = ld2(r, 24); pdx[0] = v.x; pdx[1] = v.y;
-            v = ld2(r, 26); pdx[2] = v.x; pdy[0] = v.y;
-            v = ld2(r, 28); pdy[1] = v.x; pdy[2] = v.y;
-            v = ld2(r, 30); pdz[0] = v.x; pdz[1] = v.y;
-            pdz[2] = tail.x;
-        } else {
-            code = r[FLAG];
-            if (code >= REC_NONE) return false;
-#pragma unroll
-            for (int a = 0; a < FW; ++a) {
-                s0x[a] = r[R::S0X + a]; dsx[a] = r[R::DSX + a]; s0y[a] = r[R::S0Y + a]; dsy[a] = r[R::DSY + a];
-            }
-#pragma unroll
-            for (int a = 0; a < FW - 1; ++a) { pdx[a] = r[R::PDX + a]; pdy[a] = r[R::PDY + a]; pdz[a] = r[R::PDZ + a]; }
+            v = ld2(r, R::S0X + a); s0x[a] = v.x; s0x[a + 1] = v.y;
+            v = ld2(r, R::DSX + a); dsx[a] = v.x; dsx[a + 1] = v.y;
+            v = ld2(r, R::S0Y + a); s0y[a] = v.x; s0y[a + 1] = v.y;
+            v = ld2(r, R::DSY + a); dsy[a] = v.x; dsy[a + 1] = v.y;
+            v = ld2(r, R::DSZ + a); dsz[a] = v.x; dsz[a + 1] = v.y;
         }
-        const double s0z = r[R::S0Z + s], dsz = r[R::DSZ + s];
-        const double az = s0z + 0.5 * dsz, bz = 0.5 * s0z + third * dsz;
-        const double s0ys = r[R::S0Y + s], dsys = r[R::DSY + s];
+        const double s0z = r[R::S0Z + s];
+        // a face crosser's prefix starts with the weight that fell below the window in the crossed dimension
+        double e = 0.0, pd_ov = 0.0, e0x = 0.0, e0y = 0.0, e0z = 0.0;
+        if (code != REC_FAST) {
+            const double2 x = ld2(ext, 0);
+            e = x.x; pd_ov = x.y;
+            e0x = (code == 1.0) ? e : 0.0;
+            e0y = (code == 3.0) ? e : 0.0;
+            e0z = (code == 5.0) ? e : 0.0;
+        }
+        {
+            const double cqx = tail.x * area_x, cqy = tail.x * area_y, cqz = tail.x * area_z;
+            double rx = e0x, ry = e0y, rz = e0z;
+#pragma unroll
+            for (int a = 0; a < FW - 1; ++a) {
+                rx += dsx[a]; ry += dsy[a]; rz += dsz[a];
+                pdx[a] = cqx * rx; pdy[a] = cqy * ry; pdz[a] = cqz * rz;
+            }
+        }
+        const double dsz_s = pick<FW>(dsz, s);
+        const double az = s0z + 0.5 * dsz_s, bz = 0.5 * s0z + third * dsz_s;
+        const double s0ys = pick<FW>(s0y, s), dsys = pick<FW>(dsy, s);
         const double ay = s0ys + 0.5 * dsys, by = 0.5 * s0ys + third * dsys;
         double tx[FW], ty[FW], tz[FW];   // cross-section factors of Jx (per b), Jy (per a), Jz (per a)
 #pragma unroll
@@ -427,8 +447,6 @@ struct CellAcc {
         }
         if (code != REC_FAST) {
             // ---- face crosser: the node layer just outside the window (S0 = 0, DS = e) ----------------
-            const double2 x = ld2(ext, 0);
-            const double e = x.x, pd_ov = x.y;
             const int k = (int)code - 1, d = k >> 1, hi = k & 1;
             const long long node = hi ? FW : -1;          // node slot of the layer
             const long long edge = hi ? FW - 1 : -1;      // edge slot between the layer and the window
@@ -455,7 +473,7 @@ struct CellAcc {
                 for (int a = 0; a < FW - 1; ++a) red_add(px + a, pdx[a] * ebz);
                 if (s < FW - 1) {     // the layer's Jz row belongs to no lane: lane s takes plane c = s
                     double* pz = jz0 + sy * node + sz * s;
-                    const double pc = r[R::PDZ + s];
+                    const double pc = pick<FW - 1>(pdz, s);
 #pragma unroll
                     for (int a = 0; a < FW; ++a) red_add(pz + a, pc * (s0x[a] * he + dsx[a] * te));
                 }
@@ -469,7 +487,7 @@ struct CellAcc {
                 for (int a = 0; a < FW - 1; ++a) red_add(px + a, pdx[a] * t);
                 if (s < FW - 1) {
                     double* py = jy0 + sy * s + sz * node;
-                    const double pb = r[R::PDY + s];
+                    const double pb = pick<FW - 1>(pdy, s);
 #pragma unroll
                     for (int a = 0; a < FW; ++a) red_add(py + a, pb * (s0x[a] * he + dsx[a] * te));
                 }
@@ -599,6 +617,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
 
     const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
     const double inv_dt = 1.0 / g.dt;
+    const double area_x = g.inv_dy * g.inv_dz, area_y = g.inv_dx * g.inv_dz, area_z = g.inv_dx * g.inv_dy;
     double* stg = stg_all + warp * C::STG_W;
     const int bq = lane >> 2, bs = lane & 3;     // phase B role: cell of the row, plane of the window
     unsigned int n_fast = 0, n_slow = 0, n_glob = 0;
@@ -637,7 +656,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                 prefetch_particles(p, perm, ip + 64, row_hi, delta);   // rows longer than the two sub-chunks prefetched a row ahead
                 double* rec = stg + skew(sub + lane) * C::PITCH;
                 bool is_slow = false;
-                if (ip < row_hi) {
+                if (ip < row_hi && sub + lane < C::CHUNK) {
                     const int is = (perm != nullptr) ? (int)perm[ip] : ip;     // where this particle's data sits
                     const double x = p.x[is], y = p.y[is], z = p.z[is];
                     double ux = p.ux[is], uy = p.uy[is], uz = p.uz[is];
@@ -725,18 +744,17 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                                 fr[2 * FW * d + a] = s0[a];
                                 fr[2 * FW * d + FW + a] = dd;
                                 run += dd;
-                                if (a < FW - 1) fr[FR::PDX + (FW - 1) * d + a] = cq * run;
                             }
                             if (e_lo != 0.0) { code = 1.0 + 2.0 * d; ext_e = e_lo; ext_pd = pd_lo; }
                             if (e_hi != 0.0) { code = 2.0 + 2.0 * d; ext_e = e_hi; ext_pd = cq * run; }
                         }
-                        fr[FLAG] = code;
 #pragma unroll
-                        for (int k = 0; k < (FR::LEN + 1) / 2; ++k) st2(rec, 2 * k, fr[2 * k], fr[2 * k + 1]);
-                        if ((FR::LEN + 1) / 2 <= FLAG / 2) st2(rec, FLAG - 1, 0.0, code);
+                        for (int k = 0; k < FR::LEN / 2; ++k) st2(rec, 2 * k, fr[2 * k], fr[2 * k + 1]);
+                        st2(rec, RCQ, -qw * inv_dt, code);
                         if (code != REC_FAST) st2(stg, ext_word(sub + lane, C::PITCH), ext_e, ext_pd);
                     } else if (is_slow) {
-                        slow_write<N>(rec, g, xi, et, ze, xi1, et1, ze1, qw, inv_dt);
+                        st2(rec, 0, xi, et); st2(rec, 2, ze, xi1); st2(rec, 4, et1, ze1); st2(rec, 6, qw, 0.0);
+                        st2(rec, RCQ, 0.0, REC_SLOW);
                     } else {
                         rec[FLAG] = REC_NONE;
                     }
@@ -747,7 +765,10 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                 while (slow_mask) {
                     const int L = __ffs(slow_mask) - 1;
                     slow_mask &= slow_mask - 1;
-                    slow_deposit<N>(stg + skew(sub + L) * C::PITCH, g, f, lane);
+                    double* scr = stg + C::PITCH * C::NSLOT;
+                    slow_build<N>(stg + skew(sub + L) * C::PITCH, scr, g, inv_dt, lane);
+                    slow_deposit<N>(scr, g, f, lane);
+                    __syncwarp();
                 }
             }
             // ---------------- phase B: lane <-> (cell, plane) ------------------------------------
@@ -760,7 +781,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                     if (t < len) {
                         const int pslot = lo + t - base;
                         acc.add(stg + skew(pslot) * C::PITCH, bs, stg + ext_word(pslot, C::PITCH), f.Jx + win0,
-                                f.Jy + win0, f.Jz + win0, g.sy, g.sz);
+                                f.Jy + win0, f.Jz + win0, g.sy, g.sz, area_x, area_y, area_z);
                     }
             }
             __syncwarp();
@@ -783,8 +804,8 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
 // CfgDrift: a species that has moved since its last sort (particles up to one cell outside their listed
 // cell still gather from shared memory); one block of 8 warps per SM.
 // CfgFresh: right after pic_sort; two blocks of 4 warps per SM (2 x 112.6 KB of shared memory).
-using CfgDrift = TileCfg<8, 4, 4, 8, 1, 1>;
-using CfgFresh = TileCfg<8, 4, 4, 4, 2, 0>;
+using CfgDrift = TileCfg<8, 4, 4, 8, 1, 1, 80>;
+using CfgFresh = TileCfg<8, 4, 4, 4, 2, 0, 80>;
 static_assert(2 * (CfgFresh::SMEM + 64 + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
 
 template <int N, class Cfg>
