@@ -422,9 +422,9 @@ struct CellAcc {
                 pdx[a] = cqx * rx; pdy[a] = cqy * ry; pdz[a] = cqz * rz;
             }
         }
-        const double dsz_s = pick<FW>(dsz, s);
+        const double dsz_s = r[R::DSZ + s];
         const double az = s0z + 0.5 * dsz_s, bz = 0.5 * s0z + third * dsz_s;
-        const double s0ys = pick<FW>(s0y, s), dsys = pick<FW>(dsy, s);
+        const double s0ys = r[R::S0Y + s], dsys = r[R::DSY + s];
         const double ay = s0ys + 0.5 * dsys, by = 0.5 * s0ys + third * dsys;
         double tx[FW], ty[FW], tz[FW];   // cross-section factors of Jx (per b), Jy (per a), Jz (per a)
 #pragma unroll
