@@ -229,7 +229,7 @@ __device__ __forceinline__ void boris_push_rsqrt(double h, double inv_c2, double
     const double hg = h * rsqrt(1.0 + (umx * umx + umy * umy + umz * umz) * inv_c2);
     const double tx = hg * bx, ty = hg * by, tz = hg * bz;
     const double t2 = tx * tx + ty * ty + tz * tz;
-    const double f = 2.0 / (1.0 + t2);
+    const double f = 2.0 * __drcp_rn(1.0 + t2);      // = RN(2 / (1 + t2)): the scaling by 2 is exact
     const double sx = f * tx, sy = f * ty, sz = f * tz;
     const double upx = umx + (umy * tz - umz * ty);
     const double upy = umy + (umz * tx - umx * tz);
@@ -727,10 +727,9 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                     po.uy[ip] = uy;
                     po.uz[ip] = uz;
                     // ---- classify: fast = stayed inside the cell the sort listed it in -------------
-                    int lc = 0;
-#pragma unroll
-                    for (int c = 1; c < C::TX; ++c) lc += (off[c] <= ip) ? 1 : 0;
-                    const bool listed = in_tile && rx == lc && ry == ry0 && rz == rz0;
+                    const int rxc = min(max(rx, 0), C::TX - 1);
+                    const bool listed = in_tile && rx == rxc && off[rxc] <= ip && ip < off[rxc + 1] && ry == ry0 &&
+                                        rz == rz0;      // ip lies in the sorted range of the cell the particle is in
                     const bool deposits = !bad && qw != 0.0;
                     const int ncross = (__double2int_rd(xi1) != ci) + (__double2int_rd(et1) != cj) +
                                        (__double2int_rd(ze1) != ck);
