@@ -131,11 +131,12 @@ template <int N>
 __device__ __forceinline__ void place_new_window(const double (&w)[N + 1], int sh, double (&out)[FastWin<N>::FW],
                                                  double& e_lo, double& e_hi) {
     constexpr int FW = FastWin<N>::FW;
+    constexpr int TMAX = (N == 2) ? 2 : 1;    // orders 1 and 3 anchor their support at floor(xi): sh = -1, 0 or 1
 #pragma unroll
     for (int a = 0; a < FW; ++a) {
         double v = 0.0;
 #pragma unroll
-        for (int t = -1; t <= 2; ++t) {
+        for (int t = -1; t <= TMAX; ++t) {
             const int k = a - t;                      // weight index that lands on slot a when sh == t
             if (k >= 0 && k <= N) v = (sh == t) ? w[k] : v;
         }
@@ -144,7 +145,7 @@ __device__ __forceinline__ void place_new_window(const double (&w)[N + 1], int s
     e_lo = (sh == -1) ? w[0] : 0.0;
     e_hi = 0.0;
 #pragma unroll
-    for (int t = 0; t <= 2; ++t) {
+    for (int t = 0; t <= TMAX; ++t) {
         const int k = FW - t;
         if (k >= 0 && k <= N) e_hi = (sh == t) ? w[k] : e_hi;
     }
