@@ -56,13 +56,13 @@ YEE_BYTES_PER_CELL = 240.0
 # fp64-pipe roofline of the fused kernel.  Instructions per particle = DFMA + DMUL + DADD
 # thread instructions executed per particle by the committed kernel (ncu, profiles/); order 3 measured,
 # orders 1 and 2 scaled by the gather/deposit operation counts.
-FP64_INSTR_PER_PARTICLE = {1: 420.0, 2: 800.0, 3: 1170.0}
+FP64_INSTR_PER_PARTICLE = {1: 410.0, 2: 780.0, 3: 1129.0}
 FP64_LANES_PER_SM = 64
 N_SM = 148
 SM_MAX_MHZ = 1965.0
-# shared-memory bytes the kernel moves per particle: order 3 = 39.1 wavefronts x 128 B (ncu, profiles/r01_v5);
+# shared-memory bytes the kernel moves per particle: order 3 = 39.0 wavefronts x 128 B (ncu, profiles/r01_v5, section v6);
 # orders 1 and 2 scaled by the gather/deposit operand counts
-SMEM_BYTES_PER_PARTICLE = {1: 1050.0, 2: 2550.0, 3: 5010.0}
+SMEM_BYTES_PER_PARTICLE = {1: 1050.0, 2: 2550.0, 3: 4990.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch at the default workload (profiles/)
 TRAFFIC_BYTES_PER_LAUNCH = 22.15e9
 
