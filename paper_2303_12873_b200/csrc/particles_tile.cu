@@ -1,31 +1,35 @@
 // particles_tile.cu -- fused gather + Boris push + Esirkepov deposition per
 // cell-sorted tile (BASELINE.json:north_star parts
-// 1-3, "fused per cell-sorted tile").  Kernel v2.
+// 1-3, "fused per cell-sorted tile").  Kernel v5/v6 of DESIGN.md section 5.1;
+// measurements in profiles/r01_v4_tile_kernel.md and r01_v5_tile_kernel.md.
 //
 // One thread block owns a tile of TX x TY x TZ cells; its E,B stencil (+ halo
 // for the shape support and DRIFT cells of drift since the last pic_sort) is
 // staged in shared memory once.  After that the block's warps run without any
 // block-wide barrier: a warp pulls x-rows of the tile (TX cells, contiguous in
 // the cell-sorted SoA arrays) from a shared counter and processes each row in
-// chunks of 32 consecutive particles:
-//   phase A  lane <-> particle (coalesced loads/stores).  Gather from the
-//            shared stencil (the 32 lanes sit in ~4 cells: broadcast LDS),
-//            Boris, move, store of the wrapped state.  A particle that stayed
-//            inside its listed cell ("fast") writes its old/new nodal shapes
-//            and the three prefix-summed current factors to a per-warp staging
-//            slot.
+// chunks of CHUNK = 80 particles (a row of 8 cells x 8 ppc is one chunk):
+//   phase A  lane <-> particle, 32 at a time (coalesced loads/stores; with a
+//            deferred sort pending the loads go through perm[] and all eight
+//            arrays are written, in sorted order, to the other buffer).
+//            Gather from the shared stencil, Boris, move, store of the wrapped
+//            state.  A particle that stayed inside its listed cell or crossed
+//            ONE of its faces ("fast") writes its old nodal shapes and shape
+//            differences on the cell's window plus q w / dt to a per-warp
+//            staging slot (26 doubles).
 //   phase B  lane <-> (cell q of the row, plane s of that cell's window).  The
 //            four lanes of a cell walk the cell's staged particles and
 //            accumulate the Esirkepov window of the CELL in registers
 //            (3 x 12 accumulators per lane at order 3), so the per-particle
-//            cost is FMAs and broadcast LDS, not atomics.
-//   slow     a particle that crossed a cell face or is not in its listed cell
-//            is deposited by the whole warp: its (N+2)^3 window is spread over
-//            the lanes, one global RED.ADD.F64 per non-zero point.
-//   flush    at the end of a row every lane adds its accumulators to the
-//            padded global J arrays with RED.ADD.F64 (fire-and-forget; fp64
-//            atomicAdd on SHARED memory is a CAS loop on sm_100a, which is why
-//            there is no shared J tile).
+//            cost is FMAs and shared-memory loads, not atomics.
+//   slow     a particle that crossed several faces or is not in its listed
+//            cell stages its positions and is deposited by the whole warp: its
+//            (N+2)^3 window is spread over the lanes, one global RED.ADD.F64
+//            per non-zero point.
+//   flush    at the end of a row the lanes add up, with shuffles, what lands on
+//            the same global node and issue one RED.ADD.F64 per distinct node
+//            (fire-and-forget; fp64 atomicAdd on SHARED memory is a CAS loop on
+//            sm_100a, which is why there is no shared J tile).
 // A particle outside the tile's halo gathers from global memory instead; the
 // kernel is correct for any particle order, only slower (R39).
 #include "particle_update.cuh"
