@@ -8,10 +8,12 @@
 // staged in shared memory once.  After that the block's warps run without any
 // block-wide barrier: a warp pulls x-rows of the tile (TX cells, contiguous in
 // the cell-sorted SoA arrays) from a shared counter and processes each row in
-// chunks of CHUNK = 80 particles (a row of 8 cells x 8 ppc is one chunk):
-//   phase A  lane <-> particle, 32 at a time (coalesced loads/stores; with a
-//            deferred sort pending the loads go through perm[] and all eight
-//            arrays are written, in sorted order, to the other buffer).
+// chunks of CHUNK = 72 particles (a row of 8 cells x 8 ppc is mostly one chunk):
+//   phase A  lane <-> particle, 32 at a time.  The particle data of a sub-chunk
+//            are copied into a per-warp landing buffer by cp.async one
+//            sub-chunk ahead (with a deferred sort pending: through perm[],
+//            and all eight arrays are then written, in sorted order, to the
+//            other buffer).
 //            Gather from the shared stencil, Boris, move, store of the wrapped
 //            state.  A particle that stayed inside its listed cell or crossed
 //            ONE of its faces ("fast") writes its old nodal shapes and shape
@@ -74,9 +76,10 @@ struct TileCfg {
     }
     // per-warp staging: CHUNK skewed slots of PITCH doubles (PITCH/2 odd and the skew make the eight
     // 16-byte words a phase-B warp load touches fall into eight different 16-byte bank groups), then the
-    // scratch record of the slow path.  CHUNK = 80: a row of 8 cells x 8 ppc (64 +- 8 particles) is ONE chunk.
-    static constexpr int CHUNK = CHUNK_, PITCH = 26, NSLOT = CHUNK + (CHUNK + 7) / 8, SLOW_W = 32;
-    static constexpr int STG_W = PITCH * NSLOT + SLOW_W;
+    // scratch record of the slow path and the landing buffer of the next sub-chunk's particle data (8 arrays x
+    // 32 lanes, filled by cp.async).  CHUNK = 72: a row of 8 cells x 8 ppc (64 +- 8 particles) is mostly ONE chunk.
+    static constexpr int CHUNK = CHUNK_, PITCH = 26, NSLOT = CHUNK + (CHUNK + 7) / 8, SLOW_W = 32, PBUF_W = 8 * 32;
+    static constexpr int STG_W = PITCH * NSLOT + SLOW_W + PBUF_W;
     static_assert(CHUNK % 8 == 0 && STG_W % 2 == 0, "staging layout");
     static constexpr int NOFF = NROW * (TX + 1);
     static constexpr size_t SMEM = sizeof(double) * ((size_t)TOT + (size_t)NW * STG_W) + sizeof(int) * (NOFF + 4);
@@ -276,24 +279,24 @@ __device__ __forceinline__ void red_add(double* p, double v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // pull one 32-particle sub-chunk of the SoA arrays towards the SM ahead of its use
-// (delta = where the sorted position's data sits in the source buffer relative to the position itself:
-// 0 in place, else the shift of the row's first particle under the deferred-sort permutation)
-__device__ __forceinline__ void prefetch_particles(const Particles& p, const unsigned int* perm, int ip, int hi,
-                                                   int delta) {
-    if (ip < hi) {
-        if (perm != nullptr) {
-            prefetch_l1(perm + ip);
-            prefetch_l1(p.id + ip + delta);
-        }
-        ip += delta;
-        prefetch_l1(p.x + ip); prefetch_l1(p.y + ip); prefetch_l1(p.z + ip);
-        prefetch_l1(p.ux + ip); prefetch_l1(p.uy + ip); prefetch_l1(p.uz + ip);
-        prefetch_l1(p.w + ip);
-    }
+// A load the compiler must issue HERE (it otherwise sinks the load next to its first use, which is the point
+// where the latency was meant to be over).
+__device__ __forceinline__ int ld_u32_now(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return (int)v;
 }
+
+// 8-byte asynchronous copy global -> shared (LDGSTS): the data land in shared memory without a register
+// and without a scoreboard wait in the issuing warp
+__device__ __forceinline__ void cp_async8(double* dst_smem, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 __device__ __forceinline__ double2 ld2(const double* r, int i) { return *reinterpret_cast<const double2*>(r + i); }
 __device__ __forceinline__ void st2(double* r, int i, double a, double b) {
@@ -577,7 +580,6 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
     double* stg_all = Et + C::TOT;                               // NW * STG_W
     int* row_off = reinterpret_cast<int*>(stg_all + C::NW * C::STG_W);   // NROW x (TX+1) container indices
     int* next_row = row_off + C::NOFF;
-    __shared__ int row_delta[C::NROW];     // deferred sort: perm[first particle of the row] - its sorted position
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     int b = blockIdx.x;
@@ -596,12 +598,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
         row_off[e] = v;
     }
     if (tid == 0) *next_row = 0;
-    if (tid < C::NROW) row_delta[tid] = 0;
     __syncthreads();
-    if (perm != nullptr && tid < C::NROW) {
-        const int lo = row_off[tid * (C::TX + 1)], hi = row_off[tid * (C::TX + 1) + C::TX];
-        if (lo < hi) row_delta[tid] = (int)perm[lo] - lo;     // read by the row's warp long after the stencil barrier
-    }
     int n_tile = 0;
 #pragma unroll 4
     for (int r = 0; r < C::NROW; ++r) n_tile += row_off[r * (C::TX + 1) + C::TX] - row_off[r * (C::TX + 1)];
@@ -645,6 +642,8 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
     const int bq = lane >> 2, bs = lane & 3;     // phase B role: cell of the row, plane of the window
     unsigned int n_fast = 0, n_slow = 0, n_glob = 0;
     bool bad_any = false;
+    double* pbuf = stg + C::PITCH * C::NSLOT + C::SLOW_W;     // landing buffer: [x y z ux uy uz w id][lane]
+    int buf_start = -1;                                        // sorted index of lane 0's particle in it
 
     int row_ahead = 0;
     if (lane == 0) row_ahead = atomicAdd(next_row, 1);
@@ -654,17 +653,15 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
         if (row >= C::NROW) break;
         if (lane == 0) row_ahead = atomicAdd(next_row, 1);     // the row after this one: prefetch its head
         row_ahead = __shfl_sync(0xffffffffu, row_ahead, 0);
+        int nrow_lo = 0, nrow_hi = 0;      // sorted range of the row fetched ahead
         if (row_ahead < C::NROW) {
-            const int* offn = row_off + row_ahead * (C::TX + 1);
-            const int dl = row_delta[row_ahead];
-            prefetch_particles(p, perm, offn[0] + lane, offn[C::TX], dl);
-            prefetch_particles(p, perm, offn[0] + 32 + lane, offn[C::TX], dl);
+            nrow_lo = row_off[row_ahead * (C::TX + 1)];
+            nrow_hi = row_off[row_ahead * (C::TX + 1) + C::TX];
         }
         const int* off = row_off + row * (C::TX + 1);
         const int row_lo = off[0], row_hi = off[C::TX];
         if (row_lo >= row_hi) continue;
         const int ry0 = row % C::TY, rz0 = row / C::TY;     // the row's tile-relative (y, z) cell
-        const int delta = row_delta[row];
         const int cell_lo = off[bq], cell_hi = off[bq + 1];  // phase B: this lane's cell
         CellAcc<N> acc;
         acc.clear();
@@ -676,18 +673,38 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
             for (int sub = 0; sub < C::CHUNK; sub += 32) {
                 const int ip = base + sub + lane;
                 if (base + sub >= row_hi) break;
-                prefetch_particles(p, perm, ip + 64, row_hi, delta);   // rows longer than the two sub-chunks prefetched a row ahead
+                // ---- particle data of this sub-chunk: copied to the warp's landing buffer one sub-chunk ago ----
+                if (buf_start != base + sub) {      // cold start, or the row fetched ahead was empty: fetch now
+                    if (ip < row_hi) {
+                        const int is = (perm != nullptr) ? (int)perm[ip] : ip;
+                        cp_async8(pbuf + 0 * 32 + lane, p.x + is); cp_async8(pbuf + 1 * 32 + lane, p.y + is);
+                        cp_async8(pbuf + 2 * 32 + lane, p.z + is); cp_async8(pbuf + 3 * 32 + lane, p.ux + is);
+                        cp_async8(pbuf + 4 * 32 + lane, p.uy + is); cp_async8(pbuf + 5 * 32 + lane, p.uz + is);
+                        cp_async8(pbuf + 6 * 32 + lane, p.w + is);
+                        if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + is);
+                    }
+                    cp_async_commit();
+                }
+                cp_async_wait_all();
+                __syncwarp();
+                const double x = pbuf[0 * 32 + lane], y = pbuf[1 * 32 + lane], z = pbuf[2 * 32 + lane];
+                double ux = pbuf[3 * 32 + lane], uy = pbuf[4 * 32 + lane], uz = pbuf[5 * 32 + lane];
+                const double wgt = pbuf[6 * 32 + lane], idv = pbuf[7 * 32 + lane];
+                __syncwarp();       // every lane has read: the buffer may be refilled
+                // source index of this lane's particle of the NEXT sub-chunk this warp will walk: rest of the
+                // row, else head of the row fetched ahead (deferred sort: through perm[]; the load is consumed
+                // after the gather, which hides its latency)
+                int nstart = (sub + 32 < C::CHUNK) ? base + sub + 32 : base + C::CHUNK, nhi = row_hi;
+                if (nstart >= row_hi) { nstart = nrow_lo; nhi = nrow_hi; }
+                int isn = -1;
+                if (nstart + lane < nhi) isn = (perm != nullptr) ? ld_u32_now(perm + nstart + lane) : nstart + lane;
                 double* rec = stg + skew(sub + lane) * C::PITCH;
                 bool is_slow = false;
                 if (ip < row_hi && sub + lane < C::CHUNK) {
-                    const int is = (perm != nullptr) ? (int)perm[ip] : ip;     // where this particle's data sits
-                    const double x = p.x[is], y = p.y[is], z = p.z[is];
-                    double ux = p.ux[is], uy = p.uy[is], uz = p.uz[is];
-                    const double wgt = p.w[is];
                     const double qw = q * wgt;
                     if (perm != nullptr) {          // deferred sort: the other buffer gets every array, in sorted order
                         po.w[ip] = wgt;
-                        po.id[ip] = p.id[is];
+                        po.id[ip] = (unsigned long long)__double_as_longlong(idv);
                     }
                     const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy,
                                  ze = (z - g.zmin) * g.inv_dz;
@@ -783,6 +800,16 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                         rec[FLAG] = REC_NONE;
                     }
                 }
+                // ---- next sub-chunk's particle data -> landing buffer (in flight during phase B / the next row fetch)
+                if (isn >= 0) {
+                    cp_async8(pbuf + 0 * 32 + lane, p.x + isn); cp_async8(pbuf + 1 * 32 + lane, p.y + isn);
+                    cp_async8(pbuf + 2 * 32 + lane, p.z + isn); cp_async8(pbuf + 3 * 32 + lane, p.ux + isn);
+                    cp_async8(pbuf + 4 * 32 + lane, p.uy + isn); cp_async8(pbuf + 5 * 32 + lane, p.uz + isn);
+                    cp_async8(pbuf + 6 * 32 + lane, p.w + isn);
+                    if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + isn);
+                }
+                cp_async_commit();
+                buf_start = (nstart < nhi) ? nstart : -1;
                 __syncwarp();
                 // ---------------- slow path: one particle at a time, whole warp ---------------------
                 unsigned int slow_mask = __ballot_sync(0xffffffffu, is_slow);
@@ -828,9 +855,9 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
 // CfgDrift: a species that has moved since its last sort (particles up to one cell outside their listed
 // cell still gather from shared memory); one block of 8 warps per SM.
 // CfgFresh: right after pic_sort; two blocks of 4 warps per SM (2 x 112.6 KB of shared memory).
-using CfgDrift = TileCfg<8, 4, 4, 8, 1, 1, 80>;
-using CfgFresh = TileCfg<8, 4, 4, 4, 2, 0, 80>;
-static_assert(2 * (CfgFresh::SMEM + 64 + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
+using CfgDrift = TileCfg<8, 4, 4, 8, 1, 1, 72>;
+using CfgFresh = TileCfg<8, 4, 4, 4, 2, 0, 72>;
+static_assert(2 * (CfgFresh::SMEM + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
 
 template <int N, class Cfg>
 void launch_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po, const unsigned int* perm,
