@@ -644,6 +644,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
     bool bad_any = false;
     double* pbuf = stg + C::PITCH * C::NSLOT + C::SLOW_W;     // landing buffer: [x y z ux uy uz w id][lane]
     int buf_start = -1;                                        // sorted index of lane 0's particle in it
+    int isn_reg = 0, isn_tag = -2;                             // perm[] entry read two sub-chunks ahead, and for which start
 
     int row_ahead = 0;
     if (lane == 0) row_ahead = atomicAdd(next_row, 1);
@@ -691,13 +692,39 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                 double ux = pbuf[3 * 32 + lane], uy = pbuf[4 * 32 + lane], uz = pbuf[5 * 32 + lane];
                 const double wgt = pbuf[6 * 32 + lane], idv = pbuf[7 * 32 + lane];
                 __syncwarp();       // every lane has read: the buffer may be refilled
-                // source index of this lane's particle of the NEXT sub-chunk this warp will walk: rest of the
-                // row, else head of the row fetched ahead (deferred sort: through perm[]; the load is consumed
-                // after the gather, which hides its latency)
-                int nstart = (sub + 32 < C::CHUNK) ? base + sub + 32 : base + C::CHUNK, nhi = row_hi;
-                if (nstart >= row_hi) { nstart = nrow_lo; nhi = nrow_hi; }
-                int isn = -1;
-                if (nstart + lane < nhi) isn = (perm != nullptr) ? ld_u32_now(perm + nstart + lane) : nstart + lane;
+                // ---- next sub-chunk this warp will walk (rest of the row, else head of the row fetched ahead):
+                // its particle data start their way to the landing buffer NOW, so that they have this whole
+                // sub-chunk to arrive.  Deferred sort: their places come from perm[], read ONE MORE sub-chunk
+                // ahead into a register (isn_reg, valid for the sub-chunk that starts at isn_tag).
+                {
+                    int base1 = base, sub1 = sub + 32, hi1 = row_hi;
+                    bool in_next = false;
+                    if (!(sub1 < C::CHUNK && base1 + sub1 < row_hi)) {
+                        base1 = base + C::CHUNK; sub1 = 0;
+                        if (base1 >= row_hi) { base1 = nrow_lo; hi1 = nrow_hi; in_next = true; }
+                    }
+                    const int nstart = base1 + sub1;
+                    if (nstart + lane < hi1) {
+                        int isn = nstart + lane;
+                        if (perm != nullptr) isn = (isn_tag == nstart) ? isn_reg : (int)perm[nstart + lane];
+                        cp_async8(pbuf + 0 * 32 + lane, p.x + isn); cp_async8(pbuf + 1 * 32 + lane, p.y + isn);
+                        cp_async8(pbuf + 2 * 32 + lane, p.z + isn); cp_async8(pbuf + 3 * 32 + lane, p.ux + isn);
+                        cp_async8(pbuf + 4 * 32 + lane, p.uy + isn); cp_async8(pbuf + 5 * 32 + lane, p.uz + isn);
+                        cp_async8(pbuf + 6 * 32 + lane, p.w + isn);
+                        if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + isn);
+                    }
+                    cp_async_commit();
+                    buf_start = (nstart < hi1) ? nstart : -1;
+                    if (perm != nullptr) {      // the sub-chunk after that one
+                        int start2 = base1 + sub1 + 32, hi2 = hi1;
+                        if (!(sub1 + 32 < C::CHUNK && start2 < hi1)) {
+                            start2 = base1 + C::CHUNK;
+                            if (start2 >= hi1) { start2 = in_next ? -2 : nrow_lo; hi2 = in_next ? -2 : nrow_hi; }
+                        }
+                        isn_tag = start2;
+                        isn_reg = (start2 >= 0 && start2 + lane < hi2) ? ld_u32_now(perm + start2 + lane) : 0;
+                    }
+                }
                 double* rec = stg + skew(sub + lane) * C::PITCH;
                 bool is_slow = false;
                 if (ip < row_hi && sub + lane < C::CHUNK) {
@@ -800,16 +827,6 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                         rec[FLAG] = REC_NONE;
                     }
                 }
-                // ---- next sub-chunk's particle data -> landing buffer (in flight during phase B / the next row fetch)
-                if (isn >= 0) {
-                    cp_async8(pbuf + 0 * 32 + lane, p.x + isn); cp_async8(pbuf + 1 * 32 + lane, p.y + isn);
-                    cp_async8(pbuf + 2 * 32 + lane, p.z + isn); cp_async8(pbuf + 3 * 32 + lane, p.ux + isn);
-                    cp_async8(pbuf + 4 * 32 + lane, p.uy + isn); cp_async8(pbuf + 5 * 32 + lane, p.uz + isn);
-                    cp_async8(pbuf + 6 * 32 + lane, p.w + isn);
-                    if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + isn);
-                }
-                cp_async_commit();
-                buf_start = (nstart < nhi) ? nstart : -1;
                 __syncwarp();
                 // ---------------- slow path: one particle at a time, whole warp ---------------------
                 unsigned int slow_mask = __ballot_sync(0xffffffffu, is_slow);
