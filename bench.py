@@ -60,11 +60,11 @@ FP64_INSTR_PER_PARTICLE = {1: 410.0, 2: 780.0, 3: 1129.0}
 FP64_LANES_PER_SM = 64
 N_SM = 148
 SM_MAX_MHZ = 1965.0
-# shared-memory bytes the kernel moves per particle: order 3 = 39.0 wavefronts x 128 B (ncu, profiles/r01_v5, section v6);
+# shared-memory bytes the kernel moves per particle: order 3 = 41.3 wavefronts x 128 B (ncu, profiles/r01_v5, section v7);
 # orders 1 and 2 scaled by the gather/deposit operand counts
-SMEM_BYTES_PER_PARTICLE = {1: 1050.0, 2: 2550.0, 3: 4990.0}
+SMEM_BYTES_PER_PARTICLE = {1: 1350.0, 2: 2850.0, 3: 5290.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch at the default workload (profiles/)
-TRAFFIC_BYTES_PER_LAUNCH = 22.15e9
+TRAFFIC_BYTES_PER_LAUNCH = 22.09e9
 
 
 def _peaks():
