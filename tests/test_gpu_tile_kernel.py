@@ -181,3 +181,39 @@ def test_fresh_and_drift_variants_of_the_tile_kernel(ora, Sim, order, fresh):
     o.step(1)
     g.step(1)
     check_step_parity(o, g, wl, "fresh=%d order %d step 2" % (fresh, order))
+
+
+def test_full_size_config1_drift_step_continuity_and_gauss(ora, Sim):
+    """BASELINE.json configs[1] at full size (128^3 cells, 16.8 M electrons + 16.8 M protons, order 3, sort every
+    4 steps): properties that hold at any size, on the launch sequence bench.py --config 1 times.  Step 1 runs
+    the fresh-sort variant through the deferred permutation, steps 2-4 the drift-tolerant variant in place.
+    (a) discrete continuity of the total current on the whole grid for step 4 (R20), (b) Gauss's law residual
+    div E - rho/eps0 unchanged from t = 0 (R19; it is zero here: electrons and protons start co-located),
+    (c) every particle took the fused kernel, and only drifted / multi-face crossers its slow path."""
+    import torch
+    eps0 = 8.8541878128e-12
+    wl = W.config(1)
+    n = wl.nx
+    g = Sim.from_workload(wl)
+    g.sort()
+    g.step(3)
+    rho3 = g.deposit_rho(-1, device=True)
+    g.step(1)
+    rho4 = g.deposit_rho(-1, device=True)
+    F = g.get_fields(names=("Ex", "Ey", "Ez", "Jx", "Jy", "Jz"), device=True)
+
+    def div_back(a, b, c):
+        a, b, c = (t.view(n, n, n) for t in (a, b, c))
+        return ((a - torch.roll(a, 1, 2)) / wl.dx + (b - torch.roll(b, 1, 1)) / wl.dy + (c - torch.roll(c, 1, 0)) / wl.dz)
+
+    # scale of one species' charge density (the total cancels to roundoff at t = 0)
+    sp = wl.species[0]
+    rho_scale = abs(sp.q) * float(sp.w[0]) * 8 / (wl.dx * wl.dy * wl.dz)
+    res = div_back(F["Jx"], F["Jy"], F["Jz"]) + (rho4 - rho3).view(n, n, n) / wl.dt
+    assert float(res.abs().max()) <= 1e-12 * rho_scale / wl.dt, float(res.abs().max())
+    gauss = div_back(F["Ex"], F["Ey"], F["Ez"]) - rho4.view(n, n, n) / eps0
+    assert float(gauss.abs().max()) <= 1e-10 * rho_scale / eps0, float(gauss.abs().max())
+    c = g.counters()
+    N = wl.nparticles
+    assert c["global"] == 0 and c["fast"] + c["slow"] == 4 * N and c["slow"] < 0.05 * 4 * N
+    assert c["sorts"] == 1 and c["steps"] == 4
