@@ -217,3 +217,44 @@ def test_full_size_config1_drift_step_continuity_and_gauss(ora, Sim):
     N = wl.nparticles
     assert c["global"] == 0 and c["fast"] + c["slow"] == 4 * N and c["slow"] < 0.05 * 4 * N
     assert c["sorts"] == 1 and c["steps"] == 4
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_laser_configs_continuity_and_gauss(ora, Sim, cfg):
+    """BASELINE.json configs[3] (laser-wakefield box, 128 x 128 x 1024, 13 M electrons behind a density ramp)
+    and configs[4] (plasma mirror, 256 x 256 x 512, 101 M electrons at 16 ppc + 25 M protons at 4 ppc in a slab:
+    empty tiles next to rows several chunks long) at full size, laser pulse in E and B: sort, two steps (the
+    fresh-sort variant, then the drift variant), and the properties that hold at any size: continuity of the
+    total current for step 2 on the whole grid (R20) and a Gauss residual div E - rho/eps0 that stays what it
+    was at t = 0 (R19)."""
+    import torch
+    eps0 = 8.8541878128e-12
+    wl = W.config(cfg)
+    nx, ny, nz = wl.nx, wl.ny, wl.nz
+    g = Sim.from_workload(wl)
+
+    def div_back(a, b, c):
+        a, b, c = (t.view(nz, ny, nx) for t in (a, b, c))
+        return ((a - torch.roll(a, 1, 2)) / wl.dx + (b - torch.roll(b, 1, 1)) / wl.dy + (c - torch.roll(c, 1, 0)) / wl.dz)
+
+    def gauss_residual():
+        F = g.get_fields(names=("Ex", "Ey", "Ez"), device=True)
+        return div_back(F["Ex"], F["Ey"], F["Ez"]) - g.deposit_rho(-1, device=True).view(nz, ny, nx) / eps0
+
+    g0 = gauss_residual()
+    g.sort()
+    g.step(1)
+    rho1 = g.deposit_rho(-1, device=True)
+    g.step(1)
+    rho2 = g.deposit_rho(-1, device=True)
+    J = g.get_fields(names=("Jx", "Jy", "Jz"), device=True)
+    rho_scale = float(rho1.abs().max())
+    assert rho_scale > 0
+    res = div_back(J["Jx"], J["Jy"], J["Jz"]) + (rho2 - rho1).view(nz, ny, nx) / wl.dt
+    assert float(res.abs().max()) <= 1e-12 * rho_scale / wl.dt, float(res.abs().max())
+    del res, J, rho1
+    drift = gauss_residual() - g0
+    assert float(drift.abs().max()) <= 1e-10 * rho_scale / eps0, float(drift.abs().max())
+    c = g.counters()
+    N = wl.nparticles
+    assert c["global"] == 0 and c["fast"] + c["slow"] == 2 * N
