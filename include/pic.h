@@ -139,9 +139,15 @@ int pic_step(pic_ctx*, int nsteps);
 /*
  * Counting sort of every loaded species by cell key = i + nx*(j + ny*k),
  * (i,j,k) = clamp(floor((x - xmin)/dx), 0, nx-1) etc. of the stored position:
- * histogram, exclusive scan, scatter of x,y,z,ux,uy,uz,w,id into the second
- * SoA buffer, buffer swap.  Afterwards keys are non-decreasing in container
- * order; the order inside one cell is unspecified (R24).  Asynchronous.
+ * histogram, exclusive scan, and the move of x,y,z,ux,uy,uz,w,id into the
+ * second SoA buffer with a buffer swap.  Afterwards keys are non-decreasing in
+ * container order (as seen by pic_get_particles / pic_get_cell_offsets); the
+ * order inside one cell is unspecified (R24).  By default (option
+ * "sort_deferred") only the permutation is computed here and the move is
+ * carried out by the next reader of the container -- normally the fused
+ * per-tile kernel of the next pic_step, which reads its inputs through the
+ * permutation at no extra pass over the data; the observable result is the
+ * same.  Asynchronous.
  */
 int pic_sort(pic_ctx*);
 
