@@ -283,6 +283,9 @@ def run_ours(args):
                 "peak_kind": "derived: 148 SMs x 64 fp64 lanes/clk x 1965 MHz (DESIGN.md 5.1; DFMA probe)",
                 "unit": "T fp64-instr/s", "frac": fp64_ach / fp64_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH
                 if (args.config == 2 and args.n is None) else None,
+                "traffic_note": "ncu dram bytes of one launch that also carries out the deferred sort: 15.57 GB "
+                                "algorithmic (104 B/particle + 96 B/cell) + 3.76 GB of the sort row (perm, w, id: "
+                                "28 B/particle) + 2.8 GB of halo and partial-sector overhead (profiles/r01_v5)",
                 "ms_per_launch": ms_launch, "algorithmic_fp64_instr_per_launch": fp64_alg,
                 "particle_updates_per_s_kernel_only": np_launch / (ms_launch * 1e-3)}
     hbm_ach = alg_bytes / (ms_launch * 1e-3) / 1e9
