@@ -85,6 +85,33 @@ __global__ void fold_guards_kernel(Grid g, double* F) {
 // NOTE: the fold reads guard images while other threads overwrite interior
 // cells; an interior cell is an image only of itself (|a| = 0), and it is read
 // by its own thread only, so there is no race.
+// the three J components in one launch (one thread per interior cell; only the edge cells do work)
+__global__ void fold_guards3_kernel(Grid g, double* F0, double* F1, double* F2) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int j = blockIdx.y, k = blockIdx.z;
+    if (i >= g.nx) return;
+    const bool edge = i < NG || i >= g.nx - NG || j < NG || j >= g.ny - NG || k < NG || k >= g.nz - NG;
+    if (!edge) return;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int kk = first_image(k, g.nz); kk < g.nz + NG; kk += g.nz)
+        for (int jj = first_image(j, g.ny); jj < g.ny + NG; jj += g.ny)
+            for (int ii = first_image(i, g.nx); ii < g.nx + NG; ii += g.nx) {
+                const long long o = g.idx(ii, jj, kk);
+                s0 += F0[o];
+                s1 += F1[o];
+                s2 += F2[o];
+            }
+    const long long o = g.idx(i, j, k);
+    F0[o] = s0;
+    F1[o] = s1;
+    F2[o] = s2;
+}
+
+void launch_fold_guards3(const Grid& g, double* F0, double* F1, double* F2, cudaStream_t st) {
+    dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
+    fold_guards3_kernel<<<nb, bs, 0, st>>>(g, F0, F1, F2);
+}
+
 void launch_fold_guards(const Grid& g, double* F, cudaStream_t st) {
     dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
     fold_guards_kernel<<<nb, bs, 0, st>>>(g, F);

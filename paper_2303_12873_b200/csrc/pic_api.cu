@@ -416,10 +416,8 @@ int pic_step(pic_ctx* c, int nsteps) {
         }
         if (timing) cudaEventRecord(ev[2], c->stream);
         // periodic fold of the J guard cells into the interior
-        launch_fold_guards(g, c->f.Jx, c->stream);
-        launch_fold_guards(g, c->f.Jy, c->stream);
-        launch_fold_guards(g, c->f.Jz, c->stream);
-        c->launches += 3;
+        launch_fold_guards3(g, c->f.Jx, c->f.Jy, c->f.Jz, c->stream);
+        c->launches += 1;
         if (timing) cudaEventRecord(ev[3], c->stream);
         // steps 6-8
         launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);

@@ -71,6 +71,7 @@ void launch_particles_global(const Grid& g, const Fields& f, const Particles& p,
 void launch_deposit_rho(const Grid& g, const Particles& p, long long n, double q, int order, double* rho_pad,
                         cudaStream_t st);
 void launch_fold_guards(const Grid& g, double* F, cudaStream_t st);       // sum periodic images into the interior
+void launch_fold_guards3(const Grid& g, double* F0, double* F1, double* F2, cudaStream_t st);   // three components, one launch
 void launch_validate(const Grid& g, const Particles& p, long long n, DevStatus* status, cudaStream_t st);
 void launch_iota(unsigned long long* id, long long n, cudaStream_t st);
 
