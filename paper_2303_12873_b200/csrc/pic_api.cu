@@ -387,9 +387,13 @@ int pic_step(pic_ctx* c, int nsteps) {
             cudaEventRecord(ev[0], c->stream);
         }
         // J := 0 (R13).  Jx,Jy,Jz are contiguous in the arena.
-        CU(c, cudaMemsetAsync(c->f.Jx, 0, comp_bytes, c->stream));
-        CU(c, cudaMemsetAsync(c->f.Jy, 0, comp_bytes, c->stream));
-        CU(c, cudaMemsetAsync(c->f.Jz, 0, comp_bytes, c->stream));
+        if (c->f.Jx < c->f.Jy && c->f.Jy < c->f.Jz) {     // one memset over the three components (and the alignment gaps)
+            CU(c, cudaMemsetAsync(c->f.Jx, 0, (size_t)((char*)c->f.Jz - (char*)c->f.Jx) + comp_bytes, c->stream));
+        } else {
+            CU(c, cudaMemsetAsync(c->f.Jx, 0, comp_bytes, c->stream));
+            CU(c, cudaMemsetAsync(c->f.Jy, 0, comp_bytes, c->stream));
+            CU(c, cudaMemsetAsync(c->f.Jz, 0, comp_bytes, c->stream));
+        }
         if (timing) cudaEventRecord(ev[1], c->stream);
         // steps 1-5 per species, in index order (R37)
         for (int s = 0; s < c->nspecies; ++s) {
