@@ -230,6 +230,10 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    other reader -- pic_get_particles, the global-atomic
  *                    kernel -- triggers the move first); 0 = pic_sort moves
  *                    the data itself.  Same result either way.
+ *   "fuse_keys"      1 (default) = the fused per-tile kernel also writes every
+ *                    particle's new cell key, so that the next pic_sort
+ *                    skips its pass over the positions; 0 = pic_sort always
+ *                    computes the keys itself
  * Unknown name: PIC_EINVAL.
  */
 int pic_set_option(pic_ctx*, const char* name, long long value);

@@ -571,8 +571,9 @@ namespace {
 
 template <int N, class C>
 __global__ void __launch_bounds__(C::NT, C::MINB)
-particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigned int* __restrict__ perm, double q,
-                      double h, const unsigned int* __restrict__ cell_offset, int ntx, int nty, DevStatus* status) {
+particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigned int* __restrict__ perm,
+                      unsigned int* __restrict__ key_out, double q, double h,
+                      const unsigned int* __restrict__ cell_offset, int ntx, int nty, DevStatus* status) {
     constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA, DRIFT = C::DRIFT;
     using FR = FastRec<N>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -769,9 +770,17 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                     const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
                                      !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
                     bad_any = bad_any || bad;
-                    po.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
-                    po.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
-                    po.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
+                    const double xw = wrap1(x1, g.xmin, g.xmax, g.Lx), yw = wrap1(y1, g.ymin, g.ymax, g.Ly),
+                                 zw = wrap1(z1, g.zmin, g.zmax, g.Lz);
+                    po.x[ip] = xw;
+                    po.y[ip] = yw;
+                    po.z[ip] = zw;
+                    if (key_out != nullptr) {       // the next pic_sort's key (same formula as key_hist_kernel)
+                        const int ki = min(max(__double2int_rd((xw - g.xmin) * g.inv_dx), 0), g.nx - 1);
+                        const int kj = min(max(__double2int_rd((yw - g.ymin) * g.inv_dy), 0), g.ny - 1);
+                        const int kk = min(max(__double2int_rd((zw - g.zmin) * g.inv_dz), 0), g.nz - 1);
+                        key_out[ip] = (unsigned int)ki + (unsigned int)g.nx * ((unsigned int)kj + (unsigned int)g.ny * (unsigned int)kk);
+                    }
                     po.ux[ip] = ux;
                     po.uy[ip] = uy;
                     po.uz[ip] = uz;
@@ -878,12 +887,13 @@ static_assert(2 * (CfgFresh::SMEM + 1024) <= 228 * 1024, "two fresh-sort blocks 
 
 template <int N, class Cfg>
 void launch_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po, const unsigned int* perm,
-                 double q, double h, const unsigned int* cell_offset, DevStatus* status, cudaStream_t st) {
+                 unsigned int* key_out, double q, double h, const unsigned int* cell_offset, DevStatus* status,
+                 cudaStream_t st) {
     const int ntx = (g.nx + Cfg::TX - 1) / Cfg::TX, nty = (g.ny + Cfg::TY - 1) / Cfg::TY,
               ntz = (g.nz + Cfg::TZ - 1) / Cfg::TZ;
     const long long nb = (long long)ntx * nty * ntz;
-    particles_tile_kernel<N, Cfg><<<(unsigned)nb, Cfg::NT, Cfg::SMEM, st>>>(g, f, p, po, perm, q, h, cell_offset, ntx,
-                                                                           nty, status);
+    particles_tile_kernel<N, Cfg><<<(unsigned)nb, Cfg::NT, Cfg::SMEM, st>>>(g, f, p, po, perm, key_out, q, h, cell_offset,
+                                                                           ntx, nty, status);
 }
 
 template <int N, class Cfg>
@@ -909,18 +919,18 @@ int tile_setup() {
 }
 
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po,
-                          const unsigned int* perm, long long n, double q, double m, int order,
+                          const unsigned int* perm, unsigned int* key_out, long long n, double q, double m, int order,
                           const unsigned int* cell_offset, bool fresh, DevStatus* status, cudaStream_t st) {
     if (n <= 0) return 0;
     const double h = q * g.dt / (2.0 * m);
     if (fresh) {
-        if (order == 1) launch_tile<1, CfgFresh>(g, f, p, po, perm, q, h, cell_offset, status, st);
-        else if (order == 2) launch_tile<2, CfgFresh>(g, f, p, po, perm, q, h, cell_offset, status, st);
-        else launch_tile<3, CfgFresh>(g, f, p, po, perm, q, h, cell_offset, status, st);
+        if (order == 1) launch_tile<1, CfgFresh>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else if (order == 2) launch_tile<2, CfgFresh>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else launch_tile<3, CfgFresh>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
     } else {
-        if (order == 1) launch_tile<1, CfgDrift>(g, f, p, po, perm, q, h, cell_offset, status, st);
-        else if (order == 2) launch_tile<2, CfgDrift>(g, f, p, po, perm, q, h, cell_offset, status, st);
-        else launch_tile<3, CfgDrift>(g, f, p, po, perm, q, h, cell_offset, status, st);
+        if (order == 1) launch_tile<1, CfgDrift>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else if (order == 2) launch_tile<2, CfgDrift>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else launch_tile<3, CfgDrift>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
     }
     return 1;
 }

@@ -28,6 +28,10 @@ struct Species {
     // the next fused particle kernel (which writes buf[cur ^ 1]) or by materialize() for any other reader.
     unsigned int* perm = nullptr;
     bool perm_pending = false;
+    // Written by the fused per-tile kernel: the cell key of every particle's NEW position, in the container order
+    // of the buffer it wrote; the next pic_sort then skips its pass over the positions.
+    unsigned int* key = nullptr;
+    bool keys_valid = false;
 };
 
 constexpr int NSTAGE = PIC_NSTAGES;
@@ -54,7 +58,7 @@ struct pic_ctx {
     int sticky = PIC_OK;
     unsigned long long launches = 0, steps = 0, sorts = 0;
     // options
-    int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1;
+    int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1, fuse_keys = 1;
     YeeMaps yee_maps{};
     std::vector<cudaEvent_t> ev_pool;   // grows on demand; never waited on inside pic_step / pic_sort
     size_t ev_used = 0;
@@ -89,7 +93,7 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 int padded_pitch(int nx) { return (nx + 2 * NG + 1) & ~1; }   // even: rows stay 16-byte aligned (TMA)
 
 struct Layout {
-    size_t status, fields, tmp, species[MAX_SPECIES], cell_offset[MAX_SPECIES], perm[MAX_SPECIES], key, rank, block_sums,
+    size_t status, fields, tmp, species[MAX_SPECIES], cell_offset[MAX_SPECIES], perm[MAX_SPECIES], skey[MAX_SPECIES], key, rank, block_sums,
         total;
     size_t comp_bytes, np_bytes[MAX_SPECIES];
 };
@@ -108,6 +112,7 @@ int make_layout(int nx, int ny, int nz, int nspecies, const long long* np_max, L
         L->species[s] = off; off += 2 * 8 * L->np_bytes[s];
         L->cell_offset[s] = off; off += align_up((ncell + 1) * sizeof(unsigned int));
         L->perm[s] = off; off += align_up((size_t)np_max[s] * sizeof(unsigned int));
+        L->skey[s] = off; off += align_up((size_t)np_max[s] * sizeof(unsigned int));
         if (np_max[s] > npm) npm = np_max[s];
     }
     L->key = off; off += align_up((size_t)npm * sizeof(unsigned int));
@@ -293,6 +298,7 @@ int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, d
         }
         S.cell_offset = (unsigned int*)(base + L.cell_offset[s]);
         S.perm = (unsigned int*)(base + L.perm[s]);
+        S.key = (unsigned int*)(base + L.skey[s]);
     }
     c->sort_scratch.key = (unsigned int*)(base + L.key);
     c->sort_scratch.rank = (unsigned int*)(base + L.rank);
@@ -336,6 +342,7 @@ int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n,
     if (n > S.np_max) return fail(c, PIC_ENOMEM, "n = %lld exceeds np_max = %lld", n, S.np_max);
     S.cur = 0;
     S.perm_pending = false;
+    S.keys_valid = false;
     Particles& P = S.buf[0];
     const double* src[7] = {x, y, z, ux, uy, uz, w};
     double* dst[7] = {P.x, P.y, P.z, P.ux, P.uy, P.uz, P.w};
@@ -404,15 +411,19 @@ int pic_step(pic_ctx* c, int nsteps) {
                 const bool deferred = S.perm_pending;
                 const Particles& P = S.buf[S.cur];
                 const Particles& PO = deferred ? S.buf[S.cur ^ 1] : P;
-                c->launches += launch_particles_tile(g, c->f, P, PO, deferred ? S.perm : nullptr, S.n, S.q, S.m, c->order,
-                                                     S.cell_offset, S.steps_since_sort == 0 && c->tile_fresh != 0,
-                                                     c->status, c->stream);
+                const bool keys = c->fuse_keys != 0;
+                c->launches += launch_particles_tile(g, c->f, P, PO, deferred ? S.perm : nullptr, keys ? S.key : nullptr,
+                                                     S.n, S.q, S.m, c->order, S.cell_offset,
+                                                     S.steps_since_sort == 0 && c->tile_fresh != 0, c->status,
+                                                     c->stream);
+                S.keys_valid = keys;
                 if (deferred) {
                     S.cur ^= 1;
                     S.perm_pending = false;
                 }
             } else {
                 materialize(c, S);
+                S.keys_valid = false;
                 launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->status, c->stream);
                 c->launches += 1;
             }
@@ -458,7 +469,9 @@ int pic_sort(pic_ctx* c) {
         // (a still pending deferred sort is simply superseded: the keys are taken from the unsorted buffer)
         const bool deferred = c->sort_deferred != 0 && c->force_path != 1;
         c->launches += launch_sort(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, S.cell_offset,
-                                   deferred ? S.perm : nullptr, c->sort_scratch, c->stream);
+                                   deferred ? S.perm : nullptr, S.keys_valid ? S.key : nullptr, c->sort_scratch,
+                                   c->stream);
+        S.keys_valid = false;
         if (deferred) S.perm_pending = S.n > 0;
         else { S.cur ^= 1; S.perm_pending = false; }
         S.sorted = true;
@@ -603,6 +616,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     } else if (!strcmp(name, "yee_tma")) c->yee_tma = (int)value & 3;
     else if (!strcmp(name, "tile_fresh")) c->tile_fresh = value != 0;
     else if (!strcmp(name, "sort_deferred")) c->sort_deferred = value != 0;
+    else if (!strcmp(name, "fuse_keys")) c->fuse_keys = value != 0;
     else return fail(c, PIC_EINVAL, "unknown option '%s'", name);
     return PIC_OK;
 }

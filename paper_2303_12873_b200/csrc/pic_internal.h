@@ -84,8 +84,10 @@ struct SortScratch {
     long long block_sums_len;
 };
 // perm == nullptr: src is scattered into dst; else only perm[] (sorted position -> index in src) is written
+// keys_in != nullptr: per-particle cell keys of src written by the last fused particle kernel (key pass skipped)
 int launch_sort(const Grid& g, const Particles& src, const Particles& dst, long long n, unsigned int* cell_offset,
-                unsigned int* perm, const SortScratch& sc, cudaStream_t st);   // returns kernels launched
+                unsigned int* perm, const unsigned int* keys_in, const SortScratch& sc,
+                cudaStream_t st);   // returns kernels launched
 void launch_apply_perm(const Particles& src, const Particles& dst, long long n, const unsigned int* perm,
                        cudaStream_t st);                     // dst[d] = src[perm[d]]
 long long sort_block_sums_len(long long ncell);
@@ -99,8 +101,9 @@ struct TileScratch {
 // fresh = no step since the species' last sort (every particle sits in its listed cell): smaller stencil, 2 blocks/SM.
 // perm != nullptr (deferred sort): sorted particle d is read from p at perm[d] and every array (w and id too)
 // is written to pout at d; perm == nullptr: pout == p, in place.
+// key_out != nullptr: the kernel also writes the cell key of every particle's new position (for the next pic_sort)
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& pout,
-                          const unsigned int* perm, long long n, double q, double m, int order,
+                          const unsigned int* perm, unsigned int* key_out, long long n, double q, double m, int order,
                           const unsigned int* cell_offset, bool fresh, DevStatus* status,
                           cudaStream_t st);  // kernels launched
 int tile_setup();   // one-time cudaFuncSetAttribute calls; returns cudaError_t as int

@@ -169,8 +169,9 @@ def test_error_codes(B):
     assert e.value.code == B.PIC_EPHYS
 
 
+@pytest.mark.parametrize("fuse", [0, 1])
 @pytest.mark.parametrize("deferred", [0, 1])
-def test_deferred_and_immediate_sort_give_the_same_state(ora, B, deferred):
+def test_deferred_and_immediate_sort_give_the_same_state(ora, B, deferred, fuse):
     """sort_deferred = 1 (default): pic_sort writes only the permutation and the next fused per-tile kernel (or
     pic_get_particles, or the global-atomic kernel) moves the data; 0: pic_sort moves it.  Every reader must
     see the sorted container either way: sort -> get, sort -> step -> get, sort -> sort -> step, sort ->
@@ -179,6 +180,7 @@ def test_deferred_and_immediate_sort_give_the_same_state(ora, B, deferred):
     wl = W.uniform_plasma(13, 9, 6, ppc=7, u_th=0.2, order=3, seed=71, shuffle=True, protons=True)
     o, g = make_pair(ora, B.Sim, wl)
     g.set_option("sort_deferred", deferred)
+    g.set_option("fuse_keys", fuse)      # 1: the per-tile kernel writes the keys the next pic_sort uses
     before = [g.get_particles(s) for s in range(2)]
     g.sort()
     rho = g.deposit_rho(0)                        # reads the (possibly not yet moved) container: order-free
@@ -205,3 +207,10 @@ def test_deferred_and_immediate_sort_give_the_same_state(ora, B, deferred):
     g.sort()
     o.step(2); g.step(2)                           # one permuted step, one in-place (drift variant) step
     check_step_parity(o, g, wl, "deferred=%d steps 3-4" % deferred)
+    g.sort()                                       # keys written by the last step (fuse = 1) or recomputed
+    o.sort()
+    for s in range(2):
+        after = g.get_particles(s)
+        key = ora.cell_keys(o.g, after["x"], after["y"], after["z"])
+        assert (np.diff(key) >= 0).all()
+        assert np.array_equal(g.get_cell_offsets(s).astype(np.int64), o.cell_offset[s])
