@@ -383,7 +383,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=4)
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: 256^3 x 8 ppc)")
-    ap.add_argument("--n", type=int, default=None, help="override the cube edge of configs 0-2 (debugging)")
+    ap.add_argument("--n", "--cube", dest="n", type=int, default=None,
+                    help="override the cube edge of configs 0-2 (debugging; under torchrun use --cube: --n is ambiguous there)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--sort-every", type=int, default=None, help="override the workload's sort cadence (steps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
