@@ -130,8 +130,10 @@ int pic_load_particles(pic_ctx*, int species, double q, double m, long long n,
  *   periodic wrap;  B -= (dt/2) curl E;  E += dt (c^2 curl B - J/eps0);
  *   B -= (dt/2) curl E.
  * Correct for ANY particle order; a species that has been sorted (pic_sort)
- * and is still close to sorted runs the fused per-tile kernel, anything else
- * the global-atomic path.  Asynchronous.  Errors: PIC_ESTATE (no species
+ * and is still close to sorted (option "drift_watch") runs the fused per-tile
+ * kernel, anything else the global-atomic path; both evaluate the same
+ * expressions per particle, so the path only changes summation order in J.
+ * Asynchronous.  Errors: PIC_ESTATE (no species
  * loaded), PIC_EINVAL (nsteps < 0), PIC_ECUDA.
  */
 int pic_step(pic_ctx*, int nsteps);
@@ -192,7 +194,13 @@ int pic_get_cell_offsets(pic_ctx*, int species, unsigned int* offsets, int dst_o
  *   [2] particle updates done with global atomics (unsorted species, or a
  *       particle found outside its tile's halo)
  *   [3] kernels launched by the library
- *   [4] steps completed     [5] sorts completed     [6],[7] reserved
+ *   [4] steps completed     [5] sorts completed
+ *   [6] 1 = the TMA-staged Yee kernels are available, 0 = their tensor maps
+ *       could not be built at pic_init_grid and pic_step runs the plain Yee
+ *       kernels (same values, about 40 % slower); pic_last_error right after
+ *       pic_init_grid then holds a warning
+ *   [7] particle launches that ran the global-atomic kernel for a SORTED
+ *       species because the drift watch (option "drift_watch") found it stale
  */
 int pic_get_counters(pic_ctx*, unsigned long long* counters /*host*/);
 
@@ -234,6 +242,16 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    particle's new cell key, so that the next pic_sort
  *                    skips its pass over the positions; 0 = pic_sort always
  *                    computes the keys itself
+ *   "drift_watch"    1 (default) = after every fused-kernel launch the library
+ *                    reads back (asynchronously, never waiting) how many
+ *                    particles left the fast per-cell deposit path; a species
+ *                    that lost more than 20 % of them since its last pic_sort
+ *                    runs the global-atomic kernel until it is sorted again
+ *                    (the fused kernel deposits such particles one per warp
+ *                    iteration, which is slower than global atomics).  The
+ *                    values computed do not depend on the path beyond
+ *                    summation order.  0 = a sorted species always runs the
+ *                    fused kernel.  Ignored while force_path != 0.
  * Unknown name: PIC_EINVAL.
  */
 int pic_set_option(pic_ctx*, const char* name, long long value);
@@ -250,6 +268,36 @@ int pic_destroy(pic_ctx*);
 
 /* Library version string, e.g. "pic_b200 0.1 (sm_100a)". */
 const char* pic_version(void);
+
+/*
+ * + Micro-probes of the machine rates the rooflines are quoted against
+ * ("Builder must measure first: fp64 FMA peak ...,
+ * shared-memory LDS.64 wavefront rate with 1/2/4 distinct addresses per warp
+ * ..., global fp64 red.add rate at L2").  Not part of a simulation: no ctx;
+ * they run on the current CUDA device and the default stream, allocate a few
+ * MB of device scratch themselves (the one place the library calls
+ * cudaMalloc) and free it before returning.  All pointers are HOST pointers.
+ * Return PIC_OK, PIC_EINVAL (bad argument), PIC_ENOMEM or PIC_ECUDA.
+ *
+ * pic_probe_dfma: clocks per warp-wide DFMA per SM with `warps_per_sm` warps
+ *   of 8 independent dependent chains each (one block per SM, clock64).
+ * pic_probe_lds: clocks per warp-wide LDS.64 (vec_bytes 8) or LDS.128 (16) per
+ *   SM.  Lane l of every warp reads the fp64 word lane_word[l] (32 ints; even
+ *   for LDS.128) of a 6,144-word shared array, eight independent loads per
+ *   loop trip, load k displaced by k*plane_words words; lanes whose bit in
+ *   active_mask is 0 leave before the loop.
+ * pic_probe_red: lane-level red.global.add.f64 per second over the whole GPU
+ *   (8 blocks of 256 threads per SM, CUDA events) into `footprint_doubles`
+ *   doubles.  pattern 0: a warp adds to 32 consecutive doubles; 1: one 32-byte
+ *   sector per lane; 2: one 128-byte line per lane; 3: all lanes one double;
+ *   4: 8 unrelated places x 4 planes `plane_doubles` apart (an unmerged
+ *   per-cell accumulator flush); 5: 8 unrelated places x 4 consecutive doubles.
+ */
+int pic_probe_dfma(int warps_per_sm, int iters, double* clk_per_warp_instr);
+int pic_probe_lds(int vec_bytes, const int* lane_word, unsigned int active_mask, int plane_words,
+                  int warps_per_sm, int iters, double* clk_per_warp_instr);
+int pic_probe_red(int pattern, long long footprint_doubles, long long plane_doubles,
+                  int reds_per_thread, double* lane_reds_per_s);
 
 #ifdef __cplusplus
 }

@@ -23,7 +23,7 @@ _CODE_NAMES = {0: "PIC_OK", -1: "PIC_EINVAL", -2: "PIC_ENOMEM", -3: "PIC_ECUDA",
 SYMBOLS = ("pic_query_arena", "pic_init_grid", "pic_set_fields", "pic_load_particles", "pic_step",
            "pic_sort", "pic_get_fields", "pic_get_particles", "pic_deposit_rho", "pic_get_cell_offsets",
            "pic_get_counters", "pic_get_stage_ms", "pic_set_option", "pic_sync", "pic_last_error",
-           "pic_destroy", "pic_version")
+           "pic_destroy", "pic_version", "pic_probe_dfma", "pic_probe_lds", "pic_probe_red")
 
 
 class PicError(RuntimeError):
@@ -67,6 +67,9 @@ def load_library(path: str | None = None):
     L.pic_set_option.argtypes = [vp, C.c_char_p, ll]
     L.pic_sync.argtypes = [vp]
     L.pic_destroy.argtypes = [vp]
+    L.pic_probe_dfma.argtypes = [i, i, C.POINTER(d)]
+    L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
+    L.pic_probe_red.argtypes = [i, ll, ll, i, C.POINTER(d)]
     for name in SYMBOLS:
         if name not in ("pic_version", "pic_last_error"):
             getattr(L, name).restype = i
@@ -270,7 +273,8 @@ class Sim:
         arr = (C.c_ulonglong * PIC_NCOUNTERS)()
         self._check(self._L.pic_get_counters(self._ctx, arr), "pic_get_counters")
         v = list(arr)
-        return {"fast": v[0], "slow": v[1], "global": v[2], "launches": v[3], "steps": v[4], "sorts": v[5]}
+        return {"fast": v[0], "slow": v[1], "global": v[2], "launches": v[3], "steps": v[4], "sorts": v[5],
+                "yee_tma": v[6], "fallbacks": v[7]}
 
     def set_option(self, name, value):
         self._check(self._L.pic_set_option(self._ctx, name.encode(), int(value)), "pic_set_option")

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpic_b200.so")
-SOURCES = ["pic_api.cu", "yee.cu", "particles_global.cu", "particles_tile.cu", "sort.cu"]
+SOURCES = ["pic_api.cu", "yee.cu", "particles_global.cu", "particles_tile.cu", "sort.cu", "peaks.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 
@@ -60,7 +60,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     objs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in SOURCES]
     if jobs or force or not os.path.exists(LIB):
         tmp = LIB + ".tmp%d" % os.getpid()
-        r = subprocess.run([nvcc, "-shared", "-o", tmp, *objs, "-lcudart", "-lcuda"], capture_output=True, text=True)
+        r = subprocess.run([nvcc, "-shared", "-o", tmp, *objs, "-lcudart"], capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("link failed:\n%s\n%s" % (r.stdout, r.stderr))
         os.replace(tmp, LIB)

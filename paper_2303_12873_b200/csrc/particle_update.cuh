@@ -1,7 +1,7 @@
 // particle_update.cuh -- device code shared by the two particle kernels (CUDA
 // path only): gather of one component from the padded global arrays, the
 // general Esirkepov deposition of one particle through an "adder" (global
-// fp64 atomics, or the fused kernel's shared-memory tile), and the complete
+// fp64 atomics), and the complete
 // order-independent update of one particle against the GLOBAL arrays.
 // Follows SURVEY 8(c.1) steps 1-5 (BASELINE.json:north_star parts 1-3).
 #pragma once
@@ -154,8 +154,8 @@ __device__ __forceinline__ void update_particle_global(const Grid& g, const Fiel
     const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
     boris_push(h, inv_c2, ux, uy, uz, ex, ey, ez, bx, by, bz);
     // step 3: move (unwrapped)
-    const double gam = sqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
-    const double x1 = x + g.dt * ux / gam, y1 = y + g.dt * uy / gam, z1 = z + g.dt * uz / gam;
+    const double dtg = dt_over_gamma(g.dt, inv_c2, ux, uy, uz);
+    const double x1 = x + dtg * ux, y1 = y + dtg * uy, z1 = z + dtg * uz;
     // step 4: deposit from (x^n, x~^{n+1})
     const double xi1 = (x1 - g.xmin) * g.inv_dx, et1 = (y1 - g.ymin) * g.inv_dy, ze1 = (z1 - g.zmin) * g.inv_dz;
     bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1));

@@ -229,24 +229,6 @@ __device__ __noinline__ void gather_global6(const Grid& g, const Fields& f, doub
     eb[5] = gather_comp<N>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
 }
 
-// boris_push (shapes.cuh) with h / gamma taken as h * rsqrt(gamma^2): the tile kernel is bound by instruction
-// latency, and a reciprocal square root is half the instructions of a square root plus a division.
-__device__ __forceinline__ void boris_push_rsqrt(double h, double inv_c2, double& ux, double& uy, double& uz, double ex,
-                                                 double ey, double ez, double bx, double by, double bz) {
-    const double umx = ux + h * ex, umy = uy + h * ey, umz = uz + h * ez;
-    const double hg = h * rsqrt(1.0 + (umx * umx + umy * umy + umz * umz) * inv_c2);
-    const double tx = hg * bx, ty = hg * by, tz = hg * bz;
-    const double t2 = tx * tx + ty * ty + tz * tz;
-    const double f = 2.0 * __drcp_rn(1.0 + t2);      // = RN(2 / (1 + t2)): the scaling by 2 is exact
-    const double sx = f * tx, sy = f * ty, sz = f * tz;
-    const double upx = umx + (umy * tz - umz * ty);
-    const double upy = umy + (umz * tx - umx * tz);
-    const double upz = umz + (umx * ty - umy * tx);
-    ux = umx + (upy * sz - upz * sy) + h * ex;
-    uy = umy + (upz * sx - upx * sz) + h * ey;
-    uz = umz + (upx * sy - upy * sx) + h * ez;
-}
-
 // tile-relative cell index with the periodic image nearest to the tile
 template <int DRIFT>
 __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
@@ -760,10 +742,8 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                         gather_global6<N>(g, f, xi, et, ze, eb);
                         ++n_glob;
                     }
-                    boris_push_rsqrt(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
-                    // dt / gamma as dt * rsqrt(gamma^2): one reciprocal square root instead of a square root and
-                    // three divisions (a few ulp away from dt u / gamma; the 1-step bound is 1e-12)
-                    const double dtg = g.dt * rsqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
+                    boris_push(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
+                    const double dtg = dt_over_gamma(g.dt, inv_c2, ux, uy, uz);
                     const double x1 = x + dtg * ux, y1 = y + dtg * uy, z1 = z + dtg * uz;
                     const double xi1 = (x1 - g.xmin) * g.inv_dx, et1 = (y1 - g.ymin) * g.inv_dy,
                                  ze1 = (z1 - g.zmin) * g.inv_dz;

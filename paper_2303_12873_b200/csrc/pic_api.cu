@@ -9,6 +9,8 @@
 #include <new>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>     // header-only; ranges are no-ops unless a profiler injects itself
+
 #include "pic_internal.h"
 
 using namespace pic;
@@ -32,7 +34,15 @@ struct Species {
     // of the buffer it wrote; the next pic_sort then skips its pass over the positions.
     unsigned int* key = nullptr;
     bool keys_valid = false;
+    // Drift watch: share of the last fused-kernel launch that left the fast path (slow + global), read back
+    // asynchronously; above DRIFT_LIMIT the species runs the global-atomic kernel until its next pic_sort.
+    bool degraded = false;
 };
+
+// A species whose last fused-kernel launch sent more than this share of its particles down the warp-serialised
+// slow path (or the global gather) is faster on the global-atomic kernel: the slow path deposits ONE particle
+// per warp iteration.
+constexpr double DRIFT_LIMIT = 0.20;
 
 constexpr int NSTAGE = PIC_NSTAGES;
 constexpr int EV_PER_STEP = 7, EV_PER_SORT = 2;
@@ -60,6 +70,16 @@ struct pic_ctx {
     // options
     int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1, fuse_keys = 1;
     YeeMaps yee_maps{};
+    int device = 0;                     // ordinal of the device the arena lives on; made current by every call
+    int yee_tma_ok = 0;                 // tensor maps built: the TMA-staged Yee kernels are available
+    // drift watch (pinned host memory, one event): counters before the first and after each species' launch of
+    // the last pic_step iteration; evaluated by a later pic_step once the event has completed, never waited on
+    DevStatus* watch = nullptr;         // [MAX_SPECIES + 1]
+    cudaEvent_t watch_ev = nullptr;
+    bool watch_armed = false;
+    bool watch_tile[MAX_SPECIES] = {false};
+    int drift_watch = 1;
+    unsigned long long fallbacks = 0;   // particle launches that took the global kernel because of the watch
     std::vector<cudaEvent_t> ev_pool;   // grows on demand; never waited on inside pic_step / pic_sort
     size_t ev_used = 0;
     std::vector<TimedSpan> spans;
@@ -126,6 +146,8 @@ int check_dims(int nx, int ny, int nz, int order, int nspecies, const long long*
     if (nx < 1 || ny < 1 || nz < 1 || order < 1 || order > 3 || nspecies < 1 || nspecies > MAX_SPECIES || !np_max)
         return PIC_EINVAL;
     if ((long long)nx * ny * nz >= (1LL << 31) - 1) return PIC_EINVAL;
+    // several kernels launch with gridDim.y / gridDim.z = the padded extents in y and z
+    if (ny + 2 * NG > 65535 || nz + 2 * NG > 65535) return PIC_EINVAL;
     for (int s = 0; s < nspecies; ++s)
         if (np_max[s] < 0 || np_max[s] >= (1LL << 31)) return PIC_EINVAL;
     return PIC_OK;
@@ -178,6 +200,7 @@ int copy_in(pic_ctx* c, const double* src, double* pad, int on_device) {
     }
     launch_fill_guards(c->g, pad, c->stream);
     c->launches += 2;
+    CU(c, cudaGetLastError());
     if (!on_device) CU(c, cudaStreamSynchronize(c->stream));
     return PIC_OK;
 }
@@ -219,8 +242,34 @@ bool take_events(pic_ctx* c, int n, size_t* first) {
 
 bool use_tile_path(const pic_ctx* c, const Species& s) {
     if (c->force_path == 1) return false;
-    return s.sorted;
+    if (c->force_path == 2) return s.sorted;
+    return s.sorted && !s.degraded;
 }
+
+// Drift watch, host side: if the counters of the last watched pic_step iteration have arrived, mark every
+// species whose fused-kernel launch left the fast path for more than DRIFT_LIMIT of its particles.
+void poll_watch(pic_ctx* c) {
+    if (!c->watch_armed || cudaEventQuery(c->watch_ev) != cudaSuccess) {
+        cudaGetLastError();      // cudaErrorNotReady is not an error
+        return;
+    }
+    c->watch_armed = false;
+    for (int s = 0; s < c->nspecies; ++s) {
+        Species& S = c->sp[s];
+        if (!c->watch_tile[s] || S.n == 0 || S.steps_since_sort == 0) continue;   // sorted since: nothing to conclude
+        const DevStatus &a = c->watch[s], &b = c->watch[s + 1];
+        const double off_fast = (double)((b.n_slow - a.n_slow) + (b.n_global - a.n_global));
+        if (off_fast > DRIFT_LIMIT * (double)S.n) S.degraded = true;
+    }
+}
+
+#define ENTER(c)                                                                   \
+    do {                                                                           \
+        if (!(c)) return PIC_EINVAL;                                               \
+        if ((c)->sticky != PIC_OK) return (c)->sticky;                             \
+        cudaError_t e_ = cudaSetDevice((c)->device);                               \
+        if (e_ != cudaSuccess) return cuda_fail((c), e_, "cudaSetDevice");         \
+    } while (0)
 
 // Carry out a deferred sort for a reader other than the fused per-tile kernel.
 void materialize(pic_ctx* c, Species& S) {
@@ -280,6 +329,16 @@ int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, d
     c->order = order;
     c->nspecies = nspecies;
     c->stream = (cudaStream_t)cuda_stream;
+    {   // the device the arena lives on becomes the context's device (every later call makes it current)
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, arena_dev) != cudaSuccess || pa.type != cudaMemoryTypeDevice ||
+            cudaSetDevice(pa.device) != cudaSuccess) {
+            cudaGetLastError();
+            delete c;
+            return PIC_EINVAL;
+        }
+        c->device = pa.device;
+    }
 
     char* base = (char*)arena_dev;
     c->status = (DevStatus*)(base + L.status);
@@ -308,19 +367,28 @@ int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, d
     // zero the status block, the fields and the scratch component (particles are written at load)
     cudaError_t e = cudaMemsetAsync(base, 0, L.tmp + L.comp_bytes, c->stream);
     if (e == cudaSuccess) e = (cudaError_t)tile_setup();
-    make_yee_maps(c->g, c->f, &c->yee_maps);   // on failure yee_maps.valid stays 0: plain Yee kernels
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->watch, sizeof(DevStatus) * (MAX_SPECIES + 1));
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->watch_ev, cudaEventDisableTiming);
     if (e != cudaSuccess) {
+        if (c->watch) cudaFreeHost(c->watch);
         delete c;
         return PIC_ECUDA;
     }
+    // Tensor maps for the TMA-staged Yee kernels.  A failure is not fatal (the plain kernels compute the same
+    // values) but it is not silent either: pic_last_error says so and pic_get_counters[6] stays 0.
+    const int yrc = make_yee_maps(c->g, c->f, &c->yee_maps);
+    c->yee_tma_ok = (yrc == 0 && c->yee_maps.valid) ? 1 : 0;
+    if (!c->yee_tma_ok)
+        snprintf(c->err, sizeof(c->err),
+                 "warning: tensor maps for the TMA-staged Yee kernels could not be built (make_yee_maps = %d); "
+                 "pic_step uses the plain Yee kernels", yrc);
     *out = c;
     return PIC_OK;
 }
 
 int pic_set_fields(pic_ctx* c, const double* Ex, const double* Ey, const double* Ez, const double* Bx,
                    const double* By, const double* Bz, int src_on_device) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     const double* src[6] = {Ex, Ey, Ez, Bx, By, Bz};
     double* dst[6] = {c->f.Ex, c->f.Ey, c->f.Ez, c->f.Bx, c->f.By, c->f.Bz};
     for (int k = 0; k < 6; ++k) {
@@ -333,8 +401,7 @@ int pic_set_fields(pic_ctx* c, const double* Ex, const double* Ey, const double*
 int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n, const double* x, const double* y,
                        const double* z, const double* ux, const double* uy, const double* uz, const double* w,
                        int src_on_device) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     if (species < 0 || species >= c->nspecies) return fail(c, PIC_EINVAL, "species index %d out of range", species);
     if (n < 0 || !(m > 0.0) || !isfinite(q) || !isfinite(m)) return fail(c, PIC_EINVAL, "bad n, q or m");
     if (n > 0 && (!x || !y || !z || !ux || !uy || !uz || !w)) return fail(c, PIC_EINVAL, "NULL particle array");
@@ -352,11 +419,12 @@ int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n,
     launch_iota(P.id, n, c->stream);
     launch_validate(c->g, P, n, c->status, c->stream);
     c->launches += (n > 0) ? 2 : 0;
+    CU(c, cudaGetLastError());
     DevStatus h;
     CU(c, cudaMemcpyAsync(&h, c->status, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     S.q = q; S.m = m; S.n = n;
-    S.sorted = false; S.steps_since_sort = 0;
+    S.sorted = false; S.steps_since_sort = 0; S.degraded = false;
     if (h.ebox) {
         int zero = 0;
         CU(c, cudaMemcpyAsync(&c->status->ebox, &zero, sizeof(int), cudaMemcpyHostToDevice, c->stream));
@@ -369,8 +437,7 @@ int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n,
 }
 
 int pic_step(pic_ctx* c, int nsteps) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     if (nsteps < 0) return fail(c, PIC_EINVAL, "nsteps < 0");
     bool any = false;
     for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
@@ -382,8 +449,8 @@ int pic_step(pic_ctx* c, int nsteps) {
     const bool timing = c->stage_timing != 0;
     const Grid& g = c->g;
     const size_t comp_bytes = (size_t)g.npad * sizeof(double);
-    const YeeMaps* tma_B = ((c->yee_tma & 1) && c->yee_maps.valid) ? &c->yee_maps : nullptr;
-    const YeeMaps* tma_E = ((c->yee_tma & 2) && c->yee_maps.valid) ? &c->yee_maps : nullptr;
+    const YeeMaps* tma_B = ((c->yee_tma & 1) && c->yee_tma_ok) ? &c->yee_maps : nullptr;
+    const YeeMaps* tma_E = ((c->yee_tma & 2) && c->yee_tma_ok) ? &c->yee_maps : nullptr;
     for (int it = 0; it < nsteps; ++it) {
         cudaEvent_t* ev = nullptr;
         if (timing) {
@@ -393,7 +460,9 @@ int pic_step(pic_ctx* c, int nsteps) {
             ev = c->ev_pool.data() + first;
             cudaEventRecord(ev[0], c->stream);
         }
+        nvtxRangePushA("pic_step");
         // J := 0 (R13).  Jx,Jy,Jz are contiguous in the arena.
+        nvtxRangePushA("zero_J");
         if (c->f.Jx < c->f.Jy && c->f.Jy < c->f.Jz) {     // one memset over the three components (and the alignment gaps)
             CU(c, cudaMemsetAsync(c->f.Jx, 0, (size_t)((char*)c->f.Jz - (char*)c->f.Jx) + comp_bytes, c->stream));
         } else {
@@ -401,48 +470,72 @@ int pic_step(pic_ctx* c, int nsteps) {
             CU(c, cudaMemsetAsync(c->f.Jy, 0, comp_bytes, c->stream));
             CU(c, cudaMemsetAsync(c->f.Jz, 0, comp_bytes, c->stream));
         }
+        nvtxRangePop();
         if (timing) cudaEventRecord(ev[1], c->stream);
         // steps 1-5 per species, in index order (R37)
+        nvtxRangePushA("particles");
+        if (c->drift_watch) poll_watch(c);
+        // the watch is re-armed only when no earlier snapshot is still in flight (its pinned slots are reused)
+        const bool watch = c->drift_watch && !c->watch_armed && c->force_path == 0;
+        if (watch) {
+            CU(c, cudaMemcpyAsync(&c->watch[0], c->status, sizeof(DevStatus), cudaMemcpyDeviceToHost, c->stream));
+            for (int s = 0; s < c->nspecies; ++s) c->watch_tile[s] = false;
+        }
         for (int s = 0; s < c->nspecies; ++s) {
             Species& S = c->sp[s];
-            if (!S.loaded || S.n == 0) continue;
-            if (use_tile_path(c, S)) {
-                // a deferred sort is carried out here: inputs read through perm, outputs to the other buffer
-                const bool deferred = S.perm_pending;
-                const Particles& P = S.buf[S.cur];
-                const Particles& PO = deferred ? S.buf[S.cur ^ 1] : P;
-                const bool keys = c->fuse_keys != 0;
-                c->launches += launch_particles_tile(g, c->f, P, PO, deferred ? S.perm : nullptr, keys ? S.key : nullptr,
-                                                     S.n, S.q, S.m, c->order, S.cell_offset,
-                                                     S.steps_since_sort == 0 && c->tile_fresh != 0, c->status,
-                                                     c->stream);
-                S.keys_valid = keys;
-                if (deferred) {
-                    S.cur ^= 1;
-                    S.perm_pending = false;
+            if (S.loaded && S.n > 0) {
+                if (use_tile_path(c, S)) {
+                    // a deferred sort is carried out here: inputs read through perm, outputs to the other buffer
+                    const bool deferred = S.perm_pending;
+                    const Particles& P = S.buf[S.cur];
+                    const Particles& PO = deferred ? S.buf[S.cur ^ 1] : P;
+                    const bool keys = c->fuse_keys != 0;
+                    c->launches += launch_particles_tile(g, c->f, P, PO, deferred ? S.perm : nullptr,
+                                                         keys ? S.key : nullptr, S.n, S.q, S.m, c->order, S.cell_offset,
+                                                         S.steps_since_sort == 0 && c->tile_fresh != 0, c->status,
+                                                         c->stream);
+                    S.keys_valid = keys;
+                    if (deferred) {
+                        S.cur ^= 1;
+                        S.perm_pending = false;
+                    }
+                    if (watch) c->watch_tile[s] = true;
+                } else {
+                    if (S.sorted && S.degraded) c->fallbacks += 1;
+                    materialize(c, S);
+                    S.keys_valid = false;
+                    launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->status, c->stream);
+                    c->launches += 1;
                 }
-            } else {
-                materialize(c, S);
-                S.keys_valid = false;
-                launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->status, c->stream);
-                c->launches += 1;
+                S.steps_since_sort += 1;
             }
-            S.steps_since_sort += 1;
+            if (watch)
+                CU(c, cudaMemcpyAsync(&c->watch[s + 1], c->status, sizeof(DevStatus), cudaMemcpyDeviceToHost, c->stream));
         }
+        if (watch) {
+            CU(c, cudaEventRecord(c->watch_ev, c->stream));
+            c->watch_armed = true;
+        }
+        nvtxRangePop();
         if (timing) cudaEventRecord(ev[2], c->stream);
         // periodic fold of the J guard cells into the interior
+        nvtxRangePushA("fold_J");
         launch_fold_guards3(g, c->f.Jx, c->f.Jy, c->f.Jz, c->stream);
         c->launches += 1;
+        nvtxRangePop();
         if (timing) cudaEventRecord(ev[3], c->stream);
         // steps 6-8
+        nvtxRangePushA("yee");
         launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
         if (timing) cudaEventRecord(ev[4], c->stream);
         launch_push_E(g, c->f, g.dt, tma_E, c->stream);
         if (timing) cudaEventRecord(ev[5], c->stream);
         launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
+        nvtxRangePop();
         c->launches += 3;
         c->steps += 1;
         if (timing) cudaEventRecord(ev[6], c->stream);
+        nvtxRangePop();
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_step launch");
@@ -450,15 +543,15 @@ int pic_step(pic_ctx* c, int nsteps) {
 }
 
 int pic_sort(pic_ctx* c) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     bool any = false;
     for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
     if (!any) return fail(c, PIC_ESTATE, "pic_sort before any pic_load_particles");
     cudaEvent_t* ev = nullptr;
+    nvtxRangePushA("pic_sort");
     if (c->stage_timing) {
         size_t first;
-        if (!take_events(c, EV_PER_SORT, &first)) return fail(c, PIC_ECUDA, "cudaEventCreate failed");
+        if (!take_events(c, EV_PER_SORT, &first)) { nvtxRangePop(); return fail(c, PIC_ECUDA, "cudaEventCreate failed"); }
         c->spans.push_back(TimedSpan{first, 1});
         ev = c->ev_pool.data() + first;
         cudaEventRecord(ev[0], c->stream);
@@ -476,8 +569,10 @@ int pic_sort(pic_ctx* c) {
         else { S.cur ^= 1; S.perm_pending = false; }
         S.sorted = true;
         S.steps_since_sort = 0;
+        S.degraded = false;
     }
     if (ev) cudaEventRecord(ev[1], c->stream);
+    nvtxRangePop();
     c->sorts += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_sort launch");
@@ -486,8 +581,7 @@ int pic_sort(pic_ctx* c) {
 
 int pic_get_fields(pic_ctx* c, double* Ex, double* Ey, double* Ez, double* Bx, double* By, double* Bz, double* Jx,
                    double* Jy, double* Jz, int dst_on_device) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     double* dst[9] = {Ex, Ey, Ez, Bx, By, Bz, Jx, Jy, Jz};
     const double* src[9] = {c->f.Ex, c->f.Ey, c->f.Ez, c->f.Bx, c->f.By, c->f.Bz, c->f.Jx, c->f.Jy, c->f.Jz};
     for (int k = 0; k < 9; ++k) {
@@ -499,8 +593,7 @@ int pic_get_fields(pic_ctx* c, double* Ex, double* Ey, double* Ez, double* Bx, d
 
 int pic_get_particles(pic_ctx* c, int species, long long* n, double* x, double* y, double* z, double* ux,
                       double* uy, double* uz, double* w, unsigned long long* id, int dst_on_device) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     if (species < 0 || species >= c->nspecies) return fail(c, PIC_EINVAL, "species index %d out of range", species);
     Species& S = c->sp[species];
     if (!S.loaded) return fail(c, PIC_ESTATE, "species %d was never loaded", species);
@@ -516,8 +609,7 @@ int pic_get_particles(pic_ctx* c, int species, long long* n, double* x, double* 
 }
 
 int pic_deposit_rho(pic_ctx* c, int species, double* rho, int dst_on_device) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     if (species < -1 || species >= c->nspecies || !rho) return fail(c, PIC_EINVAL, "bad species index or NULL rho");
     if (species >= 0 && !c->sp[species].loaded) return fail(c, PIC_ESTATE, "species %d was never loaded", species);
     // tmp serves as the padded rho: deposit with global atomics, fold the guards, strip them on the way out
@@ -548,8 +640,7 @@ int pic_deposit_rho(pic_ctx* c, int species, double* rho, int dst_on_device) {
 }
 
 int pic_get_cell_offsets(pic_ctx* c, int species, unsigned int* offsets, int dst_on_device) {
-    if (!c) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    ENTER(c);
     if (species < 0 || species >= c->nspecies || !offsets) return fail(c, PIC_EINVAL, "bad species or NULL offsets");
     Species& S = c->sp[species];
     if (!S.loaded || !S.sorted) return fail(c, PIC_ESTATE, "species %d was never sorted", species);
@@ -560,8 +651,8 @@ int pic_get_cell_offsets(pic_ctx* c, int species, unsigned int* offsets, int dst
 }
 
 int pic_get_counters(pic_ctx* c, unsigned long long* counters) {
-    if (!c || !counters) return PIC_EINVAL;
-    if (c->sticky != PIC_OK) return c->sticky;
+    if (!counters) return PIC_EINVAL;
+    ENTER(c);
     DevStatus h;
     CU(c, cudaMemcpyAsync(&h, c->status, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
@@ -571,7 +662,8 @@ int pic_get_counters(pic_ctx* c, unsigned long long* counters) {
     counters[3] = c->launches;
     counters[4] = c->steps;
     counters[5] = c->sorts;
-    counters[6] = counters[7] = 0;
+    counters[6] = (unsigned long long)c->yee_tma_ok;
+    counters[7] = c->fallbacks;
     return PIC_OK;
 }
 
@@ -617,6 +709,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     else if (!strcmp(name, "tile_fresh")) c->tile_fresh = value != 0;
     else if (!strcmp(name, "sort_deferred")) c->sort_deferred = value != 0;
     else if (!strcmp(name, "fuse_keys")) c->fuse_keys = value != 0;
+    else if (!strcmp(name, "drift_watch")) c->drift_watch = value != 0;
     else return fail(c, PIC_EINVAL, "unknown option '%s'", name);
     return PIC_OK;
 }
@@ -633,7 +726,13 @@ const char* pic_last_error(pic_ctx* c) {
 
 int pic_destroy(pic_ctx* c) {
     if (!c) return PIC_EINVAL;
+    cudaSetDevice(c->device);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    if (c->watch_ev) {
+        cudaEventSynchronize(c->watch_ev);      // a snapshot copy may still be writing the pinned block
+        cudaEventDestroy(c->watch_ev);
+    }
+    if (c->watch) cudaFreeHost(c->watch);
     delete c;
     return PIC_OK;
 }

@@ -93,7 +93,7 @@ void launch_apply_perm(const Particles& src, const Particles& dst, long long n, 
 long long sort_block_sums_len(long long ncell);
 
 // ---- particles_tile.cu ------------------------------------------------------
-// fused gather + push + deposit per cell-sorted tile (shared-memory stencil and J tile).
+// fused gather + push + deposit per cell-sorted tile (shared-memory stencil, per-cell register accumulators).
 struct TileScratch {
     void* ptr;
     size_t bytes;

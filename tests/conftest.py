@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    config.addinivalue_line("markers", "slow: parity at SURVEY.md 8(d)'s parity sizes / full sizes (minutes, not seconds)")
 
 
 @pytest.fixture(scope="session")

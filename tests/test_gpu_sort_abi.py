@@ -214,3 +214,60 @@ def test_deferred_and_immediate_sort_give_the_same_state(ora, B, deferred, fuse)
         key = ora.cell_keys(o.g, after["x"], after["y"], after["z"])
         assert (np.diff(key) >= 0).all()
         assert np.array_equal(g.get_cell_offsets(s).astype(np.int64), o.cell_offset[s])
+
+
+def test_drift_watch_moves_a_stale_species_to_the_global_kernel(ora, B):
+    """ADVICE r1 / include/pic.h "drift_watch": a species sorted once and then stepped at 0.3 c leaves its
+    listed cells; once more than 20 % of a launch left the fast deposit path the next steps run the
+    global-atomic kernel (counter [7]) until the next pic_sort.  The values do not depend on the path."""
+    from parity_util import TOL_FIELD_L2_10STEP, field_l2_error
+    wl = W.uniform_plasma(16, 12, 12, ppc=6, u_th=0.3, order=3, seed=91)
+    o, g = make_pair(ora, B.Sim, wl)
+    g.sort()
+    for _ in range(8):
+        g.step(1)
+        g.sync()                     # lets the asynchronous counter snapshot of this step arrive
+    o.step(8)
+    c = g.counters()
+    assert c["fallbacks"] >= 1 and c["global"] == c["fallbacks"] * wl.nparticles, c
+    assert c["fast"] + c["slow"] + c["global"] == 8 * wl.nparticles
+    assert field_l2_error(o.get_fields(), g.get_fields()) <= TOL_FIELD_L2_10STEP
+    g.sort()                         # sorted again: back on the fused kernel
+    g.step(1)
+    c2 = g.counters()
+    assert c2["fallbacks"] == c["fallbacks"] and c2["global"] == c["global"]
+    # with the watch off a sorted species stays on the fused kernel whatever its drift
+    g2 = B.Sim.from_workload(wl)
+    g2.set_option("drift_watch", 0)
+    g2.sort()
+    for _ in range(6):
+        g2.step(1)
+        g2.sync()
+    assert g2.counters()["fallbacks"] == 0 and g2.counters()["global"] < 0.2 * 6 * wl.nparticles
+
+
+def test_counters_report_the_yee_path_and_init_rejects_oversized_y(B):
+    d = 0.5e-6
+    g = B.Sim(8, 8, 8, d, d, d, 0, 0, 0, W.courant_dt(d, d, d), 1, [8])
+    assert g.counters()["yee_tma"] == 1, g.last_error()     # a B200 with a current driver builds the tensor maps
+    with pytest.raises(B.PicError) as e:                     # gridDim.y = ny + 2 NG must fit 65535
+        B.query_arena(4, 65530, 4, 1, [8])
+    assert e.value.code == B.PIC_EINVAL
+
+
+def test_machine_rate_probes_return_sane_numbers():
+    """pic_probe_* (SURVEY 8(d) "Builder must measure first"): DFMA issues at about 0.5 clk per warp
+    instruction per SM; a conflict-free full-warp LDS.64 returns 256 B = 2 clk; REDs make progress."""
+    from paper_2303_12873_b200 import peaks
+    clk = peaks.probe_dfma(16, iters=2000)
+    assert 0.45 <= clk <= 0.7, clk
+    words = [64 + l for l in range(32)]
+    clk = peaks.probe_lds(8, words, 0xFFFFFFFF, 16, iters=2000)
+    assert 1.8 <= clk <= 2.6, clk
+    assert peaks.probe_red(0, 5 << 20, n=16) > 1e9
+
+
+def test_selfcheck_module_passes():
+    from paper_2303_12873_b200 import selfcheck
+    selfcheck.run_case(12, 3, "drift", verbose=False)
+    selfcheck.run_case(12, 1, "global", verbose=False)
