@@ -281,6 +281,8 @@ const char* pic_version(void);
  *
  * pic_probe_dfma: clocks per warp-wide DFMA per SM with `warps_per_sm` warps
  *   of 8 independent dependent chains each (one block per SM, clock64).
+ * pic_probe_dmma: clocks per warp-wide DMMA m8n8k4 (256 fp64 FMA) per SM, 8
+ *   independent accumulator fragments per warp.
  * pic_probe_lds: clocks per warp-wide LDS.64 (vec_bytes 8) or LDS.128 (16) per
  *   SM.  Lane l of every warp reads the fp64 word lane_word[l] (32 ints; even
  *   for LDS.128) of a 6,144-word shared array, eight independent loads per
@@ -294,6 +296,7 @@ const char* pic_version(void);
  *   per-cell accumulator flush); 5: 8 unrelated places x 4 consecutive doubles.
  */
 int pic_probe_dfma(int warps_per_sm, int iters, double* clk_per_warp_instr);
+int pic_probe_dmma(int warps_per_sm, int iters, double* clk_per_warp_instr);
 int pic_probe_lds(int vec_bytes, const int* lane_word, unsigned int active_mask, int plane_words,
                   int warps_per_sm, int iters, double* clk_per_warp_instr);
 int pic_probe_red(int pattern, long long footprint_doubles, long long plane_doubles,

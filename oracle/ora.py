@@ -57,6 +57,10 @@ def lib():
         L.ora_courant_dt.restype = C.c_double
         L.ora_courant_dt.argtypes = [G]
         L.ora_gather.argtypes = [G, C.c_int, C.c_longlong] + [_dp] * 15
+        L.ora_shape0.restype = C.c_double
+        L.ora_shape0.argtypes = [C.c_double]
+        L.ora_gather_variant.argtypes = [G, C.c_int, C.c_int, C.c_longlong] + [_dp] * 15
+        L.ora_smooth_binomial.argtypes = [G, C.c_int, _dp]
         L.ora_boris.argtypes = [C.c_longlong, C.c_double, C.c_double, C.c_double] + [_dp] * 9
         L.ora_move.argtypes = [C.c_longlong, C.c_double] + [_dp] * 9
         L.ora_deposit_esirkepov.argtypes = [G, C.c_int, C.c_longlong, C.c_double, C.c_double] + [_dp] * 10
@@ -115,6 +119,26 @@ def gather(g: OraGrid, order: int, x, y, z, E, B):
     _check(lib().ora_gather(C.byref(g), order, n, _d(x), _d(y), _d(z), *[_d(a) for a in F],
                             *[_d(a) for a in out]), "gather")
     return tuple(out)
+
+
+def shape0(r: float) -> float:
+    return lib().ora_shape0(float(r))
+
+
+def gather_variant(g: OraGrid, order: int, variant: int, x, y, z, E, B):
+    """NEXT-3: variant 0 = gather(); 1 = order n-1 along each component's staggered directions."""
+    x, y, z = _f64(x), _f64(y), _f64(z)
+    n = x.size
+    F = [_f64(a) for a in (*E, *B)]
+    out = [np.empty(n) for _ in range(6)]
+    _check(lib().ora_gather_variant(C.byref(g), order, variant, n, _d(x), _d(y), _d(z), *[_d(a) for a in F],
+                                    *[_d(a) for a in out]), "gather_variant")
+    return tuple(out)
+
+
+def smooth_binomial(g: OraGrid, npass: int, F: np.ndarray):
+    """NEXT-3: in-place periodic 1-2-1 smoothing, `npass` passes of x, y, z."""
+    _check(lib().ora_smooth_binomial(C.byref(g), int(npass), _d(F)), "smooth_binomial")
 
 
 def boris(q, m, dt, ux, uy, uz, Ep, Bp):
@@ -181,8 +205,12 @@ class OracleSim:
     """The PIC cycle of SURVEY.md 8(c.1), steps 1-8, on host arrays.  Mirrors
     the method names of the CUDA binding so one test can drive both."""
 
-    def __init__(self, nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, dt, order, nspecies):
+    def __init__(self, nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, dt, order, nspecies, gather_variant=0,
+                 smooth_passes=0):
         self.g = make_grid(nx, ny, nz, dx, dy, dz, xmin, ymin, zmin)
+        if gather_variant not in (0, 1) or smooth_passes < 0:
+            raise ValueError("gather_variant must be 0 or 1, smooth_passes >= 0")
+        self.gather_variant, self.smooth_passes = int(gather_variant), int(smooth_passes)   # NEXT-3 options
         if order not in (1, 2, 3):
             raise ValueError("order must be 1, 2 or 3")
         if not (0.0 < dt <= courant_dt(self.g)):
@@ -216,12 +244,18 @@ class OracleSim:
             for sp in self.species:
                 if sp is None or sp.x.size == 0:
                     continue
-                F = gather(g, n, sp.x, sp.y, sp.z, self.E, self.B)                 # step 1
+                if self.gather_variant:
+                    F = gather_variant(g, n, self.gather_variant, sp.x, sp.y, sp.z, self.E, self.B)
+                else:
+                    F = gather(g, n, sp.x, sp.y, sp.z, self.E, self.B)             # step 1
                 boris(sp.q, sp.m, dt, sp.ux, sp.uy, sp.uz, F[:3], F[3:])          # step 2
                 x1, y1, z1 = move(dt, sp.x, sp.y, sp.z, sp.ux, sp.uy, sp.uz)      # step 3
                 deposit_esirkepov(g, n, sp.q, dt, sp.w, (sp.x, sp.y, sp.z), (x1, y1, z1), self.J)  # 4
                 wrap(g, x1, y1, z1)                                               # step 5
                 sp.x, sp.y, sp.z = x1, y1, z1
+            for a in self.J:                       # NEXT-3: optional binomial smoothing of J
+                if self.smooth_passes:
+                    smooth_binomial(g, self.smooth_passes, a)
             yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 6
             yee_push_E(g, dt, self.E, self.B, self.J)                             # step 7
             yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 8

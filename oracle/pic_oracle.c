@@ -109,6 +109,90 @@ int ora_gather(const ora_grid* g, int order, long long np,
     return 0;
 }
 
+/* ---- NEXT-3 (8(c.2) item 5): gather variants --------------------------------
+ * variant 0: the same order n in every direction (ora_gather, reading R5).
+ * variant 1: "energy-conserving" / Galerkin gather: along every direction in which the
+ *   component is STAGGERED the shape order is n-1, along the others n:
+ *   Ex_p = sum S^{n-1}(xi-i-1/2) S^n(eta-j) S^n(zeta-k) Ex[i,j,k], Bx_p = sum S^n(xi-i)
+ *   S^{n-1}(eta-j-1/2) S^{n-1}(zeta-k-1/2) Bx[i,j,k], and cyclic permutations.
+ * S^0 is the top-hat on the half-open interval [-1/2, 1/2) (so that a particle on a cell
+ * boundary belongs to the cell floor(xi) puts it in). */
+double ora_shape0(double r) { return (r >= -0.5 && r < 0.5) ? 1.0 : 0.0; }
+
+static double shape_any(int n, double r) { return n == 0 ? ora_shape0(r) : ora_shape(n, r); }
+
+/* one component, staggering offsets (ox,oy,oz) in {0, 1/2}, per-direction orders (n1,n2,n3) */
+static double gather_one_orders(const ora_grid* g, int n, int n1, int n2, int n3, double xi, double eta,
+                                double zeta, double ox, double oy, double oz, const double* F)
+{
+    int h = window_h(n), wn = 2 * h + 2;      /* the order-n window contains every lower-order support */
+    long long i0 = (long long)floor(xi), j0 = (long long)floor(eta), k0 = (long long)floor(zeta);
+    double sum = 0.0;
+    for (int c = 0; c < wn; ++c) {
+        long long k = k0 - h + c;
+        double sz = shape_any(n3, zeta - (double)k - oz);
+        for (int b = 0; b < wn; ++b) {
+            long long j = j0 - h + b;
+            double sy = shape_any(n2, eta - (double)j - oy);
+            for (int a = 0; a < wn; ++a) {
+                long long i = i0 - h + a;
+                double sx = shape_any(n1, xi - (double)i - ox);
+                sum += sx * sy * sz * F[gidx(g, i, j, k)];
+            }
+        }
+    }
+    return sum;
+}
+
+int ora_gather_variant(const ora_grid* g, int order, int variant, long long np,
+                       const double* x, const double* y, const double* z,
+                       const double* Ex, const double* Ey, const double* Ez,
+                       const double* Bx, const double* By, const double* Bz,
+                       double* Exp, double* Eyp, double* Ezp,
+                       double* Bxp, double* Byp, double* Bzp)
+{
+    if (order < 1 || order > 3 || variant < 0 || variant > 1) return -1;
+    if (variant == 0)
+        return ora_gather(g, order, np, x, y, z, Ex, Ey, Ez, Bx, By, Bz, Exp, Eyp, Ezp, Bxp, Byp, Bzp);
+    int n = order, m = order - 1;             /* m: order along a staggered direction */
+    double inv_dx = 1.0 / g->dx, inv_dy = 1.0 / g->dy, inv_dz = 1.0 / g->dz;
+    for (long long p = 0; p < np; ++p) {
+        double xi = (x[p] - g->xmin) * inv_dx;
+        double eta = (y[p] - g->ymin) * inv_dy;
+        double zeta = (z[p] - g->zmin) * inv_dz;
+        Exp[p] = gather_one_orders(g, n, m, n, n, xi, eta, zeta, 0.5, 0.0, 0.0, Ex);
+        Eyp[p] = gather_one_orders(g, n, n, m, n, xi, eta, zeta, 0.0, 0.5, 0.0, Ey);
+        Ezp[p] = gather_one_orders(g, n, n, n, m, xi, eta, zeta, 0.0, 0.0, 0.5, Ez);
+        Bxp[p] = gather_one_orders(g, n, n, m, m, xi, eta, zeta, 0.0, 0.5, 0.5, Bx);
+        Byp[p] = gather_one_orders(g, n, m, n, m, xi, eta, zeta, 0.5, 0.0, 0.5, By);
+        Bzp[p] = gather_one_orders(g, n, m, m, n, xi, eta, zeta, 0.5, 0.5, 0.0, Bz);
+    }
+    return 0;
+}
+
+/* NEXT-3: binomial (1-2-1) smoothing of one field component, periodic, `npass` passes; one pass
+ * filters along x, then y, then z: F'[i] = F[i-1]/4 + F[i]/2 + F[i+1]/4. */
+int ora_smooth_binomial(const ora_grid* g, int npass, double* F)
+{
+    if (npass < 0) return -1;
+    size_t n = (size_t)g->nx * g->ny * g->nz;
+    double* T = (double*)malloc(n * sizeof(double));
+    if (!T) return -2;
+    for (int pass = 0; pass < npass; ++pass)
+        for (int d = 0; d < 3; ++d) {
+            for (long long k = 0; k < g->nz; ++k)
+                for (long long j = 0; j < g->ny; ++j)
+                    for (long long i = 0; i < g->nx; ++i) {
+                        size_t lo = gidx(g, i - (d == 0), j - (d == 1), k - (d == 2));
+                        size_t hi = gidx(g, i + (d == 0), j + (d == 1), k + (d == 2));
+                        T[gidx(g, i, j, k)] = 0.25 * F[lo] + 0.5 * F[gidx(g, i, j, k)] + 0.25 * F[hi];
+                    }
+            memcpy(F, T, n * sizeof(double));
+        }
+    free(T);
+    return 0;
+}
+
 /* Boris (1970), relativistic form:
  *  h = q dt/(2m); u- = u + h E; gamma- = sqrt(1+|u-|^2/c^2); t = h B/gamma-;
  *  s = 2t/(1+|t|^2); u' = u- + u- x t; u+ = u- + u' x s; u_new = u+ + h E. */

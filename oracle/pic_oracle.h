@@ -63,6 +63,22 @@ int ora_gather(const ora_grid* g, int order, long long np,
                double* Exp, double* Eyp, double* Ezp,
                double* Bxp, double* Byp, double* Bzp);
 
+/* NEXT-3.  S^0: top-hat on [-1/2, 1/2). */
+double ora_shape0(double r);
+
+/* Gather variants.  variant 0 = ora_gather (same order n everywhere).  variant 1 =
+ * "energy-conserving" (Galerkin) gather: order n-1 along every direction in which the component
+ * is staggered, order n along the others.  Returns 0, -1 on a bad order / variant. */
+int ora_gather_variant(const ora_grid* g, int order, int variant, long long np,
+                       const double* x, const double* y, const double* z,
+                       const double* Ex, const double* Ey, const double* Ez,
+                       const double* Bx, const double* By, const double* Bz,
+                       double* Exp, double* Eyp, double* Ezp,
+                       double* Bxp, double* Byp, double* Bzp);
+
+/* Binomial (1-2-1) smoothing of one component in place, periodic; one pass = x, then y, then z. */
+int ora_smooth_binomial(const ora_grid* g, int npass, double* F);
+
 /* Step 2: relativistic Boris push, u^{n-1/2} -> u^{n+1/2}, in place. */
 int ora_boris(long long np, double q, double m, double dt,
               double* ux, double* uy, double* uz,

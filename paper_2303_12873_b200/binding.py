@@ -23,7 +23,7 @@ _CODE_NAMES = {0: "PIC_OK", -1: "PIC_EINVAL", -2: "PIC_ENOMEM", -3: "PIC_ECUDA",
 SYMBOLS = ("pic_query_arena", "pic_init_grid", "pic_set_fields", "pic_load_particles", "pic_step",
            "pic_sort", "pic_get_fields", "pic_get_particles", "pic_deposit_rho", "pic_get_cell_offsets",
            "pic_get_counters", "pic_get_stage_ms", "pic_set_option", "pic_sync", "pic_last_error",
-           "pic_destroy", "pic_version", "pic_probe_dfma", "pic_probe_lds", "pic_probe_red")
+           "pic_destroy", "pic_version", "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
 
 
 class PicError(RuntimeError):
@@ -68,6 +68,7 @@ def load_library(path: str | None = None):
     L.pic_sync.argtypes = [vp]
     L.pic_destroy.argtypes = [vp]
     L.pic_probe_dfma.argtypes = [i, i, C.POINTER(d)]
+    L.pic_probe_dmma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
     L.pic_probe_red.argtypes = [i, ll, ll, i, C.POINTER(d)]
     for name in SYMBOLS:

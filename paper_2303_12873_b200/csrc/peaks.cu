@@ -37,6 +37,29 @@ __global__ void probe_dfma_kernel(int iters, long long* clk, double* sink) {
     if (threadIdx.x == 0) clk[blockIdx.x] = t1 - t0;
 }
 
+// ---- fp64 tensor path: DMMA m8n8k4 (256 FMA per warp instruction) ----------------------------------
+__global__ void probe_dmma_kernel(int iters, long long* clk, double* sink) {
+    double c[8][2];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { c[k][0] = 1e-9 * threadIdx.x; c[k][1] = 1e-9 * k; }
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-7;
+    __syncthreads();
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k)      // 8 independent accumulator fragments
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                         : "+d"(c[k][0]), "+d"(c[k][1]) : "d"(a), "d"(b));
+    }
+    const long long t1 = clock64();
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += c[k][0] + c[k][1];
+    if (s == 12345.678) sink[0] = s;
+    if (threadIdx.x == 0) clk[blockIdx.x] = t1 - t0;
+}
+
 // ---- shared-memory return path: LDS.64 / LDS.128 with a given lane -> word map -------------------
 // Every active lane of every warp reads word lane_word[lane] (+ a per-load offset that keeps the
 // bank pattern) of a shared array laid out like the tile kernel's stencil; eight independent loads
@@ -44,29 +67,37 @@ __global__ void probe_dfma_kernel(int iters, long long* clk, double* sink) {
 constexpr int PROBE_SMEM_WORDS = 6144;
 template <int VEC>
 __global__ void probe_lds_kernel(const int* __restrict__ lane_word, unsigned active, int plane_words, int iters,
-                                 long long* clk, double* sink) {
+                                 int zero, long long* clk, double* sink) {
     __shared__ __align__(16) double sm[PROBE_SMEM_WORDS];
     for (int i = threadIdx.x; i < PROBE_SMEM_WORDS; i += blockDim.x) sm[i] = 0.5 * i;
     __syncthreads();
     const int lane = threadIdx.x & 31;
     if (!((active >> lane) & 1u)) return;
-    const unsigned base = (unsigned)__cvta_generic_to_shared(sm + lane_word[lane]);
+    const double* base = sm + lane_word[lane];
     double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     const long long t0 = clock64();
 #pragma unroll 1
     for (int it = 0; it < iters; ++it) {
+        // `zero` is 0 at run time but opaque to the compiler: the addresses change with the trip as far as it
+        // can tell, so the eight loads are issued on every trip (with trip-invariant addresses the whole
+        // loop collapsed into one trip, volatile asm or not).
+        const double* a = base + it * zero;
+        double v[8], w[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {       // plain loads: ptxas may keep all eight in flight
+            if constexpr (VEC == 8) {
+                v[k] = a[k * plane_words];
+                w[k] = 0.0;
+            } else {
+                const double2 t = *reinterpret_cast<const double2*>(a + k * plane_words);
+                v[k] = t.x;
+                w[k] = t.y;
+            }
+        }
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            if constexpr (VEC == 8) {
-                double v;
-                asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(base + 8u * (unsigned)(k * plane_words)));
-                acc[k] = v;
-            } else {
-                double v, w;
-                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v), "=d"(w)
-                             : "r"(base + 8u * (unsigned)(k * plane_words)));
-                acc[k] = v + w;
-            }
+            acc[k] += v[k];
+            if constexpr (VEC == 16) acc[k] += w[k];
         }
     }
     const long long t1 = clock64();
@@ -153,6 +184,21 @@ int pic_probe_dfma(int warps_per_sm, int iters, double* clk_per_warp_instr) {
     return e == cudaSuccess ? PIC_OK : PIC_ECUDA;
 }
 
+int pic_probe_dmma(int warps_per_sm, int iters, double* clk_per_warp_instr) {
+    if (!clk_per_warp_instr || warps_per_sm < 1 || warps_per_sm > 32 || iters < 1) return PIC_EINVAL;
+    const int nsm = sm_count();
+    if (nsm <= 0) return PIC_ECUDA;
+    long long* clk = nullptr;
+    double* sink = nullptr;
+    if (cudaMalloc(&clk, sizeof(long long) * nsm) != cudaSuccess || cudaMalloc(&sink, 8) != cudaSuccess) return PIC_ENOMEM;
+    probe_dmma_kernel<<<nsm, 32 * warps_per_sm>>>(iters, clk, sink);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) *clk_per_warp_instr = median_clk(clk, nsm) / ((double)iters * 8.0 * warps_per_sm);
+    cudaFree(clk);
+    cudaFree(sink);
+    return e == cudaSuccess ? PIC_OK : PIC_ECUDA;
+}
+
 int pic_probe_lds(int vec_bytes, const int* lane_word, unsigned int active_mask, int plane_words, int warps_per_sm,
                   int iters, double* clk_per_warp_instr) {
     if (!clk_per_warp_instr || !lane_word || (vec_bytes != 8 && vec_bytes != 16) || !active_mask || warps_per_sm < 1 ||
@@ -172,8 +218,8 @@ int pic_probe_lds(int vec_bytes, const int* lane_word, unsigned int active_mask,
         cudaMalloc(&dw, 128) != cudaSuccess)
         return PIC_ENOMEM;
     cudaMemcpy(dw, lane_word, 128, cudaMemcpyHostToDevice);
-    if (vec_bytes == 8) probe_lds_kernel<8><<<nsm, 32 * warps_per_sm>>>(dw, active_mask, plane_words, iters, clk, sink);
-    else probe_lds_kernel<16><<<nsm, 32 * warps_per_sm>>>(dw, active_mask, plane_words, iters, clk, sink);
+    if (vec_bytes == 8) probe_lds_kernel<8><<<nsm, 32 * warps_per_sm>>>(dw, active_mask, plane_words, iters, 0, clk, sink);
+    else probe_lds_kernel<16><<<nsm, 32 * warps_per_sm>>>(dw, active_mask, plane_words, iters, 0, clk, sink);
     cudaError_t e = cudaDeviceSynchronize();
     if (e == cudaSuccess) *clk_per_warp_instr = median_clk(clk, nsm) / ((double)iters * 8.0 * warps_per_sm);
     cudaFree(clk);

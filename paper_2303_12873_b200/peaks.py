@@ -40,12 +40,60 @@ def lds_patterns(vec_bytes):
     return out
 
 
+def _cells(sizes):
+    """lane -> word map from a list of run lengths: run r reads the stencil word of cell r (distinct banks)."""
+    words = []
+    for r, n in enumerate(sizes):
+        words += [_word(1 + r % 8, r // 8, 1)] * n        # r < 8: even 8-byte banks, r >= 8: the odd ones
+    assert len(words) == 32
+    return words
+
+
+def rule_patterns():
+    """Lane patterns that tell apart the possible rules for when an LDS.64 is served in ONE wavefront
+    (all words used here sit in different 8-byte banks, so none of the patterns has a bank conflict)."""
+    return [
+        ("16 cells, 2 lanes each (pairs equal)", _cells([2] * 16)),
+        ("2 cells alternating by lane (l & 1)", [_word(1 + (l & 1), 0, 1) for l in range(32)]),
+        ("2 cells alternating by pair ((l >> 1) & 1)", [_word(1 + ((l >> 1) & 1), 0, 1) for l in range(32)]),
+        ("runs 6,6,4,6,6,4 (even boundaries, mixed quads)", _cells([6, 6, 4, 6, 6, 4])),
+        ("runs 2,4,4,4,2,2,4,4,4,2 (pairs equal, quads mixed)", _cells([2, 4, 4, 4, 2, 2, 4, 4, 4, 2])),
+        ("runs 7,25 (one odd boundary)", _cells([7, 25])),
+        ("runs 8,24", _cells([8, 24])),
+        ("runs 9,23", _cells([9, 23])),
+        ("runs 7,9,7,9 (odd boundaries inside both half-warps)", _cells([7, 9, 7, 9])),
+        ("runs of 3 (11 cells)", _cells([3] * 10 + [2])),
+        ("lane l reads word l % 16 (half-warps read the same 16 consecutive words)", [64 + (l % 16) for l in range(32)]),
+        ("lane l reads word l % 8", [64 + (l % 8) for l in range(32)]),
+        ("lane l reads word l // 2 (16 consecutive words, pairs equal)", [64 + l // 2 for l in range(32)]),
+        ("lane l reads word l // 4 (8 consecutive words)", [64 + l // 4 for l in range(32)]),
+        ("lanes l and l ^ 16 equal, 16 cells", [_word(1 + (l % 16) % 8, (l % 16) // 8, 1) for l in range(32)]),
+    ]
+
+
+def rule_table(warps=32):
+    rows = []
+    for k, (name, words) in enumerate(rule_patterns()):
+        clk = probe_lds(8, words, 0xFFFFFFFF, warps)
+        rows.append({"launch": k, "pattern": name, "distinct": len(set(words)), "clk_per_warp_instr_per_sm": clk})
+    return rows
+
+
 def probe_dfma(warps, iters=4000):
     L = load_library()
     out = C.c_double(0.0)
     rc = L.pic_probe_dfma(warps, iters, C.byref(out))
     if rc != PIC_OK:
         raise PicError(rc, "pic_probe_dfma")
+    return out.value
+
+
+def probe_dmma(warps, iters=2000):
+    L = load_library()
+    out = C.c_double(0.0)
+    rc = L.pic_probe_dmma(warps, iters, C.byref(out))
+    if rc != PIC_OK:
+        raise PicError(rc, "pic_probe_dmma")
     return out.value
 
 
@@ -74,7 +122,7 @@ RED_PATTERNS = ("32 consecutive doubles per warp (8 sectors)", "one 32-byte sect
                 "flush-like: 8 places x 4 planes", "8 places x 4 consecutive doubles")
 
 
-def lds_table(warps_list=(8, 16)):
+def lds_table(warps_list=(8, 16, 32)):
     rows = []
     k = 0
     for vec in (8, 16):
@@ -95,6 +143,11 @@ def main(argv=None):
     torch.cuda.set_device(0)
     torch.cuda.synchronize()
     res = {}
+    if "--rule" in argv:      # only the rule finder (one launch per row: for ncu)
+        print("| # | LDS.64 lane pattern (32 active lanes, 32 warps/SM) | distinct addr | clk per warp instr per SM |\n|---|---|---|---|")
+        for r in rule_table():
+            print("| %d | %s | %d | %.2f |" % (r["launch"], r["pattern"], r["distinct"], r["clk_per_warp_instr_per_sm"]))
+        return res
     if "--lds" not in argv:
         print("## DFMA (one block per SM, 8 independent chains per thread)\n")
         print("| warps/SM | clk per warp DFMA per SM | fp64 lanes/clk/SM |\n|---|---|---|")
@@ -103,6 +156,14 @@ def main(argv=None):
             clk = probe_dfma(w)
             res["dfma"].append({"warps_per_sm": w, "clk_per_warp_instr_per_sm": clk, "lanes_per_clk": 32.0 / clk})
             print("| %d | %.3f | %.1f |" % (w, clk, 32.0 / clk))
+    if "--lds" not in argv:
+        print("\n## DMMA m8n8k4 (256 FMA per warp instruction, 8 independent accumulator fragments per warp)\n")
+        print("| warps/SM | clk per warp DMMA per SM | fp64 FMA/clk/SM |\n|---|---|---|")
+        res["dmma"] = []
+        for w in (4, 8, 16):
+            clk = probe_dmma(w)
+            res["dmma"].append({"warps_per_sm": w, "clk_per_warp_instr_per_sm": clk, "fma_per_clk": 256.0 / clk})
+            print("| %d | %.3f | %.1f |" % (w, clk, 256.0 / clk))
     print("\n## Shared-memory loads, word(x,y,z) = y + %d z + %d x (fresh tile stencil)\n" % (SZ, SX))
     print("| # | op | lane pattern | distinct addr | active lanes | warps/SM | clk per warp instr per SM |"
           " lane bytes/clk/SM |\n|---|---|---|---|---|---|---|---|")
