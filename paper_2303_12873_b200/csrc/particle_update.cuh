@@ -10,27 +10,53 @@
 namespace pic {
 
 // ---------------------------------------------------------------- gather ----
-// One component: sum over the (N+1)^3 support, factored z(y(x)).
-template <int N>
+// One component: sum over the (NX+1)(NY+1)(NZ+1) support, factored z(y(x)).  The orders may differ per
+// direction (gather variant 1, below).
+template <int NX, int NY, int NZ>
 __device__ __forceinline__ double gather_comp(const double* __restrict__ F, const Grid& g, int fx, int fy, int fz,
-                                              const double (&wx)[N + 1], const double (&wy)[N + 1],
-                                              const double (&wz)[N + 1]) {
+                                              const double (&wx)[NX + 1], const double (&wy)[NY + 1],
+                                              const double (&wz)[NZ + 1]) {
     const double* base = F + g.idx(fx, fy, fz);
     double acc = 0.0;
 #pragma unroll
-    for (int c = 0; c <= N; ++c) {
+    for (int c = 0; c <= NZ; ++c) {
         double accy = 0.0;
 #pragma unroll
-        for (int b = 0; b <= N; ++b) {
+        for (int b = 0; b <= NY; ++b) {
             const double* row = base + b * g.sy + c * g.sz;
             double accx = 0.0;
 #pragma unroll
-            for (int a = 0; a <= N; ++a) accx = fma(wx[a], __ldg(row + a), accx);
+            for (int a = 0; a <= NX; ++a) accx = fma(wx[a], __ldg(row + a), accx);
             accy = fma(wy[b], accx, accy);
         }
         acc = fma(wz[c], accy, acc);
     }
     return acc;
+}
+
+// Gather variants (pic_set_option "gather_variant"):
+//   GV = 0  the same order N in every direction (reading R5)
+//   GV = 1  "energy-conserving" (Galerkin): order N - 1 along every direction in which the component is staggered
+template <int N, int GV>
+struct GatherOrders {
+    static constexpr int NS = GV ? N - 1 : N;      // order along a staggered direction
+};
+
+// All six components from the padded GLOBAL arrays.
+template <int N, int GV>
+__device__ __forceinline__ void gather6_global(const Grid& g, const Fields& f, double xi, double et, double ze,
+                                               double (&eb)[6]) {
+    constexpr int NS = GatherOrders<N, GV>::NS;
+    double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[NS + 1], wys[NS + 1], wzs[NS + 1];
+    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn), fzn = shape_weights<N>(ze, wzn);
+    const int fxs = shape_weights<NS>(xi - 0.5, wxs), fys = shape_weights<NS>(et - 0.5, wys),
+              fzs = shape_weights<NS>(ze - 0.5, wzs);
+    eb[0] = gather_comp<NS, N, N>(f.Ex, g, fxs, fyn, fzn, wxs, wyn, wzn);
+    eb[1] = gather_comp<N, NS, N>(f.Ey, g, fxn, fys, fzn, wxn, wys, wzn);
+    eb[2] = gather_comp<N, N, NS>(f.Ez, g, fxn, fyn, fzs, wxn, wyn, wzs);
+    eb[3] = gather_comp<N, NS, NS>(f.Bx, g, fxn, fys, fzs, wxn, wys, wzs);
+    eb[4] = gather_comp<NS, N, NS>(f.By, g, fxs, fyn, fzs, wxs, wyn, wzs);
+    eb[5] = gather_comp<NS, NS, N>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
 }
 
 // Esirkepov deposition of one particle through an adder:
@@ -131,7 +157,7 @@ __device__ __forceinline__ void deposit_global(const Grid& g, const Fields& f, d
 
 // Device function used by both particle paths: the whole update of one
 // particle against the GLOBAL field arrays.
-template <int N>
+template <int N, int GV>
 __device__ __forceinline__ void update_particle_global(const Grid& g, const Fields& f, const Particles& p,
                                                        long long ip, double q, double h, DevStatus* status) {
     const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
@@ -140,16 +166,9 @@ __device__ __forceinline__ void update_particle_global(const Grid& g, const Fiel
     // normalised coordinates: a subtraction then a multiplication (R30)
     const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy, ze = (z - g.zmin) * g.inv_dz;
     // step 1: gather
-    double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[N + 1], wys[N + 1], wzs[N + 1];
-    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn), fzn = shape_weights<N>(ze, wzn);
-    const int fxs = shape_weights<N>(xi - 0.5, wxs), fys = shape_weights<N>(et - 0.5, wys),
-              fzs = shape_weights<N>(ze - 0.5, wzs);
-    const double ex = gather_comp<N>(f.Ex, g, fxs, fyn, fzn, wxs, wyn, wzn);
-    const double ey = gather_comp<N>(f.Ey, g, fxn, fys, fzn, wxn, wys, wzn);
-    const double ez = gather_comp<N>(f.Ez, g, fxn, fyn, fzs, wxn, wyn, wzs);
-    const double bx = gather_comp<N>(f.Bx, g, fxn, fys, fzs, wxn, wys, wzs);
-    const double by = gather_comp<N>(f.By, g, fxs, fyn, fzs, wxs, wyn, wzs);
-    const double bz = gather_comp<N>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
+    double eb[6];
+    gather6_global<N, GV>(g, f, xi, et, ze, eb);
+    const double ex = eb[0], ey = eb[1], ez = eb[2], bx = eb[3], by = eb[4], bz = eb[5];
     // step 2: Boris
     const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
     boris_push(h, inv_c2, ux, uy, uz, ex, ey, ez, bx, by, bz);

@@ -1,25 +1,30 @@
 // particles_tile.cu -- fused gather + Boris push + Esirkepov deposition per
 // cell-sorted tile (BASELINE.json:north_star parts
-// 1-3, "fused per cell-sorted tile").  Kernel v5/v6 of DESIGN.md section 5.1;
-// measurements in profiles/r01_v4_tile_kernel.md and r01_v5_tile_kernel.md.
+// 1-3, "fused per cell-sorted tile").  Kernel v9 of DESIGN.md section 5.1;
+// measurements in profiles/r02_tile_kernel.md (v1-v8: profiles/r01_*).
 //
 // One thread block owns a tile of TX x TY x TZ cells; its E,B stencil (+ halo
 // for the shape support and DRIFT cells of drift since the last pic_sort) is
 // staged in shared memory once.  After that the block's warps run without any
-// block-wide barrier: a warp pulls x-rows of the tile (TX cells, contiguous in
-// the cell-sorted SoA arrays) from a shared counter and processes each row in
-// chunks of CHUNK = 72 particles (a row of 8 cells x 8 ppc is mostly one chunk):
-//   phase A  lane <-> particle, 32 at a time.  The particle data of a sub-chunk
-//            are copied into a per-warp landing buffer by cp.async one
-//            sub-chunk ahead (with a deferred sort pending: through perm[],
-//            and all eight arrays are then written, in sorted order, to the
-//            other buffer).
+// block-wide barrier.  A warp owns RPW consecutive x-rows of the tile; their
+// cells, in order, form the warp's STREAM: cell c occupies the stream positions
+// cp[c] .. cp[c] + n_c - 1, padded to an even length (so that the two lanes of
+// an aligned lane pair always work on particles of the same cell).
+//   phase A  lane <-> stream position, 32 consecutive positions at a time,
+//            ACROSS row boundaries (the lanes stay full: a row of 64 +- 8
+//            particles no longer ends in a nearly empty sub-chunk).  The
+//            particle data of a sub-chunk are copied into a per-warp landing
+//            buffer by cp.async one sub-chunk ahead (with a deferred sort
+//            pending: through perm[], read two sub-chunks ahead, and all eight
+//            arrays are then written, in sorted order, to the other buffer).
 //            Gather from the shared stencil, Boris, move, store of the wrapped
 //            state.  A particle that stayed inside its listed cell or crossed
 //            ONE of its faces ("fast") writes its old nodal shapes and shape
-//            differences on the cell's window plus q w / dt to a per-warp
-//            staging slot (26 doubles).
-//   phase B  lane <-> (cell q of the row, plane s of that cell's window).  The
+//            differences on the cell's window to slot (position mod RING) of a
+//            per-warp staging ring: 18 doubles (the last entry of each set
+//            follows from sum S = 1, sum DS = 0) + (q w / dt, e) + a code.
+//   phase B  runs as soon as a whole row is staged (or the ring is full):
+//            lane <-> (cell q of the row, plane s of that cell's window).  The
 //            four lanes of a cell walk the cell's staged particles and
 //            accumulate the Esirkepov window of the CELL in registers
 //            (3 x 12 accumulators per lane at order 3), so the per-particle
@@ -50,9 +55,12 @@ struct FastWin {
 // that has moved since its last pic_sort, 0 right after a sort (every particle is in its listed cell), which
 // shrinks the stencil from 14 x 10 x 10 to 12 x 8 x 8 nodes per component so that TWO blocks fit one SM
 // and one block's prologue (stencil staging: every warp of the block waits) overlaps the other's particles.
-template <int TX_, int TY_, int TZ_, int NW_, int MINB_, int DRIFT_, int CHUNK_>
+template <int TX_, int TY_, int TZ_, int NP_, int MINB_, int DRIFT_, int RING_, bool UG_>
 struct TileCfg {
-    static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NW = NW_, NT = 32 * NW_, MINB = MINB_, DRIFT = DRIFT_;
+    // NP producer warps (phase A) and NP consumer warps (phase B), paired one to one
+    static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NP = NP_, NW = 2 * NP_, NT = 32 * NW, MINB = MINB_,
+                         DRIFT = DRIFT_;
+    static constexpr bool UG = UG_;               // gather on cell-anchored windows (see gather6_cell)
     static constexpr int NROW = TY * TZ;
     // gather stencil: nodes i-2 .. i+2 of a particle in cell i (every order, every staggering)
     static constexpr int GL = 2 + DRIFT;
@@ -74,19 +82,28 @@ struct TileCfg {
         return k == 0 ? 0 : (k == 1 ? FP - SX : (k == 2 ? 2 * FP - 2 * SX : (k == 3 ? 3 * FP - 3 * SX
                       : (k == 4 ? 4 * FP - 3 * SX : 5 * FP - 3 * SX))));
     }
-    // per-warp staging: CHUNK skewed slots of PITCH doubles (PITCH/2 odd and the skew make the eight
-    // 16-byte words a phase-B warp load touches fall into eight different 16-byte bank groups), then the
-    // scratch record of the slow path and the landing buffer of the next sub-chunk's particle data (8 arrays x
-    // 32 lanes, filled by cp.async).  CHUNK = 72: a row of 8 cells x 8 ppc (64 +- 8 particles) is mostly ONE chunk.
-    static constexpr int CHUNK = CHUNK_, PITCH = 26, NSLOT = CHUNK + (CHUNK + 7) / 8, SLOW_W = 32, PBUF_W = 8 * 32;
-    static constexpr int STG_W = PITCH * NSLOT + SLOW_W + PBUF_W;
-    static_assert(CHUNK % 8 == 0 && STG_W % 2 == 0, "staging layout");
+    // a producer's stream: RPW rows of the tile, NC cells
+    static constexpr int RPW = NROW / NP, NC = RPW * TX;
+    static_assert(NROW % NP == 0 && NC <= 64, "rows are dealt statically; one lane scans two cells of the stream");
+    // per-pair staging ring of RING slots: a body of BODY doubles per slot (slot s at word BODY s + 2 (s >> 3): BODY / 2
+    // is odd and every eighth slot is pushed on by one 16-byte word, so that the eight 16-byte words a phase-B warp
+    // load touches -- slots about 8 apart -- fall into different 16-byte bank groups), a tail (q w / dt, e) and a
+    // code per slot; then the scratch record of the slow path, the landing buffer of the next sub-chunk's particle
+    // data (8 arrays x 32 lanes, filled by cp.async), the stream table cp[NC + 1] and the pair's two flags.
+    static constexpr int RING = RING_, BODY = 18, SLOW_W = 32, PBUF_W = 8 * 32;
+    static constexpr int BODY_W = BODY * RING + 2 * ((RING + 7) / 8), TAIL_W = 2 * RING, CODE_W = (RING + 1) / 2,
+                         TAB_W = (NC + 1 + 4 + 4) / 2 + ((NC + 1 + 4 + 4) / 2 & 1);
+    static constexpr int STG_W = BODY_W + TAIL_W + CODE_W + (CODE_W & 1) + SLOW_W + PBUF_W + TAB_W;
+    static_assert(STG_W % 2 == 0 && BODY_W % 2 == 0, "staging layout: 16-byte alignment");
     static constexpr int NOFF = NROW * (TX + 1);
-    static constexpr size_t SMEM = sizeof(double) * ((size_t)TOT + (size_t)NW * STG_W) + sizeof(int) * (NOFF + 4);
+    static constexpr size_t SMEM = sizeof(double) * ((size_t)TOT + (size_t)NP * STG_W) + sizeof(int) * (NOFF + 4);
     static_assert(TX == 8, "phase B maps 8 cells x 4 planes onto a warp");
 };
 
-__device__ __forceinline__ int skew(int slot) { return slot + (slot >> 3); }
+// word offset of ring slot s inside the body area
+template <class C>
+__device__ __forceinline__ int body_word(int s) { return C::BODY * s + 2 * (s >> 3); }
+
 
 // Old and new nodal shapes on the common window of N+2 slots anchored at
 // min(first old node, first new node); returns that node.  |move| < 1 cell.
@@ -163,31 +180,112 @@ __device__ __forceinline__ void place_new_window(const double (&w)[N + 1], int s
 template <class C>
 __device__ __forceinline__ int tile_word(int x, int y, int z) { return y + C::SZ * z + C::SX * x; }
 
+// ---- gather from the shared stencil on CELL-ANCHORED windows ---------------------------------------
+// The shared-memory return path serves a warp-wide LDS.64 in ONE wavefront instead of two when the two
+// lanes of every aligned lane pair read the same word and the warp reads at most 8 distinct words
+// (profiles/r02_lsu.md).  The stream gives the lanes of a pair particles of the same cell; for them to read
+// the same words, the window a particle gathers from must depend on its CELL only, not on where in the cell
+// it sits.  Per dimension the support of order N starts at one of two nodes for the particles of a cell
+// whenever floor() of the shape's argument can differ from the cell index (order 3 and 1: the staggered
+// windows; order 2: the nodal ones); the gather therefore runs over the union of the two, one node wider,
+// with the weights shifted into place and a zero at the unused end (a zero weight adds exactly 0, so the
+// result is bit-identical to the N+1-point sum).  At order 3 that is 540 loads per particle instead of
+// 384, at one wavefront each instead of 1.8.
+// Gather variant GV = 1 (order N - 1 along the staggered directions, particle_update.cuh): the staggered
+// windows are those of order NS = N - 1 (one node; three nodes with a shift; three nodes).
+template <int N, int GV>
+struct UWin {
+    static constexpr int NS = GatherOrders<N, GV>::NS;
+    static constexpr int WN = (N == 1) ? 2 : 4;            // nodal window: nodes AN .. AN + WN - 1 relative to the cell
+    static constexpr int AN = (N == 1) ? 0 : -1;
+    // staggered window (node m sits at m + 1/2): orders 1 and 3 anchor their support at floor(xi - 1/2), which is the
+    // cell index or one less: NS + 2 nodes; orders 0 and 2 at the cell index itself: NS + 1 nodes
+    static constexpr int WS = (NS == 0) ? 1 : ((NS == 2) ? 3 : NS + 2);
+    static constexpr int AS = (NS == 0) ? 0 : ((NS == 3) ? -2 : -1);
+    static constexpr int ZT = (WN > WS) ? WN : WS;         // trips of the rolled z loop
+};
+
+// N+1 weights whose first node sits `shift` (0 or 1) slots into a window of W >= N+1 slots, padded to P >= W entries
+template <int N, int W, int P>
+__device__ __forceinline__ void place_uniform(const double (&w)[N + 1], int shift, double (&u)[P]) {
+#pragma unroll
+    for (int a = 0; a < P; ++a) {
+        const double v0 = (a <= N) ? w[(a <= N) ? a : 0] : 0.0;
+        if constexpr (W == N + 1) {
+            u[a] = v0;
+        } else {
+            const double v1 = (a >= 1 && a <= N + 1) ? w[(a >= 1 && a <= N + 1) ? a - 1 : 0] : 0.0;
+            u[a] = shift ? v1 : v0;
+        }
+    }
+}
+
 // One z-plane of one component from the shared stencil: sum_b wy[b] sum_a wx[a] F[a,b].
-template <int N, class C>
-__device__ __forceinline__ double gather_plane(const double* __restrict__ base, const double (&wx)[N + 1],
-                                               const double (&wy)[N + 1]) {
+template <int WX, int WY, int PX, int PY, class C>
+__device__ __forceinline__ double gather_plane(const double* __restrict__ base, const double (&wx)[PX],
+                                               const double (&wy)[PY]) {
     double accy = 0.0;
 #pragma unroll
-    for (int b = 0; b <= N; ++b) {
+    for (int b = 0; b < WY; ++b) {
         double accx = 0.0;
 #pragma unroll
-        for (int a = 0; a <= N; ++a) accx = fma(wx[a], base[b + C::SX * a], accx);
+        for (int a = 0; a < WX; ++a) accx = fma(wx[a], base[b + C::SX * a], accx);
         accy = fma(wy[b], accx, accy);
     }
     return accy;
 }
 
-// All six components from the shared stencil.  (g*n) / (f*s) = tile slot of the first nodal /
-// staggered node per dimension.  The z loop is kept ROLLED (the z weights rotate through their
-// register arrays and are back in place after N+1 trips): the body is ~250 instructions that stay in
-// the L0 instruction cache instead of ~1000 straight-line ones.
-template <int N, class C>
-__device__ __forceinline__ void gather6_tile(const double* __restrict__ Et, int gxn, int gyn, int gzn, int fxs,
-                                             int fys, int fzs, const double (&wxn)[N + 1],
-                                             const double (&wyn)[N + 1], double (&wzn)[N + 1],
-                                             const double (&wxs)[N + 1], const double (&wys)[N + 1],
-                                             double (&wzs)[N + 1], double (&eb)[6]) {
+// All six components.  (un*) / (us*) = tile slot of the first node of the cell's nodal / staggered window per
+// dimension; wxn .. wzs = the particle's weights placed on those windows.  The z loop is kept ROLLED (the z
+// weights rotate through their register arrays, both padded to ZT entries, and are back in place after ZT
+// trips): the body stays a few hundred instructions instead of a few thousand straight-line ones.
+template <int N, int GV, class C>
+__device__ __forceinline__ void gather6_cell(const double* __restrict__ Et, int unx, int uny, int unz, int usx,
+                                             int usy, int usz, const double (&wxn)[UWin<N, GV>::WN],
+                                             const double (&wyn)[UWin<N, GV>::WN], double (&wzn)[UWin<N, GV>::ZT],
+                                             const double (&wxs)[UWin<N, GV>::WS], const double (&wys)[UWin<N, GV>::WS],
+                                             double (&wzs)[UWin<N, GV>::ZT], double (&eb)[6]) {
+    using U = UWin<N, GV>;
+    constexpr int WN = U::WN, WS = U::WS, ZT = U::ZT;
+    const int o_ex = C::comp_base(0) + tile_word<C>(usx, uny, unz);
+    const int o_ey = C::comp_base(1) + tile_word<C>(unx, usy, unz);
+    const int o_ez = C::comp_base(2) + tile_word<C>(unx, uny, usz);
+    const int o_bx = C::comp_base(3) + tile_word<C>(unx, usy, usz);
+    const int o_by = C::comp_base(4) + tile_word<C>(usx, uny, usz);
+    const int o_bz = C::comp_base(5) + tile_word<C>(usx, usy, unz);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) eb[k] = 0.0;
+    const double* pl = Et;
+#pragma unroll 1
+    for (int c = 0; c < ZT; ++c, pl += C::SZ) {
+        const double zn = wzn[0], zs = wzs[0];
+        if (WN == ZT || c < WN) {      // components that are nodal in z
+            eb[0] = fma(zn, gather_plane<WS, WN, WS, WN, C>(pl + o_ex, wxs, wyn), eb[0]);
+            eb[1] = fma(zn, gather_plane<WN, WS, WN, WS, C>(pl + o_ey, wxn, wys), eb[1]);
+            eb[5] = fma(zn, gather_plane<WS, WS, WS, WS, C>(pl + o_bz, wxs, wys), eb[5]);
+        }
+        if (WS == ZT || c < WS) {      // components that are staggered in z
+            eb[2] = fma(zs, gather_plane<WN, WN, WN, WN, C>(pl + o_ez, wxn, wyn), eb[2]);
+            eb[3] = fma(zs, gather_plane<WN, WS, WN, WS, C>(pl + o_bx, wxn, wys), eb[3]);
+            eb[4] = fma(zs, gather_plane<WS, WN, WS, WN, C>(pl + o_by, wxs, wyn), eb[4]);
+        }
+#pragma unroll
+        for (int k = 0; k < ZT - 1; ++k) { wzn[k] = wzn[k + 1]; wzs[k] = wzs[k + 1]; }
+        wzn[ZT - 1] = zn;
+        wzs[ZT - 1] = zs;
+    }
+}
+
+// The same gather on the particle's OWN windows (N + 1 nodes, NS + 1 along staggered directions; C::UG = false):
+// 384 loads at order 3, at 1.8 wavefronts each.  (g*n) / (f*s) = tile slot of the first nodal / staggered node per
+// dimension.  The z weights rotate through arrays padded to ZT = N + 1 entries.
+template <int N, int GV, class C>
+__device__ __forceinline__ void gather6_part(const double* __restrict__ Et, int gxn, int gyn, int gzn, int fxs,
+                                             int fys, int fzs, const double (&wxn)[N + 1], const double (&wyn)[N + 1],
+                                             double (&wzn)[N + 1], const double (&wxs)[GatherOrders<N, GV>::NS + 1],
+                                             const double (&wys)[GatherOrders<N, GV>::NS + 1], double (&wzs)[N + 1],
+                                             double (&eb)[6]) {
+    constexpr int WN = N + 1, WS = GatherOrders<N, GV>::NS + 1;
     const int o_ex = C::comp_base(0) + tile_word<C>(fxs, gyn, gzn);
     const int o_ey = C::comp_base(1) + tile_word<C>(gxn, fys, gzn);
     const int o_ez = C::comp_base(2) + tile_word<C>(gxn, gyn, fzs);
@@ -198,14 +296,16 @@ __device__ __forceinline__ void gather6_tile(const double* __restrict__ Et, int 
     for (int k = 0; k < 6; ++k) eb[k] = 0.0;
     const double* pl = Et;
 #pragma unroll 1
-    for (int c = 0; c <= N; ++c, pl += C::SZ) {
+    for (int c = 0; c < WN; ++c, pl += C::SZ) {
         const double zn = wzn[0], zs = wzs[0];
-        eb[0] = fma(zn, gather_plane<N, C>(pl + o_ex, wxs, wyn), eb[0]);
-        eb[1] = fma(zn, gather_plane<N, C>(pl + o_ey, wxn, wys), eb[1]);
-        eb[2] = fma(zs, gather_plane<N, C>(pl + o_ez, wxn, wyn), eb[2]);
-        eb[3] = fma(zs, gather_plane<N, C>(pl + o_bx, wxn, wys), eb[3]);
-        eb[4] = fma(zs, gather_plane<N, C>(pl + o_by, wxs, wyn), eb[4]);
-        eb[5] = fma(zn, gather_plane<N, C>(pl + o_bz, wxs, wys), eb[5]);
+        eb[0] = fma(zn, gather_plane<WS, WN, WS, WN, C>(pl + o_ex, wxs, wyn), eb[0]);
+        eb[1] = fma(zn, gather_plane<WN, WS, WN, WS, C>(pl + o_ey, wxn, wys), eb[1]);
+        eb[5] = fma(zn, gather_plane<WS, WS, WS, WS, C>(pl + o_bz, wxs, wys), eb[5]);
+        if (WS == WN || c < WS) {
+            eb[2] = fma(zs, gather_plane<WN, WN, WN, WN, C>(pl + o_ez, wxn, wyn), eb[2]);
+            eb[3] = fma(zs, gather_plane<WN, WS, WN, WS, C>(pl + o_bx, wxn, wys), eb[3]);
+            eb[4] = fma(zs, gather_plane<WS, WN, WS, WN, C>(pl + o_by, wxs, wyn), eb[4]);
+        }
 #pragma unroll
         for (int k = 0; k < N; ++k) { wzn[k] = wzn[k + 1]; wzs[k] = wzs[k + 1]; }
         wzn[N] = zn;
@@ -214,19 +314,10 @@ __device__ __forceinline__ void gather6_tile(const double* __restrict__ Et, int 
 }
 
 // Gather of all six components from the padded GLOBAL arrays (particle outside the tile's halo).
-template <int N>
+template <int N, int GV>
 __device__ __noinline__ void gather_global6(const Grid& g, const Fields& f, double xi, double et, double ze,
                                             double (&eb)[6]) {
-    double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[N + 1], wys[N + 1], wzs[N + 1];
-    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn), fzn = shape_weights<N>(ze, wzn);
-    const int fxs = shape_weights<N>(xi - 0.5, wxs), fys = shape_weights<N>(et - 0.5, wys),
-              fzs = shape_weights<N>(ze - 0.5, wzs);
-    eb[0] = gather_comp<N>(f.Ex, g, fxs, fyn, fzn, wxs, wyn, wzn);
-    eb[1] = gather_comp<N>(f.Ey, g, fxn, fys, fzn, wxn, wys, wzn);
-    eb[2] = gather_comp<N>(f.Ez, g, fxn, fyn, fzs, wxn, wyn, wzs);
-    eb[3] = gather_comp<N>(f.Bx, g, fxn, fys, fzs, wxn, wys, wzs);
-    eb[4] = gather_comp<N>(f.By, g, fxs, fyn, fzs, wxs, wyn, wzs);
-    eb[5] = gather_comp<N>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
+    gather6_global<N, GV>(g, f, xi, et, ze, eb);
 }
 
 // tile-relative cell index with the periodic image nearest to the tile
@@ -242,17 +333,12 @@ __device__ __forceinline__ int rel_cell(int i, int t0, int T, int n) {
 
 namespace {
 
-constexpr int FLAG = 25;           // last double of every staging slot: record kind
-constexpr int RCQ = 24;            // fast record: -q w / dt (shares a 16-byte word with the flag)
-constexpr double REC_FAST = 0.0;   // fast record (FastRec layout): old and new cell identical
+constexpr int REC_FAST = 0;   // fast record (FastRec layout): old and new cell identical
 // 1 .. 6: fast record of a particle that crossed ONE cell face: 1 + 2 d + (1 if towards +d).  The part of
-// its Esirkepov window inside the cell's window is in the record; the one node layer outside it (S0 = 0,
-// DS = e there) is described by (e, prefix factor on the outer edge) in the chunk's extras area.
-constexpr double REC_SLOW = 8.0;   // slow particle: the slot holds xi0 eta0 zeta0 xi1 eta1 zeta1 qw; deposited by the whole warp
-constexpr double REC_NONE = 7.0;   // nothing to deposit (q = 0, or the particle raised PIC_EPHYS)
-
-// extras of staging slot p (unskewed index): two doubles in the gap slot the skew leaves after every 8 slots
-__device__ __forceinline__ int ext_word(int p, int pitch) { return (9 * (p >> 3) + 8) * pitch + 2 * (p & 7); }
+// its Esirkepov window inside the cell's window is in the record; the one node layer outside it carries
+// S0 = 0, DS = e (the new weight that left the window; tail.y of the slot).
+constexpr int REC_NONE = 7;   // nothing to deposit (q = 0, or the particle raised PIC_EPHYS)
+constexpr int REC_SLOW = 8;   // slow particle: the slot holds xi0 eta0 zeta0 xi1 eta1 zeta1 qw; deposited by the whole warp
 
 // fp64 add to GLOBAL memory without a return value: REDG.E.ADD.F64 (fire-and-forget).  atomicAdd on a
 // pointer whose address space the compiler cannot prove emits a generic ATOM with a returned value
@@ -358,15 +444,17 @@ __device__ __forceinline__ void slow_deposit(const double* rec, const Grid& g, c
 }
 
 // ---- fast path: per-(cell, plane) register accumulators --------------------------------------
-// Staging slot layout (FW = window nodes): s0x dsx s0y dsy s0z dsz (FW each), then at RCQ the factor
-// -q w / dt and at FLAG the record code.  The prefix-summed current factors
+// Staging slot body (FW = window nodes): for d = x, y, z the first FW - 1 entries of S0_d, then of DS_d; the last
+// entry of each set follows from sum_a S0[a] = 1 and sum_a DS[a] = -e_d (e_d = the new weight of a face crosser
+// that left the window in dimension d, else 0).  The tail holds -q w / dt and e.  The prefix-summed current factors
 // pd_d[a] = cq_d * sum_{a' <= a} ds_d[a'] are rebuilt by the phase-B lanes (18 fp64 operations) instead of
 // being staged (9 more doubles per particle through the shared-memory pipe, which is what binds the kernel).
 template <int N>
 struct FastRec {
-    static constexpr int FW = FastWin<N>::FW;
-    static constexpr int S0X = 0, DSX = FW, S0Y = 2 * FW, DSY = 3 * FW, S0Z = 4 * FW, DSZ = 5 * FW, LEN = 6 * FW;
-    static_assert(LEN <= RCQ, "fast record overlaps its tail");
+    static constexpr int FW = FastWin<N>::FW, M = FW - 1;
+    static constexpr int LEN = 6 * M;
+    __host__ __device__ static constexpr int s0(int d, int a) { return 2 * M * d + a; }
+    __host__ __device__ static constexpr int ds(int d, int a) { return 2 * M * d + M + a; }
 };
 
 template <int K>
@@ -391,36 +479,43 @@ struct CellAcc {
             for (int a = 0; a < FW - 1; ++a) { jx[b][a] = 0.0; jy[a][b] = 0.0; jz[a][b] = 0.0; }
     }
     // one staged particle; s = this lane's plane.  Returns false for a record that is not fast.
-    // ext = the slot's extras (e, outer prefix factor), read only for a face crosser; jx0, jy0, jz0 =
-    // global J pointers at the first node of this cell's window (for the crosser's overflow layer).
-    __device__ __forceinline__ bool add(const double* __restrict__ r, int s, const double* __restrict__ ext,
+    // r = the slot's body, tail = (-q w / dt, e), code = the slot's code; jx0, jy0, jz0 = global J pointers at
+    // the first node of this cell's window (for the crosser's overflow layer).
+    __device__ __forceinline__ bool add(const double* __restrict__ r, double2 tail, int code, int s,
                                         double* jx0, double* jy0, double* jz0, long long sy, long long sz,
                                         double area_x, double area_y, double area_z) {
         using R = FastRec<N>;
         const double third = 1.0 / 3.0;
-        const double2 tail = ld2(r, RCQ);                     // -q w / dt, code
-        if (tail.y >= REC_NONE) return false;
-        const double code = tail.y;
-        double s0x[FW], dsx[FW], s0y[FW], dsy[FW], dsz[FW], pdx[FW - 1], pdy[FW - 1], pdz[FW - 1];
+        if (code >= REC_NONE) return false;
+        double raw[R::LEN];
 #pragma unroll
-        for (int a = 0; a < FW; a += 2) {
-            double2 v;
-            v = ld2(r, R::S0X + a); s0x[a] = v.x; s0x[a + 1] = v.y;
-            v = ld2(r, R::DSX + a); dsx[a] = v.x; dsx[a + 1] = v.y;
-            v = ld2(r, R::S0Y + a); s0y[a] = v.x; s0y[a + 1] = v.y;
-            v = ld2(r, R::DSY + a); dsy[a] = v.x; dsy[a + 1] = v.y;
-            v = ld2(r, R::DSZ + a); dsz[a] = v.x; dsz[a + 1] = v.y;
+        for (int k = 0; k < R::LEN; k += 2) {
+            const double2 v = ld2(r, k);
+            raw[k] = v.x; raw[k + 1] = v.y;
         }
-        const double s0z = r[R::S0Z + s];
         // a face crosser's prefix starts with the weight that fell below the window in the crossed dimension
-        double e = 0.0, pd_ov = 0.0, e0x = 0.0, e0y = 0.0, e0z = 0.0;
-        if (code != REC_FAST) {
-            const double2 x = ld2(ext, 0);
-            e = x.x; pd_ov = x.y;
-            e0x = (code == 1.0) ? e : 0.0;
-            e0y = (code == 3.0) ? e : 0.0;
-            e0z = (code == 5.0) ? e : 0.0;
+        const double e = tail.y;
+        const double ex = (code == 1 || code == 2) ? e : 0.0, ey = (code == 3 || code == 4) ? e : 0.0,
+                     ez = (code == 5 || code == 6) ? e : 0.0;
+        const double e0x = (code == 1) ? e : 0.0, e0y = (code == 3) ? e : 0.0, e0z = (code == 5) ? e : 0.0;
+        double s0x[FW], dsx[FW], s0y[FW], dsy[FW], s0zz[FW], dsz[FW], pdx[FW - 1], pdy[FW - 1], pdz[FW - 1];
+        {
+            double tx0 = 1.0, tx1 = -ex, ty0 = 1.0, ty1 = -ey, tz0 = 1.0, tz1 = -ez;
+#pragma unroll
+            for (int a = 0; a < FW - 1; ++a) {
+                s0x[a] = raw[R::s0(0, a)]; dsx[a] = raw[R::ds(0, a)];
+                s0y[a] = raw[R::s0(1, a)]; dsy[a] = raw[R::ds(1, a)];
+                s0zz[a] = raw[R::s0(2, a)]; dsz[a] = raw[R::ds(2, a)];
+                tx0 -= s0x[a]; tx1 -= dsx[a]; ty0 -= s0y[a]; ty1 -= dsy[a]; tz0 -= s0zz[a]; tz1 -= dsz[a];
+            }
+            s0x[FW - 1] = tx0; dsx[FW - 1] = tx1; s0y[FW - 1] = ty0; dsy[FW - 1] = ty1;
+            s0zz[FW - 1] = tz0; dsz[FW - 1] = tz1;
         }
+        const double s0z = pick<FW>(s0zz, s);
+        // outer prefix factor of a face crosser: the prefix over every node below the outer layer is e (towards -d:
+        // the layer comes first) or -e (towards +d: all DS sum to zero and the layer's own DS is e)
+        const double pd_ov = ((code & 1) ? e : -e) * tail.x *
+                             ((code <= 2) ? area_x : ((code <= 4) ? area_y : area_z));
         {
             const double cqx = tail.x * area_x, cqy = tail.x * area_y, cqz = tail.x * area_z;
             double rx = e0x, ry = e0y, rz = e0z;
@@ -430,9 +525,9 @@ struct CellAcc {
                 pdx[a] = cqx * rx; pdy[a] = cqy * ry; pdz[a] = cqz * rz;
             }
         }
-        const double dsz_s = r[R::DSZ + s];
+        const double dsz_s = pick<FW>(dsz, s);
         const double az = s0z + 0.5 * dsz_s, bz = 0.5 * s0z + third * dsz_s;
-        const double s0ys = r[R::S0Y + s], dsys = r[R::DSY + s];
+        const double s0ys = pick<FW>(s0y, s), dsys = pick<FW>(dsy, s);
         const double ay = s0ys + 0.5 * dsys, by = 0.5 * s0ys + third * dsys;
         double tx[FW], ty[FW], tz[FW];   // cross-section factors of Jx (per b), Jy (per a), Jz (per a)
 #pragma unroll
@@ -455,7 +550,7 @@ struct CellAcc {
         }
         if (code != REC_FAST) {
             // ---- face crosser: the node layer just outside the window (S0 = 0, DS = e) ----------------
-            const int k = (int)code - 1, d = k >> 1, hi = k & 1;
+            const int k = code - 1, d = k >> 1, hi = k & 1;
             const long long node = hi ? FW : -1;          // node slot of the layer
             const long long edge = hi ? FW - 1 : -1;      // edge slot between the layer and the window
             const double he = 0.5 * e, te = third * e;
@@ -551,18 +646,319 @@ struct CellAcc {
 
 namespace {
 
+// ---- flags of a producer / consumer pair (shared memory, block scope) ---------------------------------
+__device__ __forceinline__ int ld_acquire(const int* p) {
+    int v;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"((unsigned)__cvta_generic_to_shared(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(int* p, int v) {
+    asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+}
+
+// position t of a producer's stream -> (cell c of the stream, sorted index ip of the particle, or ip = -1 for a pad
+// position / the end of the stream).  cp[c] = first position of cell c (cp[NC] = length of the stream),
+// off = the block's table of sorted indices at every cell boundary of every row.
+template <class C>
+__device__ __forceinline__ void stream_lookup(int t, const int* __restrict__ cp, const int* __restrict__ off_all,
+                                              int row_first, int& c, int& ip) {
+    int r = 0;
+#pragma unroll
+    for (int k = 1; k < C::RPW; ++k) r += (t >= cp[C::TX * k]);
+    const int4 a = *reinterpret_cast<const int4*>(cp + C::TX * r), b = *reinterpret_cast<const int4*>(cp + C::TX * r + 4);
+    const int q = (t >= a.y) + (t >= a.z) + (t >= a.w) + (t >= b.x) + (t >= b.y) + (t >= b.z) + (t >= b.w);
+    c = C::TX * r + q;
+    const int* off = off_all + (row_first + r) * (C::TX + 1) + q;
+    const int lo = off[0], n = off[1] - lo, k = t - cp[c];
+    ip = (t < cp[C::NC] && k < n) ? lo + k : -1;
+}
+
+// per-pair staging area
+template <class C>
+struct Staging {
+    double* body;     // ring of record bodies
+    double* tails;    // RING x (-q w / dt, e)
+    int* codes;       // RING record codes
+    double* scr;      // slow-path scratch record
+    double* pbuf;     // landing buffer: [x y z ux uy uz w id][lane]
+    int* cp;          // cp[NC + 1], 16-byte aligned
+    int* flags;       // [0] = stream position up to which records are staged, [1] = ... consumed
+    __device__ __forceinline__ explicit Staging(double* stg) {
+        body = stg;
+        tails = stg + C::BODY_W;
+        codes = reinterpret_cast<int*>(tails + C::TAIL_W);
+        scr = tails + C::TAIL_W + C::CODE_W + (C::CODE_W & 1);
+        pbuf = scr + C::SLOW_W;
+        cp = reinterpret_cast<int*>(pbuf + C::PBUF_W);
+        flags = cp + ((C::NC + 1 + 3) & ~3);
+    }
+};
+
+// ---- consumer warp: phase B and the flush of every row of its producer's stream -------------------------
 template <int N, class C>
+__device__ __forceinline__ void tile_consumer(const Grid& g, const Fields& f, const Staging<C>& S, const int* row_off,
+                                              int row_first, int t0x, int t0y, int t0z, int lane) {
+    constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA;
+    const int* cp = S.cp;
+    const int T = cp[C::NC];
+    const double area_x = g.inv_dy * g.inv_dz, area_y = g.inv_dx * g.inv_dz, area_z = g.inv_dx * g.inv_dy;
+    const int bq = lane >> 2, bs = lane & 3;     // cell of the row, plane of the window
+    int b_lo = 0;                                // stream position up to which records have been consumed
+    CellAcc<N> acc;
+    acc.clear();
+#pragma unroll 1
+    for (int row_cur = 0; row_cur < C::RPW; ++row_cur) {
+        const int row_lo = cp[C::TX * row_cur], row_end = cp[C::TX * (row_cur + 1)];
+        if (row_end == row_lo) continue;         // empty row: nothing staged, nothing to flush
+        const int row_t = row_first + row_cur;
+        const long long win0 = g.idx(t0x + bq + FA, t0y + row_t % C::TY + FA, t0z + row_t / C::TY + FA);
+        const int cs = cp[C::TX * row_cur + bq];
+        const int ce = cs + (row_off[row_t * (C::TX + 1) + bq + 1] - row_off[row_t * (C::TX + 1) + bq]);
+#pragma unroll 1
+        for (;;) {
+            // wait until the whole row is staged, or the producer has run out of ring space
+            int staged;
+            for (;;) {
+                staged = ld_acquire(S.flags);
+                if (staged >= row_end || (staged + 32 - b_lo > C::RING && staged < T)) break;
+                __nanosleep(64);
+            }
+            const bool full_row = staged >= row_end;
+            const int b_hi = full_row ? row_end : staged;
+            {
+                const int lo = max(cs, b_lo), hi = min(ce, b_hi);
+                const int len = (bs < FW) ? hi - lo : 0;
+                const int maxlen = __reduce_max_sync(0xffffffffu, max(len, 0));
+                int sl = lo % C::RING;
+#pragma unroll 1
+                for (int t = 0; t < maxlen; ++t)
+                    if (t < len) {
+                        acc.add(S.body + body_word<C>(sl), ld2(S.tails, 2 * sl), S.codes[sl], bs, f.Jx + win0,
+                                f.Jy + win0, f.Jz + win0, g.sy, g.sz, area_x, area_y, area_z);
+                        sl = (sl + 1 == C::RING) ? 0 : sl + 1;
+                    }
+            }
+            __syncwarp();
+            b_lo = b_hi;
+            if (lane == 0) st_release(S.flags + 1, b_lo);      // the slots below b_lo may be reused
+            if (full_row) break;
+        }
+        acc.flush(g, f, win0, bs, lane);
+        acc.clear();
+    }
+}
+
+// ---- producer warp: phase A over its stream ------------------------------------------------------------
+template <int N, int GV, class C>
+__device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, const Particles& p, const Particles& po,
+                                              const unsigned int* __restrict__ perm, unsigned int* __restrict__ key_out,
+                                              double q, double h, const double* __restrict__ Et, const Staging<C>& S,
+                                              const int* row_off, int row_first, int t0x, int t0y, int t0z, int lane,
+                                              DevStatus* status) {
+    constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA, DRIFT = C::DRIFT;
+    using FR = FastRec<N>;
+    const int* cp = S.cp;
+    double* pbuf = S.pbuf;
+    const int T = cp[C::NC];
+    if (T == 0) return;
+    const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
+    const double inv_dt = 1.0 / g.dt;
+    unsigned int n_fast = 0, n_slow = 0, n_glob = 0;
+    bool bad_any = false;
+
+    // ---- software pipeline over the sub-chunks: lookup and perm[] two ahead, particle data one ahead --------
+    int c0, ip0, c1, ip1, is1 = 0;
+    stream_lookup<C>(lane, cp, row_off, row_first, c0, ip0);
+    if (ip0 >= 0) {
+        const int is = (perm != nullptr) ? (int)perm[ip0] : ip0;
+        cp_async8(pbuf + 0 * 32 + lane, p.x + is); cp_async8(pbuf + 1 * 32 + lane, p.y + is);
+        cp_async8(pbuf + 2 * 32 + lane, p.z + is); cp_async8(pbuf + 3 * 32 + lane, p.ux + is);
+        cp_async8(pbuf + 4 * 32 + lane, p.uy + is); cp_async8(pbuf + 5 * 32 + lane, p.uz + is);
+        cp_async8(pbuf + 6 * 32 + lane, p.w + is);
+        if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + is);
+    }
+    cp_async_commit();
+    stream_lookup<C>(32 + lane, cp, row_off, row_first, c1, ip1);
+    if (ip1 >= 0) is1 = (perm != nullptr) ? ld_u32_now(perm + ip1) : ip1;
+
+#pragma unroll 1
+    for (int t0 = 0; t0 < T; t0 += 32) {
+        cp_async_wait_all();
+        __syncwarp();
+        const double x = pbuf[0 * 32 + lane], y = pbuf[1 * 32 + lane], z = pbuf[2 * 32 + lane];
+        double ux = pbuf[3 * 32 + lane], uy = pbuf[4 * 32 + lane], uz = pbuf[5 * 32 + lane];
+        const double wgt = pbuf[6 * 32 + lane], idv = pbuf[7 * 32 + lane];
+        __syncwarp();       // every lane has read: the buffer may be refilled
+        // ---- the next sub-chunk's particle data start their way to the landing buffer NOW, so that they
+        // have this whole sub-chunk to arrive; the lookup (and perm[]) of the one after it goes into registers
+        if (ip1 >= 0) {
+            cp_async8(pbuf + 0 * 32 + lane, p.x + is1); cp_async8(pbuf + 1 * 32 + lane, p.y + is1);
+            cp_async8(pbuf + 2 * 32 + lane, p.z + is1); cp_async8(pbuf + 3 * 32 + lane, p.ux + is1);
+            cp_async8(pbuf + 4 * 32 + lane, p.uy + is1); cp_async8(pbuf + 5 * 32 + lane, p.uz + is1);
+            cp_async8(pbuf + 6 * 32 + lane, p.w + is1);
+            if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + is1);
+        }
+        cp_async_commit();
+        int c2, ip2, is2 = 0;
+        stream_lookup<C>(t0 + 64 + lane, cp, row_off, row_first, c2, ip2);
+        if (ip2 >= 0) is2 = (perm != nullptr) ? ld_u32_now(perm + ip2) : ip2;
+
+        // ---- everything of this sub-chunk that does not touch the ring: gather, push, move, store ----
+        const int ip = ip0;
+        const int slot = (t0 + lane) % C::RING;
+        bool is_slow = false, fast = false;
+        double xi = 0.0, et = 0.0, ze = 0.0, xi1 = 0.0, et1 = 0.0, ze1 = 0.0, qw = 0.0;
+        double wxn[N + 1], wyn[N + 1], wzn[N + 1];
+        int ci = 0, cj = 0, ck = 0, fxn = 0, fyn = 0, fzn = 0;
+        if (ip >= 0) {
+            const int row_t = row_first + c0 / C::TX;                 // the listed cell: tile row, x position
+            const int ry0 = row_t % C::TY, rz0 = row_t / C::TY, rx0 = c0 % C::TX;
+            qw = q * wgt;
+            if (perm != nullptr) {          // deferred sort: the other buffer gets every array, in sorted order
+                po.w[ip] = wgt;
+                po.id[ip] = (unsigned long long)__double_as_longlong(idv);
+            }
+            xi = (x - g.xmin) * g.inv_dx; et = (y - g.ymin) * g.inv_dy; ze = (z - g.zmin) * g.inv_dz;
+            ci = __double2int_rd(xi); cj = __double2int_rd(et); ck = __double2int_rd(ze);
+            const int rx = rel_cell<DRIFT>(ci, t0x, C::TX, g.nx), ry = rel_cell<DRIFT>(cj, t0y, C::TY, g.ny),
+                      rz = rel_cell<DRIFT>(ck, t0z, C::TZ, g.nz);
+            const bool in_tile = rx >= -DRIFT && rx <= C::TX - 1 + DRIFT && t0x + rx <= g.nx - 1 + DRIFT &&
+                                 ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
+                                 rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
+            fxn = shape_weights<N>(xi, wxn); fyn = shape_weights<N>(et, wyn); fzn = shape_weights<N>(ze, wzn);
+            double eb[6];
+            if (in_tile) {
+                constexpr int NS = GatherOrders<N, GV>::NS;
+                // from global node index to tile slot: slot = node - (t0 - GL) + image shift
+                const int shx = (rx - (ci - t0x)) + C::GL - t0x, shy = (ry - (cj - t0y)) + C::GL - t0y,
+                          shz = (rz - (ck - t0z)) + C::GL - t0z;
+                if constexpr (C::UG) {
+                    using U = UWin<N, GV>;
+                    double ws[NS + 1], uxn[U::WN], uyn[U::WN], uzn[U::ZT], uxs[U::WS], uys[U::WS], uzs[U::ZT];
+                    place_uniform<N, U::WN, U::WN>(wxn, fxn - (ci + U::AN), uxn);
+                    place_uniform<N, U::WN, U::WN>(wyn, fyn - (cj + U::AN), uyn);
+                    place_uniform<N, U::WN, U::ZT>(wzn, fzn - (ck + U::AN), uzn);
+                    place_uniform<NS, U::WS, U::WS>(ws, shape_weights<NS>(xi - 0.5, ws) - (ci + U::AS), uxs);
+                    place_uniform<NS, U::WS, U::WS>(ws, shape_weights<NS>(et - 0.5, ws) - (cj + U::AS), uys);
+                    place_uniform<NS, U::WS, U::ZT>(ws, shape_weights<NS>(ze - 0.5, ws) - (ck + U::AS), uzs);
+                    gather6_cell<N, GV, C>(Et, ci + U::AN + shx, cj + U::AN + shy, ck + U::AN + shz, ci + U::AS + shx,
+                                           cj + U::AS + shy, ck + U::AS + shz, uxn, uyn, uzn, uxs, uys, uzs, eb);
+                } else {
+                    double wxs[NS + 1], wys[NS + 1], ws[NS + 1], wzs[N + 1];
+                    const int fxs = shape_weights<NS>(xi - 0.5, wxs) + shx, fys = shape_weights<NS>(et - 0.5, wys) + shy,
+                              fzs = shape_weights<NS>(ze - 0.5, ws) + shz;
+#pragma unroll
+                    for (int k = 0; k <= N; ++k) wzs[k] = (k <= NS) ? ws[(k <= NS) ? k : 0] : 0.0;
+                    gather6_part<N, GV, C>(Et, fxn + shx, fyn + shy, fzn + shz, fxs, fys, fzs, wxn, wyn, wzn, wxs, wys,
+                                           wzs, eb);
+                }
+            } else {
+                gather_global6<N, GV>(g, f, xi, et, ze, eb);
+                ++n_glob;
+            }
+            boris_push(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
+            const double dtg = dt_over_gamma(g.dt, inv_c2, ux, uy, uz);
+            const double x1 = x + dtg * ux, y1 = y + dtg * uy, z1 = z + dtg * uz;
+            xi1 = (x1 - g.xmin) * g.inv_dx; et1 = (y1 - g.ymin) * g.inv_dy; ze1 = (z1 - g.zmin) * g.inv_dz;
+            const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
+                             !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
+            bad_any = bad_any || bad;
+            const double xw = wrap1(x1, g.xmin, g.xmax, g.Lx), yw = wrap1(y1, g.ymin, g.ymax, g.Ly),
+                         zw = wrap1(z1, g.zmin, g.zmax, g.Lz);
+            po.x[ip] = xw;
+            po.y[ip] = yw;
+            po.z[ip] = zw;
+            if (key_out != nullptr) {       // the next pic_sort's key (same formula as key_hist_kernel)
+                const int ki = min(max(__double2int_rd((xw - g.xmin) * g.inv_dx), 0), g.nx - 1);
+                const int kj = min(max(__double2int_rd((yw - g.ymin) * g.inv_dy), 0), g.ny - 1);
+                const int kk = min(max(__double2int_rd((zw - g.zmin) * g.inv_dz), 0), g.nz - 1);
+                key_out[ip] = (unsigned int)ki + (unsigned int)g.nx * ((unsigned int)kj + (unsigned int)g.ny * (unsigned int)kk);
+            }
+            po.ux[ip] = ux;
+            po.uy[ip] = uy;
+            po.uz[ip] = uz;
+            // ---- classify: fast = stayed inside the cell the sort listed it in -------------
+            const bool listed = in_tile && rx == rx0 && ry == ry0 && rz == rz0;   // the particle sits in the cell it is listed under
+            const bool deposits = !bad && qw != 0.0;
+            const int ncross = (__double2int_rd(xi1) != ci) + (__double2int_rd(et1) != cj) +
+                               (__double2int_rd(ze1) != ck);
+            fast = deposits && listed && ncross <= 1;   // phase B handles one crossed face
+            is_slow = deposits && !fast;
+            if (in_tile) { if (is_slow) ++n_slow; else ++n_fast; }
+        }
+        // ---- the ring slots of this sub-chunk must have been consumed ------------------------------
+        while (t0 + 32 - ld_acquire(S.flags + 1) > C::RING) __nanosleep(32);
+        if (ip >= 0) {
+            double* rec = S.body + body_word<C>(slot);
+            if (fast) {
+                // ---- fast record: old shapes and shape differences on the cell's window -------------
+                double fr[FR::LEN];
+                int code = REC_FAST;
+                double ext_e = 0.0;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const double a1 = (d == 0) ? xi1 : ((d == 1) ? et1 : ze1);
+                    const int cell = (d == 0) ? ci : ((d == 1) ? cj : ck);
+                    const int f0 = (d == 0) ? fxn : ((d == 1) ? fyn : fzn);
+                    const double (&w0)[N + 1] = (d == 0) ? wxn : ((d == 1) ? wyn : wzn);
+                    double w1[N + 1], s0[FW], s1[FW], e_lo, e_hi;
+                    const int f1 = shape_weights<N>(a1, w1);
+                    to_fast_window<N>(w0, f0, cell + FA, s0);
+                    place_new_window<N>(w1, f1 - (cell + FA), s1, e_lo, e_hi);
+#pragma unroll
+                    for (int a = 0; a < FW - 1; ++a) {
+                        fr[FR::s0(d, a)] = s0[a];
+                        fr[FR::ds(d, a)] = s1[a] - s0[a];
+                    }
+                    if (e_lo != 0.0) { code = 1 + 2 * d; ext_e = e_lo; }
+                    if (e_hi != 0.0) { code = 2 + 2 * d; ext_e = e_hi; }
+                }
+#pragma unroll
+                for (int k = 0; k < FR::LEN / 2; ++k) st2(rec, 2 * k, fr[2 * k], fr[2 * k + 1]);
+                st2(S.tails, 2 * slot, -qw * inv_dt, ext_e);
+                S.codes[slot] = code;
+            } else if (is_slow) {
+                st2(rec, 0, xi, et); st2(rec, 2, ze, xi1); st2(rec, 4, et1, ze1); st2(rec, 6, qw, 0.0);
+                S.codes[slot] = REC_SLOW;
+            } else {
+                S.codes[slot] = REC_NONE;
+            }
+        }
+        __syncwarp();
+        // ---------------- slow path: one particle at a time, whole warp ---------------------
+        unsigned int slow_mask = __ballot_sync(0xffffffffu, is_slow);
+        while (slow_mask) {
+            const int L = __ffs(slow_mask) - 1;
+            slow_mask &= slow_mask - 1;
+            slow_build<N>(S.body + body_word<C>((t0 + L) % C::RING), S.scr, g, inv_dt, lane);
+            slow_deposit<N>(S.scr, g, f, lane);
+            __syncwarp();
+        }
+        // publish: the records up to here are staged (the consumer skips slow and empty slots by their code)
+        if (lane == 0) st_release(S.flags, min(T, t0 + 32));
+        c0 = c1; ip0 = ip1; c1 = c2; ip1 = ip2; is1 = is2;
+    }
+    // ---- flags and counters ----------------------------------------------------------------------
+    if (bad_any) status->ephys = 1;
+    n_fast = __reduce_add_sync(0xffffffffu, n_fast);
+    n_slow = __reduce_add_sync(0xffffffffu, n_slow);
+    n_glob = __reduce_add_sync(0xffffffffu, n_glob);
+    if (lane == 0) {
+        if (n_fast) atomicAdd(&status->n_fast, (unsigned long long)n_fast);
+        if (n_slow) atomicAdd(&status->n_slow, (unsigned long long)n_slow);
+        if (n_glob) atomicAdd(&status->n_global, (unsigned long long)n_glob);
+    }
+}
+
+template <int N, int GV, class C>
 __global__ void __launch_bounds__(C::NT, C::MINB)
 particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigned int* __restrict__ perm,
                       unsigned int* __restrict__ key_out, double q, double h,
                       const unsigned int* __restrict__ cell_offset, int ntx, int nty, DevStatus* status) {
-    constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA, DRIFT = C::DRIFT;
-    using FR = FastRec<N>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* Et = reinterpret_cast<double*>(smem_raw);            // TOT words: Ex Ey Ez Bx By Bz
-    double* stg_all = Et + C::TOT;                               // NW * STG_W
-    int* row_off = reinterpret_cast<int*>(stg_all + C::NW * C::STG_W);   // NROW x (TX+1) container indices
-    int* next_row = row_off + C::NOFF;
+    double* stg_all = Et + C::TOT;                               // NP * STG_W
+    int* row_off = reinterpret_cast<int*>(stg_all + C::NP * C::STG_W);   // NROW x (TX+1) container indices
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     int b = blockIdx.x;
@@ -580,7 +976,6 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
             v = (int)cell_offset[(long long)g.nx * (j + (long long)g.ny * k) + min(t0x + c, g.nx)];
         row_off[e] = v;
     }
-    if (tid == 0) *next_row = 0;
     __syncthreads();
     int n_tile = 0;
 #pragma unroll 4
@@ -616,301 +1011,113 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
             }
         }
     }
-    __syncthreads();
 
-    const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
-    const double inv_dt = 1.0 / g.dt;
-    const double area_x = g.inv_dy * g.inv_dz, area_y = g.inv_dx * g.inv_dz, area_z = g.inv_dx * g.inv_dy;
-    double* stg = stg_all + warp * C::STG_W;
-    const int bq = lane >> 2, bs = lane & 3;     // phase B role: cell of the row, plane of the window
-    unsigned int n_fast = 0, n_slow = 0, n_glob = 0;
-    bool bad_any = false;
-    double* pbuf = stg + C::PITCH * C::NSLOT + C::SLOW_W;     // landing buffer: [x y z ux uy uz w id][lane]
-    int buf_start = -1;                                        // sorted index of lane 0's particle in it
-    int isn_reg = 0, isn_tag = -2;                             // perm[] entry read two sub-chunks ahead, and for which start
-
-    int row_ahead = 0;
-    if (lane == 0) row_ahead = atomicAdd(next_row, 1);
-    row_ahead = __shfl_sync(0xffffffffu, row_ahead, 0);
-    for (;;) {
-        const int row = row_ahead;
-        if (row >= C::NROW) break;
-        if (lane == 0) row_ahead = atomicAdd(next_row, 1);     // the row after this one: prefetch its head
-        row_ahead = __shfl_sync(0xffffffffu, row_ahead, 0);
-        int nrow_lo = 0, nrow_hi = 0;      // sorted range of the row fetched ahead
-        if (row_ahead < C::NROW) {
-            nrow_lo = row_off[row_ahead * (C::TX + 1)];
-            nrow_hi = row_off[row_ahead * (C::TX + 1) + C::TX];
-        }
-        const int* off = row_off + row * (C::TX + 1);
-        const int row_lo = off[0], row_hi = off[C::TX];
-        if (row_lo >= row_hi) continue;
-        const int ry0 = row % C::TY, rz0 = row / C::TY;     // the row's tile-relative (y, z) cell
-        const int cell_lo = off[bq], cell_hi = off[bq + 1];  // phase B: this lane's cell
-        CellAcc<N> acc;
-        acc.clear();
-        const long long win0 = g.idx(t0x + bq + FA, t0y + ry0 + FA, t0z + rz0 + FA);   // this lane's cell window
-
-        for (int base = row_lo; base < row_hi; base += C::CHUNK) {
-            // ---------------- phase A: lane <-> particle, 32 at a time ---------------------------
-#pragma unroll 1
-            for (int sub = 0; sub < C::CHUNK; sub += 32) {
-                const int ip = base + sub + lane;
-                if (base + sub >= row_hi) break;
-                // ---- particle data of this sub-chunk: copied to the warp's landing buffer one sub-chunk ago ----
-                if (buf_start != base + sub) {      // cold start, or the row fetched ahead was empty: fetch now
-                    if (ip < row_hi) {
-                        const int is = (perm != nullptr) ? (int)perm[ip] : ip;
-                        cp_async8(pbuf + 0 * 32 + lane, p.x + is); cp_async8(pbuf + 1 * 32 + lane, p.y + is);
-                        cp_async8(pbuf + 2 * 32 + lane, p.z + is); cp_async8(pbuf + 3 * 32 + lane, p.ux + is);
-                        cp_async8(pbuf + 4 * 32 + lane, p.uy + is); cp_async8(pbuf + 5 * 32 + lane, p.uz + is);
-                        cp_async8(pbuf + 6 * 32 + lane, p.w + is);
-                        if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + is);
-                    }
-                    cp_async_commit();
-                }
-                cp_async_wait_all();
-                __syncwarp();
-                const double x = pbuf[0 * 32 + lane], y = pbuf[1 * 32 + lane], z = pbuf[2 * 32 + lane];
-                double ux = pbuf[3 * 32 + lane], uy = pbuf[4 * 32 + lane], uz = pbuf[5 * 32 + lane];
-                const double wgt = pbuf[6 * 32 + lane], idv = pbuf[7 * 32 + lane];
-                __syncwarp();       // every lane has read: the buffer may be refilled
-                // ---- next sub-chunk this warp will walk (rest of the row, else head of the row fetched ahead):
-                // its particle data start their way to the landing buffer NOW, so that they have this whole
-                // sub-chunk to arrive.  Deferred sort: their places come from perm[], read ONE MORE sub-chunk
-                // ahead into a register (isn_reg, valid for the sub-chunk that starts at isn_tag).
-                {
-                    int base1 = base, sub1 = sub + 32, hi1 = row_hi;
-                    bool in_next = false;
-                    if (!(sub1 < C::CHUNK && base1 + sub1 < row_hi)) {
-                        base1 = base + C::CHUNK; sub1 = 0;
-                        if (base1 >= row_hi) { base1 = nrow_lo; hi1 = nrow_hi; in_next = true; }
-                    }
-                    const int nstart = base1 + sub1;
-                    if (nstart + lane < hi1) {
-                        int isn = nstart + lane;
-                        if (perm != nullptr) isn = (isn_tag == nstart) ? isn_reg : (int)perm[nstart + lane];
-                        cp_async8(pbuf + 0 * 32 + lane, p.x + isn); cp_async8(pbuf + 1 * 32 + lane, p.y + isn);
-                        cp_async8(pbuf + 2 * 32 + lane, p.z + isn); cp_async8(pbuf + 3 * 32 + lane, p.ux + isn);
-                        cp_async8(pbuf + 4 * 32 + lane, p.uy + isn); cp_async8(pbuf + 5 * 32 + lane, p.uz + isn);
-                        cp_async8(pbuf + 6 * 32 + lane, p.w + isn);
-                        if (perm != nullptr) cp_async8(pbuf + 7 * 32 + lane, p.id + isn);
-                    }
-                    cp_async_commit();
-                    buf_start = (nstart < hi1) ? nstart : -1;
-                    if (perm != nullptr) {      // the sub-chunk after that one
-                        int start2 = base1 + sub1 + 32, hi2 = hi1;
-                        if (!(sub1 + 32 < C::CHUNK && start2 < hi1)) {
-                            start2 = base1 + C::CHUNK;
-                            if (start2 >= hi1) { start2 = in_next ? -2 : nrow_lo; hi2 = in_next ? -2 : nrow_hi; }
-                        }
-                        isn_tag = start2;
-                        isn_reg = (start2 >= 0 && start2 + lane < hi2) ? ld_u32_now(perm + start2 + lane) : 0;
-                    }
-                }
-                double* rec = stg + skew(sub + lane) * C::PITCH;
-                bool is_slow = false;
-                if (ip < row_hi && sub + lane < C::CHUNK) {
-                    const double qw = q * wgt;
-                    if (perm != nullptr) {          // deferred sort: the other buffer gets every array, in sorted order
-                        po.w[ip] = wgt;
-                        po.id[ip] = (unsigned long long)__double_as_longlong(idv);
-                    }
-                    const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy,
-                                 ze = (z - g.zmin) * g.inv_dz;
-                    const int ci = __double2int_rd(xi), cj = __double2int_rd(et), ck = __double2int_rd(ze);
-                    const int rx = rel_cell<DRIFT>(ci, t0x, C::TX, g.nx), ry = rel_cell<DRIFT>(cj, t0y, C::TY, g.ny),
-                              rz = rel_cell<DRIFT>(ck, t0z, C::TZ, g.nz);
-                    const bool in_tile = rx >= -DRIFT && rx <= C::TX - 1 + DRIFT && t0x + rx <= g.nx - 1 + DRIFT &&
-                                         ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
-                                         rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
-                    double wxn[N + 1], wyn[N + 1], wzn[N + 1];
-                    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn),
-                              fzn = shape_weights<N>(ze, wzn);
-                    double eb[6];
-                    if (in_tile) {
-                        double wxs[N + 1], wys[N + 1], wzs[N + 1];
-                        // first nodes, from global node index to tile slot: slot = node - (t0 - GL) + image shift
-                        const int shx = (rx - (ci - t0x)) + C::GL - t0x, shy = (ry - (cj - t0y)) + C::GL - t0y,
-                                  shz = (rz - (ck - t0z)) + C::GL - t0z;
-                        const int fxs = shape_weights<N>(xi - 0.5, wxs) + shx,
-                                  fys = shape_weights<N>(et - 0.5, wys) + shy,
-                                  fzs = shape_weights<N>(ze - 0.5, wzs) + shz;
-                        gather6_tile<N, C>(Et, fxn + shx, fyn + shy, fzn + shz, fxs, fys, fzs, wxn, wyn, wzn, wxs,
-                                           wys, wzs, eb);
-                    } else {
-                        gather_global6<N>(g, f, xi, et, ze, eb);
-                        ++n_glob;
-                    }
-                    boris_push(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
-                    const double dtg = dt_over_gamma(g.dt, inv_c2, ux, uy, uz);
-                    const double x1 = x + dtg * ux, y1 = y + dtg * uy, z1 = z + dtg * uz;
-                    const double xi1 = (x1 - g.xmin) * g.inv_dx, et1 = (y1 - g.ymin) * g.inv_dy,
-                                 ze1 = (z1 - g.zmin) * g.inv_dz;
-                    const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
-                                     !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
-                    bad_any = bad_any || bad;
-                    const double xw = wrap1(x1, g.xmin, g.xmax, g.Lx), yw = wrap1(y1, g.ymin, g.ymax, g.Ly),
-                                 zw = wrap1(z1, g.zmin, g.zmax, g.Lz);
-                    po.x[ip] = xw;
-                    po.y[ip] = yw;
-                    po.z[ip] = zw;
-                    if (key_out != nullptr) {       // the next pic_sort's key (same formula as key_hist_kernel)
-                        const int ki = min(max(__double2int_rd((xw - g.xmin) * g.inv_dx), 0), g.nx - 1);
-                        const int kj = min(max(__double2int_rd((yw - g.ymin) * g.inv_dy), 0), g.ny - 1);
-                        const int kk = min(max(__double2int_rd((zw - g.zmin) * g.inv_dz), 0), g.nz - 1);
-                        key_out[ip] = (unsigned int)ki + (unsigned int)g.nx * ((unsigned int)kj + (unsigned int)g.ny * (unsigned int)kk);
-                    }
-                    po.ux[ip] = ux;
-                    po.uy[ip] = uy;
-                    po.uz[ip] = uz;
-                    // ---- classify: fast = stayed inside the cell the sort listed it in -------------
-                    const int rxc = min(max(rx, 0), C::TX - 1);
-                    const bool listed = in_tile && rx == rxc && off[rxc] <= ip && ip < off[rxc + 1] && ry == ry0 &&
-                                        rz == rz0;      // ip lies in the sorted range of the cell the particle is in
-                    const bool deposits = !bad && qw != 0.0;
-                    const int ncross = (__double2int_rd(xi1) != ci) + (__double2int_rd(et1) != cj) +
-                                       (__double2int_rd(ze1) != ck);
-                    const bool fast = deposits && listed && ncross <= 1;   // phase B handles one crossed face
-                    is_slow = deposits && !fast;
-                    if (in_tile) { if (is_slow) ++n_slow; else ++n_fast; }
-                    if (fast) {
-                        // ---- fast record: old/new shapes on the cell's window, prefix-summed factors --
-                        double fr[FLAG + 1];
+    // ---- a producer's stream: its RPW rows, cell by cell, every cell padded to an even length (UG) --------
+    const int pair = (warp < C::NP) ? warp : warp - C::NP;
+    const Staging<C> S(stg_all + pair * C::STG_W);
+    const int row_first = pair * C::RPW;
+    if (warp < C::NP) {
+        int carry = 0;
 #pragma unroll
-                        for (int k = 0; k <= FLAG; ++k) fr[k] = 0.0;
-                        double code = REC_FAST, ext_e = 0.0, ext_pd = 0.0;
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) {
-                            const double a1 = (d == 0) ? xi1 : ((d == 1) ? et1 : ze1);
-                            const int cell = (d == 0) ? ci : ((d == 1) ? cj : ck);
-                            const int f0 = (d == 0) ? fxn : ((d == 1) ? fyn : fzn);
-                            const double (&w0)[N + 1] = (d == 0) ? wxn : ((d == 1) ? wyn : wzn);
-                            const double area = (d == 0) ? g.inv_dy * g.inv_dz
-                                                         : ((d == 1) ? g.inv_dx * g.inv_dz : g.inv_dx * g.inv_dy);
-                            double w1[N + 1], s0[FW], s1[FW], e_lo, e_hi;
-                            const int f1 = shape_weights<N>(a1, w1);
-                            to_fast_window<N>(w0, f0, cell + FA, s0);
-                            place_new_window<N>(w1, f1 - (cell + FA), s1, e_lo, e_hi);
-                            const double cq = (-qw * inv_dt) * area;
-                            double run = e_lo;            // the prefix starts at the lowest node of the union window
-                            const double pd_lo = cq * run;
-#pragma unroll
-                            for (int a = 0; a < FW; ++a) {
-                                const double dd = s1[a] - s0[a];
-                                fr[2 * FW * d + a] = s0[a];
-                                fr[2 * FW * d + FW + a] = dd;
-                                run += dd;
-                            }
-                            if (e_lo != 0.0) { code = 1.0 + 2.0 * d; ext_e = e_lo; ext_pd = pd_lo; }
-                            if (e_hi != 0.0) { code = 2.0 + 2.0 * d; ext_e = e_hi; ext_pd = cq * run; }
-                        }
-#pragma unroll
-                        for (int k = 0; k < FR::LEN / 2; ++k) st2(rec, 2 * k, fr[2 * k], fr[2 * k + 1]);
-                        st2(rec, RCQ, -qw * inv_dt, code);
-                        if (code != REC_FAST) st2(stg, ext_word(sub + lane, C::PITCH), ext_e, ext_pd);
-                    } else if (is_slow) {
-                        st2(rec, 0, xi, et); st2(rec, 2, ze, xi1); st2(rec, 4, et1, ze1); st2(rec, 6, qw, 0.0);
-                        st2(rec, RCQ, 0.0, REC_SLOW);
-                    } else {
-                        rec[FLAG] = REC_NONE;
-                    }
-                }
-                __syncwarp();
-                // ---------------- slow path: one particle at a time, whole warp ---------------------
-                unsigned int slow_mask = __ballot_sync(0xffffffffu, is_slow);
-                while (slow_mask) {
-                    const int L = __ffs(slow_mask) - 1;
-                    slow_mask &= slow_mask - 1;
-                    double* scr = stg + C::PITCH * C::NSLOT;
-                    slow_build<N>(stg + skew(sub + L) * C::PITCH, scr, g, inv_dt, lane);
-                    slow_deposit<N>(scr, g, f, lane);
-                    __syncwarp();
-                }
+        for (int half = 0; half < (C::NC + 31) / 32; ++half) {
+            const int c = half * 32 + lane;
+            int n = 0;
+            if (c < C::NC) {
+                const int* o = row_off + (row_first + c / C::TX) * (C::TX + 1) + c % C::TX;
+                n = o[1] - o[0];
+                if (C::UG) n = (n + 1) & ~1;
             }
-            // ---------------- phase B: lane <-> (cell, plane) ------------------------------------
-            {
-                const int lo = max(cell_lo, base), hi = min(cell_hi, base + C::CHUNK);
-                const int len = (bs < FW) ? hi - lo : 0;
-                const int maxlen = __reduce_max_sync(0xffffffffu, max(len, 0));
-#pragma unroll 1
-                for (int t = 0; t < maxlen; ++t)
-                    if (t < len) {
-                        const int pslot = lo + t - base;
-                        acc.add(stg + skew(pslot) * C::PITCH, bs, stg + ext_word(pslot, C::PITCH), f.Jx + win0,
-                                f.Jy + win0, f.Jz + win0, g.sy, g.sz, area_x, area_y, area_z);
-                    }
+            int incl = n;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
             }
-            __syncwarp();
+            if (c < C::NC) S.cp[c] = carry + incl - n;
+            carry += __shfl_sync(0xffffffffu, incl, 31);
         }
-        // ---------------- flush the row's accumulators ---------------------------------------------
-        acc.flush(g, f, win0, bs, lane);
+        if (lane == 0) {
+            S.cp[C::NC] = carry;
+            S.flags[0] = 0;
+            S.flags[1] = 0;
+        }
     }
-    // ---- flags and counters ----------------------------------------------------------------------
-    if (bad_any) status->ephys = 1;
-    n_fast = __reduce_add_sync(0xffffffffu, n_fast);
-    n_slow = __reduce_add_sync(0xffffffffu, n_slow);
-    n_glob = __reduce_add_sync(0xffffffffu, n_glob);
-    if (lane == 0) {
-        if (n_fast) atomicAdd(&status->n_fast, (unsigned long long)n_fast);
-        if (n_slow) atomicAdd(&status->n_slow, (unsigned long long)n_slow);
-        if (n_glob) atomicAdd(&status->n_global, (unsigned long long)n_glob);
-    }
+    __syncthreads();      // stencil, cp[] and the flags of every pair
+
+    if (warp < C::NP)
+        tile_producer<N, GV, C>(g, f, p, po, perm, key_out, q, h, Et, S, row_off, row_first, t0x, t0y, t0z, lane, status);
+    else
+        tile_consumer<N, C>(g, f, S, row_off, row_first, t0x, t0y, t0z, lane);
 }
 
 // CfgDrift: a species that has moved since its last sort (particles up to one cell outside their listed
-// cell still gather from shared memory); one block of 8 warps per SM.
-// CfgFresh: right after pic_sort; two blocks of 4 warps per SM (2 x 112.6 KB of shared memory).
-using CfgDrift = TileCfg<8, 4, 4, 8, 1, 1, 72>;
-using CfgFresh = TileCfg<8, 4, 4, 4, 2, 0, 72>;
+// cell still gather from shared memory); one block of 6 + 6 warps per SM, tile 8 x 4 x 6.
+// CfgFresh: right after pic_sort; two blocks of 3 + 3 warps per SM, tile 8 x 4 x 6.
+using CfgDrift = TileCfg<8, 4, 6, 6, 1, 1, 112, false>;
+using CfgFresh = TileCfg<8, 4, 6, 3, 2, 0, 120, false>;
 static_assert(2 * (CfgFresh::SMEM + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
+static_assert(CfgDrift::SMEM <= 227 * 1024, "the drift block must fit one SM");
 
-template <int N, class Cfg>
+template <int N, int GV, class Cfg>
 void launch_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po, const unsigned int* perm,
                  unsigned int* key_out, double q, double h, const unsigned int* cell_offset, DevStatus* status,
                  cudaStream_t st) {
     const int ntx = (g.nx + Cfg::TX - 1) / Cfg::TX, nty = (g.ny + Cfg::TY - 1) / Cfg::TY,
               ntz = (g.nz + Cfg::TZ - 1) / Cfg::TZ;
     const long long nb = (long long)ntx * nty * ntz;
-    particles_tile_kernel<N, Cfg><<<(unsigned)nb, Cfg::NT, Cfg::SMEM, st>>>(g, f, p, po, perm, key_out, q, h, cell_offset,
-                                                                           ntx, nty, status);
+    particles_tile_kernel<N, GV, Cfg><<<(unsigned)nb, Cfg::NT, Cfg::SMEM, st>>>(g, f, p, po, perm, key_out, q, h,
+                                                                               cell_offset, ntx, nty, status);
 }
 
-template <int N, class Cfg>
+template <int N, int GV, class Cfg>
 cudaError_t setup_one() {
-    cudaError_t e = cudaFuncSetAttribute(particles_tile_kernel<N, Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(particles_tile_kernel<N, GV, Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)Cfg::SMEM);
     if (e == cudaSuccess && Cfg::MINB > 1)
-        e = cudaFuncSetAttribute(particles_tile_kernel<N, Cfg>, cudaFuncAttributePreferredSharedMemoryCarveout,
+        e = cudaFuncSetAttribute(particles_tile_kernel<N, GV, Cfg>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                  (int)cudaSharedmemCarveoutMaxShared);
     return e;
+}
+
+template <int GV, class Cfg>
+cudaError_t setup_orders() {
+    cudaError_t e = setup_one<1, GV, Cfg>();
+    if (e == cudaSuccess) e = setup_one<2, GV, Cfg>();
+    if (e == cudaSuccess) e = setup_one<3, GV, Cfg>();
+    return e;
+}
+
+template <int GV, class Cfg>
+void launch_orders(int order, const Grid& g, const Fields& f, const Particles& p, const Particles& po,
+                   const unsigned int* perm, unsigned int* key_out, double q, double h, const unsigned int* cell_offset,
+                   DevStatus* status, cudaStream_t st) {
+    if (order == 1) launch_tile<1, GV, Cfg>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+    else if (order == 2) launch_tile<2, GV, Cfg>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+    else launch_tile<3, GV, Cfg>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
 }
 
 }  // namespace
 
 int tile_setup() {
-    cudaError_t e = setup_one<1, CfgDrift>();
-    if (e == cudaSuccess) e = setup_one<2, CfgDrift>();
-    if (e == cudaSuccess) e = setup_one<3, CfgDrift>();
-    if (e == cudaSuccess) e = setup_one<1, CfgFresh>();
-    if (e == cudaSuccess) e = setup_one<2, CfgFresh>();
-    if (e == cudaSuccess) e = setup_one<3, CfgFresh>();
+    cudaError_t e = setup_orders<0, CfgDrift>();
+    if (e == cudaSuccess) e = setup_orders<0, CfgFresh>();
+    if (e == cudaSuccess) e = setup_orders<1, CfgDrift>();
+    if (e == cudaSuccess) e = setup_orders<1, CfgFresh>();
     return (int)e;
 }
 
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po,
                           const unsigned int* perm, unsigned int* key_out, long long n, double q, double m, int order,
-                          const unsigned int* cell_offset, bool fresh, DevStatus* status, cudaStream_t st) {
+                          int gather_variant, const unsigned int* cell_offset, bool fresh, DevStatus* status,
+                          cudaStream_t st) {
     if (n <= 0) return 0;
     const double h = q * g.dt / (2.0 * m);
     if (fresh) {
-        if (order == 1) launch_tile<1, CfgFresh>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
-        else if (order == 2) launch_tile<2, CfgFresh>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
-        else launch_tile<3, CfgFresh>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        if (gather_variant) launch_orders<1, CfgFresh>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else launch_orders<0, CfgFresh>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
     } else {
-        if (order == 1) launch_tile<1, CfgDrift>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
-        else if (order == 2) launch_tile<2, CfgDrift>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
-        else launch_tile<3, CfgDrift>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        if (gather_variant) launch_orders<1, CfgDrift>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else launch_orders<0, CfgDrift>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
     }
     return 1;
 }

@@ -69,6 +69,7 @@ struct pic_ctx {
     unsigned long long launches = 0, steps = 0, sorts = 0;
     // options
     int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1, fuse_keys = 1;
+    int gather_variant = 0, smooth_passes = 0;      // NEXT-3 options
     YeeMaps yee_maps{};
     int device = 0;                     // ordinal of the device the arena lives on; made current by every call
     int yee_tma_ok = 0;                 // tensor maps built: the TMA-staged Yee kernels are available
@@ -491,7 +492,8 @@ int pic_step(pic_ctx* c, int nsteps) {
                     const Particles& PO = deferred ? S.buf[S.cur ^ 1] : P;
                     const bool keys = c->fuse_keys != 0;
                     c->launches += launch_particles_tile(g, c->f, P, PO, deferred ? S.perm : nullptr,
-                                                         keys ? S.key : nullptr, S.n, S.q, S.m, c->order, S.cell_offset,
+                                                         keys ? S.key : nullptr, S.n, S.q, S.m, c->order, c->gather_variant,
+                                                         S.cell_offset,
                                                          S.steps_since_sort == 0 && c->tile_fresh != 0, c->status,
                                                          c->stream);
                     S.keys_valid = keys;
@@ -504,7 +506,8 @@ int pic_step(pic_ctx* c, int nsteps) {
                     if (S.sorted && S.degraded) c->fallbacks += 1;
                     materialize(c, S);
                     S.keys_valid = false;
-                    launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->status, c->stream);
+                    launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->gather_variant, c->status,
+                                            c->stream);
                     c->launches += 1;
                 }
                 S.steps_since_sort += 1;
@@ -522,6 +525,10 @@ int pic_step(pic_ctx* c, int nsteps) {
         nvtxRangePushA("fold_J");
         launch_fold_guards3(g, c->f.Jx, c->f.Jy, c->f.Jz, c->stream);
         c->launches += 1;
+        if (c->smooth_passes > 0) {      // NEXT-3: binomial smoothing of J before the E push
+            double* J[3] = {c->f.Jx, c->f.Jy, c->f.Jz};
+            for (int k = 0; k < 3; ++k) c->launches += launch_smooth_binomial(g, J[k], c->tmp, c->smooth_passes, c->stream);
+        }
         nvtxRangePop();
         if (timing) cudaEventRecord(ev[3], c->stream);
         // steps 6-8
@@ -710,6 +717,13 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     else if (!strcmp(name, "sort_deferred")) c->sort_deferred = value != 0;
     else if (!strcmp(name, "fuse_keys")) c->fuse_keys = value != 0;
     else if (!strcmp(name, "drift_watch")) c->drift_watch = value != 0;
+    else if (!strcmp(name, "gather_variant")) {
+        if (value < 0 || value > 1) return fail(c, PIC_EINVAL, "gather_variant must be 0 or 1");
+        c->gather_variant = (int)value;
+    } else if (!strcmp(name, "smooth_passes")) {
+        if (value < 0 || value > 16) return fail(c, PIC_EINVAL, "smooth_passes must be 0 .. 16");
+        c->smooth_passes = (int)value;
+    }
     else return fail(c, PIC_EINVAL, "unknown option '%s'", name);
     return PIC_OK;
 }

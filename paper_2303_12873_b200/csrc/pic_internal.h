@@ -63,11 +63,14 @@ int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out);   // 0 = ok; el
 void launch_push_B(const Grid& g, const Fields& f, double dth, const YeeMaps* maps, cudaStream_t st);
 void launch_push_E(const Grid& g, const Fields& f, double dt, const YeeMaps* maps, cudaStream_t st);
 void launch_fill_guards(const Grid& g, double* F, cudaStream_t st);       // periodic images of one component
+// binomial (1-2-1 along x, y, z) smoothing of the interior of F, npass passes; tmp = a padded scratch component
+int launch_smooth_binomial(const Grid& g, double* F, double* tmp, int npass, cudaStream_t st);
 
 // ---- particles_global.cu --------------------------------------------------
 // gather + Boris + move + Esirkepov with global fp64 atomics + wrap; any particle order.
+// gather_variant: 0 = order n in every direction, 1 = order n-1 along a component's staggered directions
 void launch_particles_global(const Grid& g, const Fields& f, const Particles& p, long long n, double q,
-                             double m, int order, DevStatus* status, cudaStream_t st);
+                             double m, int order, int gather_variant, DevStatus* status, cudaStream_t st);
 void launch_deposit_rho(const Grid& g, const Particles& p, long long n, double q, int order, double* rho_pad,
                         cudaStream_t st);
 void launch_fold_guards(const Grid& g, double* F, cudaStream_t st);       // sum periodic images into the interior
@@ -104,7 +107,7 @@ struct TileScratch {
 // key_out != nullptr: the kernel also writes the cell key of every particle's new position (for the next pic_sort)
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& pout,
                           const unsigned int* perm, unsigned int* key_out, long long n, double q, double m, int order,
-                          const unsigned int* cell_offset, bool fresh, DevStatus* status,
+                          int gather_variant, const unsigned int* cell_offset, bool fresh, DevStatus* status,
                           cudaStream_t st);  // kernels launched
 int tile_setup();   // one-time cudaFuncSetAttribute calls; returns cudaError_t as int
 

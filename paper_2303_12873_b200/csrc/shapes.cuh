@@ -13,10 +13,15 @@
 
 namespace pic {
 
-// Fills w[0..N] and returns the node index of w[0].
+// Fills w[0..N] and returns the node index of w[0].  N = 0 (used only by the energy-conserving gather
+// variant, along staggered directions at order 1): the top-hat on [-1/2, 1/2), i.e. all the weight on node
+// floor(xi + 1/2).
 template <int N>
 __device__ __forceinline__ int shape_weights(double xi, double (&w)[N + 1]) {
-    if constexpr (N == 1) {
+    if constexpr (N == 0) {
+        w[0] = 1.0;
+        return __double2int_rd(xi + 0.5);
+    } else if constexpr (N == 1) {
         int i = __double2int_rd(xi);
         double d = xi - (double)i;
         w[0] = 1.0 - d;

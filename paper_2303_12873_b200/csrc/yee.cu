@@ -317,4 +317,46 @@ void launch_fill_guards(const Grid& g, double* F, cudaStream_t st) {
     fill_guards_kernel<<<nb, bs, 0, st>>>(g, F);
 }
 
+// ---- binomial smoothing of one component (pic_set_option "smooth_passes") -------------
+// One pass = the 1-2-1 filter along x, then y, then z, periodic.  The kernel reads the component with its
+// periodic guard images filled and evaluates the three filters in that order on the 3 x 3 x 3 neighbourhood of
+// its cell (the same operations, in the same order, as three sweeps over the whole array), writing the
+// interior of `out`.
+__global__ void smooth121_kernel(Grid g, const double* __restrict__ F, double* __restrict__ out) {
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x), j = (int)blockIdx.y, k = (int)blockIdx.z;
+    if (i >= g.nx) return;
+    const double* c = F + g.idx(i, j, k);
+    double tz[3];
+#pragma unroll
+    for (int dz = -1; dz <= 1; ++dz) {
+        double ty[3];
+#pragma unroll
+        for (int dy = -1; dy <= 1; ++dy) {
+            const double* r = c + g.sy * dy + g.sz * dz;
+            ty[dy + 1] = 0.25 * r[-1] + 0.5 * r[0] + 0.25 * r[1];
+        }
+        tz[dz + 1] = 0.25 * ty[0] + 0.5 * ty[1] + 0.25 * ty[2];
+    }
+    out[g.idx(i, j, k)] = 0.25 * tz[0] + 0.5 * tz[1] + 0.25 * tz[2];
+}
+
+__global__ void copy_interior_kernel(Grid g, const double* __restrict__ src, double* __restrict__ dst) {
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x), j = (int)blockIdx.y, k = (int)blockIdx.z;
+    if (i < g.nx) dst[g.idx(i, j, k)] = src[g.idx(i, j, k)];
+}
+
+// F := `npass` binomial passes of F (interior; the guard cells of F are left as periodic images of the last
+// but one pass and must not be relied on).  tmp = one padded scratch component.  Returns kernels launched.
+int launch_smooth_binomial(const Grid& g, double* F, double* tmp, int npass, cudaStream_t st) {
+    dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
+    int launches = 0;
+    for (int p = 0; p < npass; ++p) {
+        launch_fill_guards(g, F, st);
+        smooth121_kernel<<<nb, bs, 0, st>>>(g, F, tmp);
+        copy_interior_kernel<<<nb, bs, 0, st>>>(g, tmp, F);
+        launches += 3;
+    }
+    return launches;
+}
+
 }  // namespace pic
