@@ -53,18 +53,48 @@ BYTES_PER_PARTICLE = 104.0
 BYTES_PER_CELL = 96.0
 # Yee: B half (72 B/cell) + E (96 B/cell) + B half (72 B/cell)
 YEE_BYTES_PER_CELL = 240.0
-# fp64-pipe roofline of the fused kernel.  Instructions per particle = DFMA + DMUL + DADD
-# thread instructions executed per particle by the committed kernel (ncu, profiles/); order 3 measured,
-# orders 1 and 2 scaled by the gather/deposit operation counts.
-FP64_INSTR_PER_PARTICLE = {1: 410.0, 2: 780.0, 3: 1129.0}
+# fp64-pipe roofline of the fused kernel.  ALGORITHMIC fp64-pipe instructions per particle
+# (an FMA counts once): order 3 = gather 6 x (64 + 16 + 4) = 504 FMA + nine shape-weight sets ~108
+# + push and move ~130 + Esirkepov ~465 + ~20; orders 1 and 2 likewise.  What the committed kernel EXECUTES
+# (ncu sm__inst_executed_pipe_fp64, thread level) is reported beside it from profiles/measured_counters.json.
+FP64_INSTR_PER_PARTICLE = {1: 380.0, 2: 710.0, 3: 1230.0}
 FP64_LANES_PER_SM = 64
 N_SM = 148
 SM_MAX_MHZ = 1965.0
-# shared-memory bytes the kernel moves per particle: order 3 = 41.3 wavefronts x 128 B (ncu, profiles/r01_v5, section v7);
-# orders 1 and 2 scaled by the gather/deposit operand counts
-SMEM_BYTES_PER_PARTICLE = {1: 1350.0, 2: 2850.0, 3: 5290.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch at the default workload (profiles/)
-TRAFFIC_BYTES_PER_LAUNCH = 22.09e9
+
+
+def _measured_counters(workload_key):
+    """ncu counters of one launch of the dominant kernel at this workload, from the committed capture summary
+    profiles/measured_counters.json (written by hand from `ncu --set full`; names the capture it came from).
+    None when there is no capture of this workload: the bench then reports traffic = null."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "measured_counters.json")) as fh:
+            return json.load(fh).get(workload_key)
+    except Exception:
+        return None
+
+
+def _host_info():
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except Exception:
+        pass
+    return {"nproc": os.cpu_count(), "cpu_model": model}
+
+
+def _pin_to_one_core():
+    """taskset-style pinning of this process to one core; returns the core or None."""
+    try:
+        cores = sorted(os.sched_getaffinity(0))
+        os.sched_setaffinity(0, {cores[-1]})
+        return cores[-1], set(cores)
+    except Exception:
+        return None, None
 
 
 def _peaks():
@@ -155,14 +185,19 @@ def time_oracle(index: int, budget_s: float = 12.0, max_steps: int = 40):
     """particle-updates/s of the oracle as it stands, single-threaded, on the host."""
     wl, desc = _oracle_sample(index)
     o = _oracle_sim(wl)
-    o.step(1)                                   # warm-up (page in, build tables)
-    t0 = time.perf_counter()
-    n = 0
-    while n < max_steps and (n < 2 or time.perf_counter() - t0 < budget_s):
-        o.step(1)
-        n += 1
-    dt = time.perf_counter() - t0
-    return {"value": wl.nparticles * n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+    core, before = _pin_to_one_core()
+    try:
+        o.step(1)                                   # warm-up (page in, build tables)
+        t0 = time.perf_counter()
+        n = 0
+        while n < max_steps and (n < 2 or time.perf_counter() - t0 < budget_s):
+            o.step(1)
+            n += 1
+        dt = time.perf_counter() - t0
+    finally:
+        if before:
+            os.sched_setaffinity(0, before)
+    return {"value": wl.nparticles * n / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "pinned_to_core": core,
             "sample": "%s, %d steps in %.1f s" % (desc, n, dt),
             "cell_updates_per_s": wl.ncell * n / dt}
 
@@ -296,25 +331,32 @@ def run_ours(args):
     # The kernel is bound by on-chip arithmetic/LSU issue, not by HBM: the headline
     # roofline is the fp64 pipe; the HBM and shared-memory figures are reported beside it.
     fp64_peak = FP64_LANES_PER_SM * N_SM * SM_MAX_MHZ * 1e6 / 1e12          # T fp64 instructions/s
-    fp64_alg = FP64_INSTR_PER_PARTICLE.get(wl.order, FP64_INSTR_PER_PARTICLE[3]) * np_launch
+    fp64_per_particle = FP64_INSTR_PER_PARTICLE.get(wl.order, FP64_INSTR_PER_PARTICLE[3])
+    fp64_alg = fp64_per_particle * np_launch
     fp64_ach = fp64_alg / (ms_launch * 1e-3) / 1e12
+    full_size = args.n is None
+    mc = _measured_counters("configs[%d]" % args.config) if full_size else None
     roofline = {"bound": "alu", "kernel": kname, "achieved": fp64_ach, "peak": fp64_peak,
-                "peak_kind": "derived: 148 SMs x 64 fp64 lanes/clk x 1965 MHz (DESIGN.md 5.1; DFMA probe)",
-                "unit": "T fp64-instr/s", "frac": fp64_ach / fp64_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH
-                if (args.config == 2 and args.n is None) else None,
-                "traffic_note": "ncu dram bytes of one launch that also carries out the deferred sort: 15.57 GB "
-                                "algorithmic (104 B/particle + 96 B/cell) + 3.76 GB of the sort row (perm, w, id: "
-                                "28 B/particle) + 2.8 GB of halo and partial-sector overhead (profiles/r01_v5)",
-                "ms_per_launch": ms_launch, "algorithmic_fp64_instr_per_launch": fp64_alg,
+                "peak_kind": "derived: 148 SMs x 64 fp64 lanes/clk x 1965 MHz (DESIGN.md 5.1; DFMA probe: 62.5 lanes/clk/SM)",
+                "unit": "T fp64-instr/s", "frac": fp64_ach / fp64_peak,
+                "traffic": mc.get("dram_bytes_per_launch") if mc else None,
+                "traffic_source": mc.get("source") if mc else None,
+                "ms_per_launch": ms_launch, "algorithmic_fp64_instr_per_particle": fp64_per_particle,
+                "algorithmic_fp64_instr_per_launch": fp64_alg,
+                "executed_fp64_instr_per_particle": mc.get("executed_fp64_instr_per_particle") if mc else None,
                 "particle_updates_per_s_kernel_only": np_launch / (ms_launch * 1e-3)}
     hbm_ach = alg_bytes / (ms_launch * 1e-3) / 1e9
     roofline_hbm = {"bound": "hbm", "kernel": kname, "achieved": hbm_ach, "peak": hbm_peak, "peak_kind": hbm_kind,
                     "unit": "GB/s", "frac": hbm_ach / hbm_peak, "algorithmic_bytes_per_launch": alg_bytes}
-    smem_peak = 128.0 * N_SM * SM_MAX_MHZ * 1e6 / 1e9                       # GB/s of shared-memory data pipe
-    smem_ach = SMEM_BYTES_PER_PARTICLE.get(wl.order, SMEM_BYTES_PER_PARTICLE[3]) * np_launch / (ms_launch * 1e-3) / 1e9
-    roofline_smem = {"bound": "smem", "kernel": kname, "achieved": smem_ach, "peak": smem_peak,
-                     "peak_kind": "derived: 148 SMs x 128 B/clk x 1965 MHz", "unit": "GB/s",
-                     "frac": smem_ach / smem_peak}
+    roofline_smem = None
+    if mc and mc.get("lsu_wavefronts_per_particle"):
+        # LSU data pipe: one wavefront per clock per SM; wavefronts per particle from the committed ncu capture
+        wf_peak = N_SM * SM_MAX_MHZ * 1e6                                    # wavefronts/s
+        wf_ach = mc["lsu_wavefronts_per_particle"] * np_launch / (ms_launch * 1e-3)
+        roofline_smem = {"bound": "lsu", "kernel": kname, "achieved": wf_ach / 1e9, "peak": wf_peak / 1e9,
+                         "peak_kind": "derived: 148 SMs x 1 wavefront/clk x 1965 MHz (profiles/r02_lsu.md)",
+                         "unit": "G wavefronts/s", "frac": wf_ach / wf_peak,
+                         "lsu_wavefronts_per_particle": mc["lsu_wavefronts_per_particle"]}
     nsteps_t = max(1.0, st["steps"])
     yee_ms = (st["yee_B"] + st["yee_E"]) / nsteps_t
     stages = {"per_step_ms": {k: st[k] / nsteps_t for k in ("zero_J", "particles", "fold_J", "yee_B", "yee_E")},
@@ -325,7 +367,9 @@ def run_ours(args):
     roofline_yee = None
     if yee_ms > 0:
         yee_gbs = YEE_BYTES_PER_CELL * ncell / (yee_ms * 1e-3) / 1e9
-        roofline_yee = {"bound": "hbm", "kernel": "push_B_tma_kernel x2 + push_E_tma_kernel", "achieved": yee_gbs,
+        yee_kernels = ("push_B_tma_kernel x2 + push_E_tma_kernel" if c1.get("yee_tma") else
+                       "push_B_kernel x2 + push_E_kernel (plain: the TMA tensor maps could not be built)")
+        roofline_yee = {"bound": "hbm", "kernel": yee_kernels, "achieved": yee_gbs,
                         "peak": hbm_peak, "peak_kind": hbm_kind, "unit": "GB/s", "frac": yee_gbs / hbm_peak,
                         "algorithmic_bytes_per_step": YEE_BYTES_PER_CELL * ncell,
                         "cell_updates_per_s": ncell / (yee_ms * 1e-3)}
@@ -372,6 +416,12 @@ def run_ours(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = time_oracle(args.config)
+        cpu["host"] = _host_info()
+        if args.config != 0:       # config 0 at full size as well (262,144 particles, order 1)
+            try:
+                cpu["config0_full_size"] = time_oracle(0, budget_s=6.0, max_steps=10)
+            except Exception as exc:
+                cpu["config0_full_size"] = {"error": str(exc)}
         try:
             cpu["all_cores"] = time_oracle_all_cores(args.config)
         except Exception as exc:      # a reported baseline, never a reason to lose the bench line

@@ -252,9 +252,70 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    values computed do not depend on the path beyond
  *                    summation order.  0 = a sorted species always runs the
  *                    fused kernel.  Ignored while force_path != 0.
+ *   "gather_variant" 0 (default) = the gather uses the same shape order n in every
+ *                    direction (reading R5); 1 = the "energy-conserving" gather:
+ *                    order n-1 along every direction in which the gathered
+ *                    component is staggered (
+ *                    oracle: ora_gather_variant).  Both particle kernels.
+ *   "smooth_passes"  k >= 0 (default 0, at most 16): after deposition and guard
+ *                    fold, each J component is filtered k times by the periodic
+ *                    binomial (1/4, 1/2, 1/4) stencil along x, then y, then z
+ *                    (NEXT-3; oracle: ora_smooth_binomial).  Not on a brick.
+ *   "open_mask"      bit d set = dimension d of this grid ends at faces shared
+ *                    with neighbouring bricks instead of wrapping onto itself
+ *                    (NEXT-1, below): particles are not wrapped along d, J guard
+ *                    layers along d are not folded, and pic_step is replaced by
+ *                    pic_step_stage plus the halo calls.  Default 0.
+ *   "id_base"        ids given by the next pic_load_particles start at this
+ *                    value (default 0), so that bricks can hand out disjoint ids.
  * Unknown name: PIC_EINVAL.
  */
 int pic_set_option(pic_ctx*, const char* name, long long value);
+
+/*
+ * ---- NEXT-1: brick decomposition -------
+ * Every brick is its own context over its own block of cells (xmin etc. of
+ * pic_init_grid are the brick's).  Along a dimension named in "open_mask" the
+ * NG = PIC_NG guard layers stand for the neighbour's cells.  One step of a brick
+ * is, in this order (paper_2303_12873_b200/bricks.py drives it):
+ *   pic_step_stage(0)   J := 0, gather + push + deposit, J fold along the periodic
+ *                       dimensions
+ *   J halos             pic_export_halo(2, d, side) -> neighbour's
+ *                       pic_import_halo(2, d, 1 - side): SUM into its interior
+ *   particles           pic_export_leavers / pic_import_arrivals per open
+ *                       dimension, one dimension after the other; then pic_sort
+ *   pic_step_stage(1)   first B half push;  B halos (group 1: copy into guards)
+ *   pic_step_stage(2)   E push;             E halos (group 0)
+ *   pic_step_stage(3)   second B half push; B halos; the step counter advances
+ * E and B halos are also exchanged once after pic_set_fields.  Exchanging the
+ * dimensions one after the other (planes cover the full padded extent of the
+ * other two dimensions) carries the edges and corners along.
+ *
+ * pic_halo_doubles: doubles of one halo message (three components, NG layers)
+ *   across a face normal to `dim`; -1 on a bad argument.
+ * pic_export_halo / pic_import_halo: group 0 = E, 1 = B, 2 = J; side 0 = the face
+ *   at the low end of `dim`, 1 = the high end; buf = DEVICE buffer of
+ *   pic_halo_doubles(dim) doubles, written / read on the context's stream.
+ *   E, B: export the NG interior layers next to the face, import into the guard
+ *   layers beyond it.  J: export the guard layers, import ADDS to the interior
+ *   layers.  PIC_EINVAL if the brick has fewer than NG cells along dim.
+ * pic_export_leavers: particles of `species` with position < min (side 0) or
+ *   >= max (side 1) along dim are removed from the container and written to
+ *   buf (DEVICE, 8 doubles each: x y z ux uy uz w and the id's bit pattern);
+ *   *count = how many.  PIC_ENOMEM (container unchanged) if more than
+ *   `capacity` leave.  Synchronises.  The species counts as unsorted afterwards.
+ * pic_import_arrivals: appends `count` such records, their positions shifted by
+ *   (shift_x, shift_y, shift_z) (the box length when the face is the periodic
+ *   seam of the whole domain, else 0).  PIC_ENOMEM if they do not fit np_max.
+ */
+int pic_step_stage(pic_ctx*, int stage);
+long long pic_halo_doubles(pic_ctx*, int dim);
+int pic_export_halo(pic_ctx*, int group, int dim, int side, double* buf_dev);
+int pic_import_halo(pic_ctx*, int group, int dim, int side, const double* buf_dev);
+int pic_export_leavers(pic_ctx*, int species, int dim, int side, double* buf_dev, long long capacity,
+                       long long* count /*host*/);
+int pic_import_arrivals(pic_ctx*, int species, const double* buf_dev, long long count, double shift_x,
+                        double shift_y, double shift_z);
 
 /* Wait for the context's stream; returns a pending PIC_EPHYS / PIC_ECUDA. */
 int pic_sync(pic_ctx*);

@@ -23,7 +23,8 @@ _CODE_NAMES = {0: "PIC_OK", -1: "PIC_EINVAL", -2: "PIC_ENOMEM", -3: "PIC_ECUDA",
 SYMBOLS = ("pic_query_arena", "pic_init_grid", "pic_set_fields", "pic_load_particles", "pic_step",
            "pic_sort", "pic_get_fields", "pic_get_particles", "pic_deposit_rho", "pic_get_cell_offsets",
            "pic_get_counters", "pic_get_stage_ms", "pic_set_option", "pic_sync", "pic_last_error",
-           "pic_destroy", "pic_version", "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
+           "pic_destroy", "pic_version", "pic_step_stage", "pic_halo_doubles", "pic_export_halo",
+           "pic_import_halo", "pic_export_leavers", "pic_import_arrivals", "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
 
 
 class PicError(RuntimeError):
@@ -67,6 +68,13 @@ def load_library(path: str | None = None):
     L.pic_set_option.argtypes = [vp, C.c_char_p, ll]
     L.pic_sync.argtypes = [vp]
     L.pic_destroy.argtypes = [vp]
+    L.pic_step_stage.argtypes = [vp, i]
+    L.pic_halo_doubles.argtypes = [vp, i]
+    L.pic_halo_doubles.restype = ll
+    L.pic_export_halo.argtypes = [vp, i, i, i, vp]
+    L.pic_import_halo.argtypes = [vp, i, i, i, vp]
+    L.pic_export_leavers.argtypes = [vp, i, i, i, vp, ll, C.POINTER(ll)]
+    L.pic_import_arrivals.argtypes = [vp, i, vp, ll, d, d, d]
     L.pic_probe_dfma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_dmma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
@@ -276,6 +284,38 @@ class Sim:
         v = list(arr)
         return {"fast": v[0], "slow": v[1], "global": v[2], "launches": v[3], "steps": v[4], "sorts": v[5],
                 "yee_tma": v[6], "fallbacks": v[7]}
+
+    # -- NEXT-1: brick calls (device buffers = torch.cuda float64 tensors) -------------------------
+    def step_stage(self, stage):
+        self._check(self._L.pic_step_stage(self._ctx, int(stage)), "pic_step_stage")
+
+    def halo_doubles(self, dim):
+        n = self._L.pic_halo_doubles(self._ctx, int(dim))
+        if n < 0:
+            raise PicError(PIC_EINVAL, "pic_halo_doubles")
+        return int(n)
+
+    def export_halo(self, group, dim, side, buf):
+        assert buf.is_cuda and buf.dtype == self._torch.float64 and buf.numel() >= self.halo_doubles(dim)
+        self._check(self._L.pic_export_halo(self._ctx, group, dim, side, C.c_void_p(buf.data_ptr())), "pic_export_halo")
+
+    def import_halo(self, group, dim, side, buf):
+        assert buf.is_cuda and buf.dtype == self._torch.float64 and buf.numel() >= self.halo_doubles(dim)
+        self._check(self._L.pic_import_halo(self._ctx, group, dim, side, C.c_void_p(buf.data_ptr())), "pic_import_halo")
+
+    def export_leavers(self, species, dim, side, buf):
+        """buf: torch.cuda float64 tensor of 8 * capacity entries.  Returns the number of records written."""
+        assert buf.is_cuda and buf.dtype == self._torch.float64
+        cnt = C.c_longlong(0)
+        self._check(self._L.pic_export_leavers(self._ctx, species, dim, side, C.c_void_p(buf.data_ptr()),
+                                               buf.numel() // 8, C.byref(cnt)), "pic_export_leavers")
+        return int(cnt.value)
+
+    def import_arrivals(self, species, buf, count, shift=(0.0, 0.0, 0.0)):
+        assert count == 0 or (buf.is_cuda and buf.dtype == self._torch.float64 and buf.numel() >= 8 * count)
+        self._check(self._L.pic_import_arrivals(self._ctx, species, C.c_void_p(buf.data_ptr()) if count else None,
+                                                int(count), float(shift[0]), float(shift[1]), float(shift[2])),
+                    "pic_import_arrivals")
 
     def set_option(self, name, value):
         self._check(self._L.pic_set_option(self._ctx, name.encode(), int(value)), "pic_set_option")

@@ -1,0 +1,131 @@
+// bricks.cu -- what one brick of a domain decomposition exchanges with its neighbours (SURVEY.md 8(e) and
+// 8(f) NEXT-1; the paper's weak scaling rests on a spatial decomposition with neighbour
+// exchange).  Each brick is an ordinary context of this library whose grid is its own block of cells; along a
+// decomposed dimension (Grid::open_mask) the brick's guard layers stand for the neighbour's cells instead of
+// periodic images of its own:
+//   E, B   the NG interior layers next to a face go to the neighbour's guard layers (copy)
+//   J      the NG guard layers beyond a face go to the neighbour's interior layers (sum)
+//   particles that left through a face travel as 8-double records and are appended to the neighbour's container
+// The kernels here only pack, unpack and partition; who talks to whom is the caller's schedule
+// (paper_2303_12873_b200/bricks.py), over NCCL send/recv, peer copies, or plain pointers on one GPU.
+#include "pic_internal.h"
+
+namespace pic {
+
+namespace {
+
+// extents of the plane spanned by the two dimensions other than `dim` (padded), and strides of all three
+struct PlaneGeom {
+    int n1, n2;              // padded extents of the two in-plane dimensions (lower dimension first)
+    long long s0, s1, s2;    // strides: along dim, along the two in-plane dimensions
+};
+
+__host__ __device__ inline PlaneGeom plane_geom(const Grid& g, int dim) {
+    PlaneGeom p;
+    const int ext[3] = {g.nx + 2 * NG, g.py, g.pz};
+    const long long str[3] = {1, g.sy, g.sz};
+    const int d1 = (dim == 0) ? 1 : 0, d2 = (dim == 2) ? 1 : 2;
+    p.n1 = ext[d1]; p.n2 = ext[d2];
+    p.s0 = str[dim]; p.s1 = str[d1]; p.s2 = str[d2];
+    return p;
+}
+
+// buf[l][v][u] <-> F at layer first_layer + l along dim (interior index, may be negative), in-plane padded (u, v)
+template <bool PACK, bool ADD>
+__global__ void halo_kernel(Grid g, PlaneGeom pg, double* F, int dim, int first_layer, double* buf) {
+    const int u = (int)(blockIdx.x * blockDim.x + threadIdx.x), v = (int)blockIdx.y, l = (int)blockIdx.z;
+    if (u >= pg.n1) return;
+    const long long o = pg.s0 * (long long)(first_layer + l + NG) + pg.s1 * u + pg.s2 * v;
+    const long long b = ((long long)l * pg.n2 + v) * pg.n1 + u;
+    if (PACK) buf[b] = F[o];
+    else if (ADD) F[o] += buf[b];
+    else F[o] = buf[b];
+}
+
+__global__ void split_leavers_kernel(Grid g, Particles src, Particles dst, long long n, int dim, int side, double* out,
+                                     long long capacity, unsigned long long* counters) {
+    const long long ip = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    bool leaves = false, valid = ip < n;
+    double v[7] = {0, 0, 0, 0, 0, 0, 0};
+    unsigned long long id = 0;
+    if (valid) {
+        v[0] = src.x[ip]; v[1] = src.y[ip]; v[2] = src.z[ip]; v[3] = src.ux[ip]; v[4] = src.uy[ip]; v[5] = src.uz[ip];
+        v[6] = src.w[ip];
+        id = src.id[ip];
+        const double pos = v[dim];
+        const double lo = (dim == 0) ? g.xmin : ((dim == 1) ? g.ymin : g.zmin);
+        const double hi = (dim == 0) ? g.xmax : ((dim == 1) ? g.ymax : g.zmax);
+        leaves = side ? (pos >= hi) : (pos < lo);
+    }
+    // one atomic per warp and destination; the order inside a warp is kept
+    const unsigned active = __activemask();
+    const unsigned m_leave = __ballot_sync(active, valid && leaves), m_stay = __ballot_sync(active, valid && !leaves);
+    unsigned long long base_l = 0, base_s = 0;
+    if (lane == __ffs(active) - 1) {
+        if (m_leave) base_l = atomicAdd(&counters[0], (unsigned long long)__popc(m_leave));
+        if (m_stay) base_s = atomicAdd(&counters[1], (unsigned long long)__popc(m_stay));
+    }
+    base_l = __shfl_sync(active, base_l, __ffs(active) - 1);
+    base_s = __shfl_sync(active, base_s, __ffs(active) - 1);
+    const unsigned below = (1u << lane) - 1u;
+    if (valid && leaves) {
+        const long long k = (long long)base_l + __popc(m_leave & below);
+        if (k < capacity) {
+            double* r = out + 8 * k;
+#pragma unroll
+            for (int a = 0; a < 7; ++a) r[a] = v[a];
+            r[7] = __longlong_as_double((long long)id);
+        }
+    } else if (valid) {
+        const long long k = (long long)base_s + __popc(m_stay & below);
+        dst.x[k] = v[0]; dst.y[k] = v[1]; dst.z[k] = v[2]; dst.ux[k] = v[3]; dst.uy[k] = v[4]; dst.uz[k] = v[5];
+        dst.w[k] = v[6];
+        dst.id[k] = id;
+    }
+}
+
+__global__ void append_arrivals_kernel(Particles dst, long long at, const double* in, long long count, double sx,
+                                       double sy, double sz) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    const double* r = in + 8 * k;
+    dst.x[at + k] = r[0] + sx; dst.y[at + k] = r[1] + sy; dst.z[at + k] = r[2] + sz;
+    dst.ux[at + k] = r[3]; dst.uy[at + k] = r[4]; dst.uz[at + k] = r[5];
+    dst.w[at + k] = r[6];
+    dst.id[at + k] = (unsigned long long)__double_as_longlong(r[7]);
+}
+
+}  // namespace
+
+long long halo_doubles(const Grid& g, int dim) {
+    const PlaneGeom pg = plane_geom(g, dim);
+    return (long long)NG * pg.n1 * pg.n2;
+}
+
+void launch_halo_pack(const Grid& g, const double* F, int dim, int first_layer, double* buf, cudaStream_t st) {
+    const PlaneGeom pg = plane_geom(g, dim);
+    dim3 bs(128, 1, 1), nb((pg.n1 + 127) / 128, pg.n2, NG);
+    halo_kernel<true, false><<<nb, bs, 0, st>>>(g, pg, const_cast<double*>(F), dim, first_layer, buf);
+}
+
+void launch_halo_unpack(const Grid& g, double* F, int dim, int first_layer, const double* buf, bool add, cudaStream_t st) {
+    const PlaneGeom pg = plane_geom(g, dim);
+    dim3 bs(128, 1, 1), nb((pg.n1 + 127) / 128, pg.n2, NG);
+    if (add) halo_kernel<false, true><<<nb, bs, 0, st>>>(g, pg, F, dim, first_layer, const_cast<double*>(buf));
+    else halo_kernel<false, false><<<nb, bs, 0, st>>>(g, pg, F, dim, first_layer, const_cast<double*>(buf));
+}
+
+void launch_split_leavers(const Grid& g, const Particles& src, const Particles& dst, long long n, int dim, int side,
+                          double* out, long long capacity, unsigned long long* counters, cudaStream_t st) {
+    if (n <= 0) return;
+    split_leavers_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g, src, dst, n, dim, side, out, capacity, counters);
+}
+
+void launch_append_arrivals(const Particles& dst, long long at, const double* in, long long count, double sx, double sy,
+                            double sz, cudaStream_t st) {
+    if (count <= 0) return;
+    append_arrivals_kernel<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(dst, at, in, count, sx, sy, sz);
+}
+
+}  // namespace pic

@@ -181,9 +181,9 @@ __device__ __forceinline__ void update_particle_global(const Grid& g, const Fiel
     if (!bad && q != 0.0) deposit_global<N>(g, f, xi, et, ze, xi1, et1, ze1, q * w, bad);
     if (bad) status->ephys = 1;
     // step 5: wrap and store
-    p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx);
-    p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly);
-    p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz);
+    p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx, g.open_mask & 1);
+    p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly, g.open_mask & 2);
+    p.z[ip] = wrap1(z1, g.zmin, g.zmax, g.Lz, g.open_mask & 4);
     p.ux[ip] = ux;
     p.uy[ip] = uy;
     p.uz[ip] = uz;

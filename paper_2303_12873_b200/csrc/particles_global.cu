@@ -76,52 +76,58 @@ __device__ __forceinline__ int first_image(int i, int n) {   // smallest i + a*n
     return i - a * n;
 }
 
-__global__ void fold_guards_kernel(Grid g, double* F) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    int j = blockIdx.y, k = blockIdx.z;
-    if (i >= g.nx) return;
-    const bool edge = i < NG || i >= g.nx - NG || j < NG || j >= g.ny - NG || k < NG || k >= g.nz - NG;
-    if (!edge) return;
-    double sum = 0.0;
-    for (int kk = first_image(k, g.nz); kk < g.nz + NG; kk += g.nz)
-        for (int jj = first_image(j, g.ny); jj < g.ny + NG; jj += g.ny)
-            for (int ii = first_image(i, g.nx); ii < g.nx + NG; ii += g.nx) sum += F[g.idx(ii, jj, kk)];
-    F[g.idx(i, j, k)] = sum;   // distinct threads own distinct interior cells; images are only read
+// Along an open dimension (brick face, NEXT-1) nothing is folded: the guard layers there belong to the
+// neighbouring brick and are handed over by pic_export_halo; the threads then also cover those guard layers,
+// so that the exported planes are already folded along the periodic dimensions.
+struct FoldRange {
+    int lo[3], n[3];       // thread index range per dimension: lo .. lo + n - 1
+};
+__host__ __device__ inline FoldRange fold_range(const Grid& g) {
+    FoldRange r;
+    const int nn[3] = {g.nx, g.ny, g.nz};
+    for (int d = 0; d < 3; ++d) {
+        const bool open = (g.open_mask >> d) & 1;
+        r.lo[d] = open ? -NG : 0;
+        r.n[d] = open ? nn[d] + 2 * NG : nn[d];
+    }
+    return r;
 }
 
-// NOTE: the fold reads guard images while other threads overwrite interior
-// cells; an interior cell is an image only of itself (|a| = 0), and it is read
-// by its own thread only, so there is no race.
-// the three J components in one launch (one thread per interior cell; only the edge cells do work)
-__global__ void fold_guards3_kernel(Grid g, double* F0, double* F1, double* F2) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    int j = blockIdx.y, k = blockIdx.z;
-    if (i >= g.nx) return;
-    const bool edge = i < NG || i >= g.nx - NG || j < NG || j >= g.ny - NG || k < NG || k >= g.nz - NG;
+template <int NF>
+__global__ void fold_guards_kernel(Grid g, FoldRange r, double* F0, double* F1, double* F2) {
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) + r.lo[0];
+    const int j = (int)blockIdx.y + r.lo[1], k = (int)blockIdx.z + r.lo[2];
+    if (i >= r.lo[0] + r.n[0]) return;
+    const bool ox = g.open_mask & 1, oy = g.open_mask & 2, oz = g.open_mask & 4;
+    const bool edge = (!ox && (i < NG || i >= g.nx - NG)) || (!oy && (j < NG || j >= g.ny - NG)) ||
+                      (!oz && (k < NG || k >= g.nz - NG));
     if (!edge) return;
     double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-    for (int kk = first_image(k, g.nz); kk < g.nz + NG; kk += g.nz)
-        for (int jj = first_image(j, g.ny); jj < g.ny + NG; jj += g.ny)
-            for (int ii = first_image(i, g.nx); ii < g.nx + NG; ii += g.nx) {
+    const int k0 = oz ? k : first_image(k, g.nz), k1 = oz ? k + 1 : g.nz + NG, kd = oz ? 1 : g.nz;
+    const int j0 = oy ? j : first_image(j, g.ny), j1 = oy ? j + 1 : g.ny + NG, jd = oy ? 1 : g.ny;
+    const int i0 = ox ? i : first_image(i, g.nx), i1 = ox ? i + 1 : g.nx + NG, id = ox ? 1 : g.nx;
+    for (int kk = k0; kk < k1; kk += kd)
+        for (int jj = j0; jj < j1; jj += jd)
+            for (int ii = i0; ii < i1; ii += id) {
                 const long long o = g.idx(ii, jj, kk);
                 s0 += F0[o];
-                s1 += F1[o];
-                s2 += F2[o];
+                if (NF == 3) { s1 += F1[o]; s2 += F2[o]; }
             }
     const long long o = g.idx(i, j, k);
-    F0[o] = s0;
-    F1[o] = s1;
-    F2[o] = s2;
+    F0[o] = s0;      // distinct threads own distinct cells; a cell is an image only of itself, images are only read
+    if (NF == 3) { F1[o] = s1; F2[o] = s2; }
 }
 
 void launch_fold_guards3(const Grid& g, double* F0, double* F1, double* F2, cudaStream_t st) {
-    dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
-    fold_guards3_kernel<<<nb, bs, 0, st>>>(g, F0, F1, F2);
+    const FoldRange r = fold_range(g);
+    dim3 bs(128, 1, 1), nb((r.n[0] + 127) / 128, r.n[1], r.n[2]);
+    fold_guards_kernel<3><<<nb, bs, 0, st>>>(g, r, F0, F1, F2);
 }
 
 void launch_fold_guards(const Grid& g, double* F, cudaStream_t st) {
-    dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, g.nz);
-    fold_guards_kernel<<<nb, bs, 0, st>>>(g, F);
+    const FoldRange r = fold_range(g);
+    dim3 bs(128, 1, 1), nb((r.n[0] + 127) / 128, r.n[1], r.n[2]);
+    fold_guards_kernel<1><<<nb, bs, 0, st>>>(g, r, F, nullptr, nullptr);
 }
 
 // ------------------------------------------------------- load validator ----
@@ -139,14 +145,14 @@ void launch_validate(const Grid& g, const Particles& p, long long n, DevStatus* 
     validate_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g, p, n, status);
 }
 
-__global__ void iota_kernel(unsigned long long* id, long long n) {
+__global__ void iota_kernel(unsigned long long* id, long long n, unsigned long long base) {
     long long ip = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (ip < n) id[ip] = (unsigned long long)ip;
+    if (ip < n) id[ip] = base + (unsigned long long)ip;
 }
 
-void launch_iota(unsigned long long* id, long long n, cudaStream_t st) {
+void launch_iota(unsigned long long* id, long long n, unsigned long long base, cudaStream_t st) {
     if (n <= 0) return;
-    iota_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(id, n);
+    iota_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(id, n, base);
 }
 
 }  // namespace pic

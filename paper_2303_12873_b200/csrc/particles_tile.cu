@@ -61,6 +61,7 @@ struct TileCfg {
     static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NP = NP_, NW = 2 * NP_, NT = 32 * NW, MINB = MINB_,
                          DRIFT = DRIFT_;
     static constexpr bool UG = UG_;               // gather on cell-anchored windows (see gather6_cell)
+    static constexpr unsigned POLL_NS = 800;      // consumer's poll interval while its producer is still staging the row
     static constexpr int NROW = TY * TZ;
     // gather stencil: nodes i-2 .. i+2 of a particle in cell i (every order, every staggering)
     static constexpr int GL = 2 + DRIFT;
@@ -721,7 +722,7 @@ __device__ __forceinline__ void tile_consumer(const Grid& g, const Fields& f, co
             for (;;) {
                 staged = ld_acquire(S.flags);
                 if (staged >= row_end || (staged + 32 - b_lo > C::RING && staged < T)) break;
-                __nanosleep(64);
+                __nanosleep(C::POLL_NS);      // a sub-chunk takes the producer ~6 us: polling faster only burns issue slots
             }
             const bool full_row = staged >= row_end;
             const int b_hi = full_row ? row_end : staged;
@@ -863,8 +864,8 @@ __device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, co
             const bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1)) || !(fabs(xi1 - xi) < 1.0) ||
                              !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
             bad_any = bad_any || bad;
-            const double xw = wrap1(x1, g.xmin, g.xmax, g.Lx), yw = wrap1(y1, g.ymin, g.ymax, g.Ly),
-                         zw = wrap1(z1, g.zmin, g.zmax, g.Lz);
+            const double xw = wrap1(x1, g.xmin, g.xmax, g.Lx, g.open_mask & 1), yw = wrap1(y1, g.ymin, g.ymax, g.Ly, g.open_mask & 2),
+                         zw = wrap1(z1, g.zmin, g.zmax, g.Lz, g.open_mask & 4);
             po.x[ip] = xw;
             po.y[ip] = yw;
             po.z[ip] = zw;

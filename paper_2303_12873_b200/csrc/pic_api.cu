@@ -70,6 +70,7 @@ struct pic_ctx {
     // options
     int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1, fuse_keys = 1;
     int gather_variant = 0, smooth_passes = 0;      // NEXT-3 options
+    unsigned long long id_base = 0;                 // ids given at load start here (bricks: unique across contexts)
     YeeMaps yee_maps{};
     int device = 0;                     // ordinal of the device the arena lives on; made current by every call
     int yee_tma_ok = 0;                 // tensor maps built: the TMA-staged Yee kernels are available
@@ -327,6 +328,7 @@ int pic_init_grid(pic_ctx** out, int nx, int ny, int nz, double dx, double dy, d
     g.Lx = nx * dx; g.Ly = ny * dy; g.Lz = nz * dz;
     g.xmax = xmin + g.Lx; g.ymax = ymin + g.Ly; g.zmax = zmin + g.Lz;
     g.dt = dt;
+    g.open_mask = 0;
     c->order = order;
     c->nspecies = nspecies;
     c->stream = (cudaStream_t)cuda_stream;
@@ -417,7 +419,7 @@ int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n,
     const cudaMemcpyKind kind = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     for (int a = 0; a < 7 && n > 0; ++a)
         CU(c, cudaMemcpyAsync(dst[a], src[a], (size_t)n * sizeof(double), kind, c->stream));
-    launch_iota(P.id, n, c->stream);
+    launch_iota(P.id, n, c->id_base, c->stream);
     launch_validate(c->g, P, n, c->status, c->stream);
     c->launches += (n > 0) ? 2 : 0;
     CU(c, cudaGetLastError());
@@ -437,8 +439,9 @@ int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n,
     return PIC_OK;
 }
 
-int pic_step(pic_ctx* c, int nsteps) {
-    ENTER(c);
+// mask: bit 0 = J := 0, particles, J fold (and smoothing); bit 1 = first B half push; bit 2 = E push;
+// bit 3 = second B half push (ends the step).  pic_step runs all four; pic_step_stage one at a time (bricks).
+static int step_impl(pic_ctx* c, int nsteps, int mask) {
     if (nsteps < 0) return fail(c, PIC_EINVAL, "nsteps < 0");
     bool any = false;
     for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
@@ -447,7 +450,7 @@ int pic_step(pic_ctx* c, int nsteps) {
         for (int s = 0; s < c->nspecies; ++s)
             if (c->sp[s].loaded && !c->sp[s].sorted)
                 return fail(c, PIC_ESTATE, "force_path=2 needs pic_sort before pic_step (species %d)", s);
-    const bool timing = c->stage_timing != 0;
+    const bool timing = c->stage_timing != 0 && mask == 15;
     const Grid& g = c->g;
     const size_t comp_bytes = (size_t)g.npad * sizeof(double);
     const YeeMaps* tma_B = ((c->yee_tma & 1) && c->yee_tma_ok) ? &c->yee_maps : nullptr;
@@ -462,6 +465,7 @@ int pic_step(pic_ctx* c, int nsteps) {
             cudaEventRecord(ev[0], c->stream);
         }
         nvtxRangePushA("pic_step");
+        if (mask & 1) {
         // J := 0 (R13).  Jx,Jy,Jz are contiguous in the arena.
         nvtxRangePushA("zero_J");
         if (c->f.Jx < c->f.Jy && c->f.Jy < c->f.Jz) {     // one memset over the three components (and the alignment gaps)
@@ -530,22 +534,136 @@ int pic_step(pic_ctx* c, int nsteps) {
             for (int k = 0; k < 3; ++k) c->launches += launch_smooth_binomial(g, J[k], c->tmp, c->smooth_passes, c->stream);
         }
         nvtxRangePop();
+        }      // mask & 1
         if (timing) cudaEventRecord(ev[3], c->stream);
         // steps 6-8
         nvtxRangePushA("yee");
-        launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
+        if (mask & 2) { launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream); c->launches += 1; }
         if (timing) cudaEventRecord(ev[4], c->stream);
-        launch_push_E(g, c->f, g.dt, tma_E, c->stream);
+        if (mask & 4) { launch_push_E(g, c->f, g.dt, tma_E, c->stream); c->launches += 1; }
         if (timing) cudaEventRecord(ev[5], c->stream);
-        launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
+        if (mask & 8) {
+            launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
+            c->launches += 1;
+            c->steps += 1;
+        }
         nvtxRangePop();
-        c->launches += 3;
-        c->steps += 1;
         if (timing) cudaEventRecord(ev[6], c->stream);
         nvtxRangePop();
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_step launch");
+    return PIC_OK;
+}
+
+int pic_step(pic_ctx* c, int nsteps) {
+    ENTER(c);
+    if (c->g.open_mask) return fail(c, PIC_ESTATE, "a brick (open_mask != 0) is stepped with pic_step_stage and the halo calls");
+    return step_impl(c, nsteps, 15);
+}
+
+int pic_step_stage(pic_ctx* c, int stage) {
+    ENTER(c);
+    if (stage < 0 || stage > 3) return fail(c, PIC_EINVAL, "stage must be 0 .. 3");
+    if (c->smooth_passes > 0 && c->g.open_mask) return fail(c, PIC_ESTATE, "smooth_passes is not available on a brick");
+    return step_impl(c, 1, 1 << stage);
+}
+
+// ---- NEXT-1: what a brick hands to its neighbours (bricks.cu) ------------------------------------------
+long long pic_halo_doubles(pic_ctx* c, int dim) {
+    if (!c || dim < 0 || dim > 2) return -1;
+    return 3 * halo_doubles(c->g, dim);
+}
+
+static int halo_args(pic_ctx* c, int group, int dim, int side, const void* buf) {
+    if (group < 0 || group > 2 || dim < 0 || dim > 2 || side < 0 || side > 1 || !buf)
+        return fail(c, PIC_EINVAL, "bad halo group, dim, side or buffer");
+    const int n = (dim == 0) ? c->g.nx : ((dim == 1) ? c->g.ny : c->g.nz);
+    if (n < NG) return fail(c, PIC_EINVAL, "a brick needs at least %d cells along an exchanged dimension", NG);
+    return PIC_OK;
+}
+
+int pic_export_halo(pic_ctx* c, int group, int dim, int side, double* buf_dev) {
+    ENTER(c);
+    int rc = halo_args(c, group, dim, side, buf_dev);
+    if (rc != PIC_OK) return rc;
+    const Grid& g = c->g;
+    double* F[3][3] = {{c->f.Ex, c->f.Ey, c->f.Ez}, {c->f.Bx, c->f.By, c->f.Bz}, {c->f.Jx, c->f.Jy, c->f.Jz}};
+    const int n = (dim == 0) ? g.nx : ((dim == 1) ? g.ny : g.nz);
+    // E, B: the interior layers next to the face; J: the guard layers beyond it
+    const int first = (group == 2) ? (side ? n : -NG) : (side ? n - NG : 0);
+    const long long per = halo_doubles(g, dim);
+    for (int k = 0; k < 3; ++k) launch_halo_pack(g, F[group][k], dim, first, buf_dev + k * per, c->stream);
+    c->launches += 3;
+    CU(c, cudaGetLastError());
+    return PIC_OK;
+}
+
+int pic_import_halo(pic_ctx* c, int group, int dim, int side, const double* buf_dev) {
+    ENTER(c);
+    int rc = halo_args(c, group, dim, side, buf_dev);
+    if (rc != PIC_OK) return rc;
+    const Grid& g = c->g;
+    double* F[3][3] = {{c->f.Ex, c->f.Ey, c->f.Ez}, {c->f.Bx, c->f.By, c->f.Bz}, {c->f.Jx, c->f.Jy, c->f.Jz}};
+    const int n = (dim == 0) ? g.nx : ((dim == 1) ? g.ny : g.nz);
+    // E, B: into the guard layers beyond the face; J: ADDED to the interior layers next to it
+    const int first = (group == 2) ? (side ? n - NG : 0) : (side ? n : -NG);
+    const long long per = halo_doubles(g, dim);
+    for (int k = 0; k < 3; ++k)
+        launch_halo_unpack(g, F[group][k], dim, first, buf_dev + k * per, group == 2, c->stream);
+    c->launches += 3;
+    CU(c, cudaGetLastError());
+    return PIC_OK;
+}
+
+int pic_export_leavers(pic_ctx* c, int species, int dim, int side, double* buf_dev, long long capacity,
+                       long long* count) {
+    ENTER(c);
+    if (species < 0 || species >= c->nspecies || dim < 0 || dim > 2 || side < 0 || side > 1 || !count ||
+        capacity < 0 || (capacity > 0 && !buf_dev))
+        return fail(c, PIC_EINVAL, "bad argument of pic_export_leavers");
+    Species& S = c->sp[species];
+    *count = 0;
+    if (!S.loaded || S.n == 0) return PIC_OK;
+    materialize(c, S);
+    // two 64-bit counters in the unused half of the 256-byte status block
+    unsigned long long* counters = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(c->status) + 128);
+    CU(c, cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), c->stream));
+    launch_split_leavers(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, dim, side, buf_dev, capacity, counters, c->stream);
+    c->launches += 1;
+    unsigned long long h[2];
+    CU(c, cudaMemcpyAsync(h, counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if ((long long)h[0] > capacity)      // nothing was lost: the source buffer is still the current one
+        return fail(c, PIC_ENOMEM, "%llu particles leave through this face, the buffer holds %lld", h[0], capacity);
+    if (h[0] + h[1] != (unsigned long long)S.n) return fail(c, PIC_ECUDA, "leaver split lost particles");
+    *count = (long long)h[0];
+    if (h[0] > 0) {
+        S.cur ^= 1;
+        S.n = (long long)h[1];
+        S.sorted = false;
+        S.keys_valid = false;
+        S.degraded = false;
+    }
+    return PIC_OK;
+}
+
+int pic_import_arrivals(pic_ctx* c, int species, const double* buf_dev, long long count, double shift_x, double shift_y,
+                        double shift_z) {
+    ENTER(c);
+    if (species < 0 || species >= c->nspecies || count < 0 || (count > 0 && !buf_dev))
+        return fail(c, PIC_EINVAL, "bad argument of pic_import_arrivals");
+    Species& S = c->sp[species];
+    if (!S.loaded) return fail(c, PIC_ESTATE, "species %d was never loaded (load it, empty if need be, to set q and m)", species);
+    if (count == 0) return PIC_OK;
+    if (S.n + count > S.np_max) return fail(c, PIC_ENOMEM, "%lld arrivals do not fit: n = %lld, np_max = %lld", count, S.n, S.np_max);
+    materialize(c, S);
+    launch_append_arrivals(S.buf[S.cur], S.n, buf_dev, count, shift_x, shift_y, shift_z, c->stream);
+    c->launches += 1;
+    S.n += count;
+    S.sorted = false;
+    S.keys_valid = false;
+    CU(c, cudaGetLastError());
     return PIC_OK;
 }
 
@@ -717,7 +835,13 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     else if (!strcmp(name, "sort_deferred")) c->sort_deferred = value != 0;
     else if (!strcmp(name, "fuse_keys")) c->fuse_keys = value != 0;
     else if (!strcmp(name, "drift_watch")) c->drift_watch = value != 0;
-    else if (!strcmp(name, "gather_variant")) {
+    else if (!strcmp(name, "open_mask")) {
+        if (value < 0 || value > 7) return fail(c, PIC_EINVAL, "open_mask must be 0 .. 7");
+        c->g.open_mask = (int)value;
+    } else if (!strcmp(name, "id_base")) {
+        if (value < 0) return fail(c, PIC_EINVAL, "id_base must be >= 0");
+        c->id_base = (unsigned long long)value;
+    } else if (!strcmp(name, "gather_variant")) {
         if (value < 0 || value > 1) return fail(c, PIC_EINVAL, "gather_variant must be 0 or 1");
         c->gather_variant = (int)value;
     } else if (!strcmp(name, "smooth_passes")) {

@@ -27,6 +27,7 @@ struct Grid {
     double xmax, ymax, zmax;         // xmin + nx*dx
     double Lx, Ly, Lz;               // nx*dx
     double dt;
+    int open_mask;                   // bit d set: dimension d is a brick face (NEXT-1), not a periodic boundary of this grid
     __host__ __device__ inline long long idx(int i, int j, int k) const {   // interior cell index -> padded offset
         return (long long)(i + NG) + sy * (long long)(j + NG) + sz * (long long)(k + NG);
     }
@@ -76,7 +77,21 @@ void launch_deposit_rho(const Grid& g, const Particles& p, long long n, double q
 void launch_fold_guards(const Grid& g, double* F, cudaStream_t st);       // sum periodic images into the interior
 void launch_fold_guards3(const Grid& g, double* F0, double* F1, double* F2, cudaStream_t st);   // three components, one launch
 void launch_validate(const Grid& g, const Particles& p, long long n, DevStatus* status, cudaStream_t st);
-void launch_iota(unsigned long long* id, long long n, cudaStream_t st);
+void launch_iota(unsigned long long* id, long long n, unsigned long long base, cudaStream_t st);
+
+// ---- bricks.cu (NEXT-1: brick decomposition) ----------------------------------
+// Halo planes of a group of three components across face (dim, side): E and B export their NG interior
+// boundary layers and import into the guard layers; J exports its guard layers and import ADDS them to
+// the interior boundary layers.  A plane covers the full padded extent of the other two dimensions.
+long long halo_doubles(const Grid& g, int dim);                    // per component and side
+void launch_halo_pack(const Grid& g, const double* F, int dim, int first_layer, double* buf, cudaStream_t st);
+void launch_halo_unpack(const Grid& g, double* F, int dim, int first_layer, const double* buf, bool add, cudaStream_t st);
+// leavers of face (dim, side) -> out[8 * k .. 8 * k + 7] = x y z ux uy uz w id; everything else -> dst (compacted);
+// counters[0] = leavers, counters[1] = stayers (device, zeroed by the caller)
+void launch_split_leavers(const Grid& g, const Particles& src, const Particles& dst, long long n, int dim, int side,
+                          double* out, long long capacity, unsigned long long* counters, cudaStream_t st);
+void launch_append_arrivals(const Particles& dst, long long at, const double* in, long long count, double sx, double sy,
+                            double sz, cudaStream_t st);
 
 // ---- sort.cu ----------------------------------------------------------------
 // scratch: key[n] u32, rank[n] u32, block_sums[...] u32

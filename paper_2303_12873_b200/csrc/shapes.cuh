@@ -73,8 +73,10 @@ __device__ __forceinline__ double dt_over_gamma(double dt, double inv_c2, double
     return dt * rsqrt(1.0 + (ux * ux + uy * uy + uz * uz) * inv_c2);
 }
 
-// One periodic wrap.
-__device__ __forceinline__ double wrap1(double v, double lo, double hi, double L) {
+// One periodic wrap.  open = this dimension is a brick face: the particle keeps its
+// unwrapped position and is handed to the neighbouring brick by pic_export_leavers (NEXT-1).
+__device__ __forceinline__ double wrap1(double v, double lo, double hi, double L, bool open = false) {
+    if (open) return v;
     if (v >= hi) v = v - L;
     else if (v < lo) v = v + L;
     if (v == hi) v = lo;
