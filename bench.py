@@ -87,12 +87,14 @@ def _host_info():
     return {"nproc": os.cpu_count(), "cpu_model": model}
 
 
-def _pin_to_one_core():
-    """taskset-style pinning of this process to one core; returns the core or None."""
+def _pin_to_one_core(which=-1):
+    """taskset-style pinning of this process to one core: the which-th of the cores it may run
+    on; returns (core, previous affinity) or (None, None)."""
     try:
         cores = sorted(os.sched_getaffinity(0))
-        os.sched_setaffinity(0, {cores[-1]})
-        return cores[-1], set(cores)
+        core = cores[which % len(cores)]
+        os.sched_setaffinity(0, {core})
+        return core, set(cores)
     except Exception:
         return None, None
 
@@ -181,11 +183,11 @@ def _oracle_sim(wl):
     return o
 
 
-def time_oracle(index: int, budget_s: float = 12.0, max_steps: int = 40):
-    """particle-updates/s of the oracle as it stands, single-threaded, on the host."""
+def time_oracle(index: int, budget_s: float = 12.0, max_steps: int = 40, core_index: int = -1):
+    """particle-updates/s of the oracle as it stands, single-threaded, pinned to one host core."""
     wl, desc = _oracle_sample(index)
     o = _oracle_sim(wl)
-    core, before = _pin_to_one_core()
+    core, before = _pin_to_one_core(core_index)
     try:
         o.step(1)                                   # warm-up (page in, build tables)
         t0 = time.perf_counter()
@@ -208,7 +210,8 @@ def time_oracle_all_cores(index: int, budget_s: float = 8.0):
     ncores = os.cpu_count() or 1
     cmd = [sys.executable, os.path.abspath(__file__), "--oracle-worker", "--config", str(index),
            "--oracle-budget", str(budget_s)]
-    procs = [subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True) for _ in range(ncores)]
+    procs = [subprocess.Popen(cmd + ["--oracle-core", str(k)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+             for k in range(ncores)]          # replica k pinned to core k
     total, ok = 0.0, 0
     for pr in procs:
         try:
@@ -283,6 +286,11 @@ def run_ours(args):
     npart, ncell = wl.nparticles, wl.ncell
 
     sim = Sim.from_workload(wl, device="cuda:%d" % local)
+    options = {}
+    for kv in args.option:
+        name, _, val = kv.partition("=")
+        options[name] = int(val)
+        sim.set_option(name, int(val))
     sim.sort()
     sim.sync()
 
@@ -388,6 +396,8 @@ def run_ours(args):
         del sim
         torch.cuda.empty_cache()
         sim = Sim.from_workload(wl, device="cuda:%d" % local, load=False)
+        for name, val in options.items():
+            sim.set_option(name, val)
         if wl.fields:
             sim.set_fields(**wl.fields)
 
@@ -437,7 +447,7 @@ def run_ours(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "configs[%d]" % args.config, "name": wl.name,
                        "grid": [wl.nx, wl.ny, wl.nz], "particles": npart, "species": len(wl.species),
-                       "order": wl.order, "sort_every": sort_every, "replicas": world,
+                       "order": wl.order, "sort_every": sort_every, "replicas": world, "options": options,
                        "l2": "inputs larger than L2 (%.1f GB of particles + fields per step)" % (
                            (BYTES_PER_PARTICLE * npart + 9 * 8 * ncell) / 1e9),
                        "generation_s": round(t_gen, 1)},
@@ -462,11 +472,14 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--sort-every", type=int, default=None, help="override the workload's sort cadence (steps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
+                    help="pic_set_option(NAME, VALUE) before the run (experiments: force_path=1, gather_variant=1, ...)")
     ap.add_argument("--oracle-worker", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--oracle-budget", type=float, default=8.0, help=argparse.SUPPRESS)
+    ap.add_argument("--oracle-core", type=int, default=-1, help=argparse.SUPPRESS)
     args = ap.parse_args()
     if args.oracle_worker:      # one replica of the all-cores oracle baseline (no CUDA, no torch)
-        print(json.dumps(time_oracle(args.config, budget_s=args.oracle_budget)))
+        print(json.dumps(time_oracle(args.config, budget_s=args.oracle_budget, core_index=args.oracle_core)))
         return 0
     if args.warmup < 3:
         args.warmup = 3

@@ -160,7 +160,7 @@ def _laser_fields(nx, ny, nz, dx, dy, dz, a0, lam, w0, ctau, z0):
     return out
 
 
-def lwfa_box(nx=128, ny=128, nz=1024, seed=SEED0 + 3, nsteps=500, order=3, sort_every=4, shuffle=False):
+def lwfa_box(nx=128, ny=128, nz=1024, seed=SEED0 + 3, nsteps=500, order=3, sort_every=1, shuffle=False):
     """Config 3 (readings R31-R34): 128x128x1024, dz = lambda/32, dx = dy = 4 dz,
     2 ppc cold electrons, linear ramp over cells 600-700, flat to cell 1000;
     Gaussian pulse a0 = 2, w0 = 8 um, 30 fs FWHM centred at cell 400.  ``nx, ny``
@@ -192,7 +192,7 @@ def lwfa_box(nx=128, ny=128, nz=1024, seed=SEED0 + 3, nsteps=500, order=3, sort_
                     fields)
 
 
-def plasma_mirror(nx=256, ny=256, nz=512, seed=SEED0 + 4, nsteps=200, order=3, sort_every=4, shuffle=False):
+def plasma_mirror(nx=256, ny=256, nz=512, seed=SEED0 + 4, nsteps=200, order=3, sort_every=1, shuffle=False):
     """Config 4 (reading R35): dx = lambda/64, slab of 30 n_c over cells 400-464,
     exponential pre-plasma (L = lambda/10 = 6.4 cells) over cells 368-400,
     electrons 16 ppc (u_th = 0.005 c), protons 4 ppc (cold); plane-wave pulse

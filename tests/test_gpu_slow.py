@@ -217,8 +217,9 @@ def _full_size_sampled(ora, Sim, wl, fields, block0, nsample=2048, bw=10, mg=3):
     g.step(1)
     J = g.get_fields(names=("Jx", "Jy", "Jz"), device=True)
     og = ora.make_grid(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz)
-    E = tuple(fields[n] for n in ("Ex", "Ey", "Ez"))
-    B = tuple(fields[n] for n in ("Bx", "By", "Bz"))
+    zero = np.zeros(wl.ncell)                          # a laser config sets only some of the components
+    E = tuple(fields.get(n, zero) for n in ("Ex", "Ey", "Ez"))
+    B = tuple(fields.get(n, zero) for n in ("Bx", "By", "Bz"))
     Ld = (wl.nx * wl.dx, wl.ny * wl.dy, wl.nz * wl.dz)
     rng = np.random.default_rng(1234)
     Jo = [np.zeros(wl.ncell) for _ in range(3)]
