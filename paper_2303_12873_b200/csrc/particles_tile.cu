@@ -6,11 +6,16 @@
 // One thread block owns a tile of TX x TY x TZ cells; its E,B stencil (+ halo
 // for the shape support and DRIFT cells of drift since the last pic_sort) is
 // staged in shared memory once.  After that the block's warps run without any
-// block-wide barrier.  A warp owns RPW consecutive x-rows of the tile; their
-// cells, in order, form the warp's STREAM: cell c occupies the stream positions
-// cp[c] .. cp[c] + n_c - 1, padded to an even length (so that the two lanes of
-// an aligned lane pair always work on particles of the same cell).
-//   phase A  lane <-> stream position, 32 consecutive positions at a time,
+// block-wide barrier, as NP producer / consumer PAIRS: a producer warp runs
+// phase A, its consumer warp phase B and the flush, concurrently, on a per-pair
+// staging ring in shared memory handed over with st.release / ld.acquire
+// counters (positions staged, positions consumed).  Neither role keeps the
+// other's registers alive: 168 registers and 12 warps per SM instead of 255 and 8.
+// A producer owns RPW consecutive x-rows of the tile; their cells, in order,
+// form its STREAM: cell c occupies the stream positions cp[c] .. cp[c] + n_c - 1
+// (padded to an even length when TileCfg::UG, so that the two lanes of an
+// aligned lane pair always work on particles of the same cell).
+//   phase A  (producer) lane <-> stream position, 32 consecutive positions at a time,
 //            ACROSS row boundaries (the lanes stay full: a row of 64 +- 8
 //            particles no longer ends in a nearly empty sub-chunk).  The
 //            particle data of a sub-chunk are copied into a per-warp landing
@@ -23,14 +28,14 @@
 //            differences on the cell's window to slot (position mod RING) of a
 //            per-warp staging ring: 18 doubles (the last entry of each set
 //            follows from sum S = 1, sum DS = 0) + (q w / dt, e) + a code.
-//   phase B  runs as soon as a whole row is staged (or the ring is full):
+//   phase B  (consumer) runs as soon as a whole row is staged (or the ring is full):
 //            lane <-> (cell q of the row, plane s of that cell's window).  The
 //            four lanes of a cell walk the cell's staged particles and
 //            accumulate the Esirkepov window of the CELL in registers
 //            (3 x 12 accumulators per lane at order 3), so the per-particle
 //            cost is FMAs and shared-memory loads, not atomics.
 //   slow     a particle that crossed several faces or is not in its listed
-//            cell stages its positions and is deposited by the whole warp: its
+//            cell stages its positions and is deposited by the whole producer warp: its
 //            (N+2)^3 window is spread over the lanes, one global RED.ADD.F64
 //            per non-zero point.
 //   flush    at the end of a row the lanes add up, with shuffles, what lands on
