@@ -203,38 +203,115 @@ class _Species:
 
 class OracleSim:
     """The PIC cycle of SURVEY.md 8(c.1), steps 1-8, on host arrays.  Mirrors
-    the method names of the CUDA binding so one test can drive both."""
+    the method names of the CUDA binding so one test can drive both.
+
+    ``open_z`` (NEXT-2: non-periodic longitudinal boundary, moving window, antenna): the box ends at
+    z = zmin and z = zmin + nz dz; every field value with a z index outside 0 .. nz-1 IS ZERO at all times, current
+    deposited there is dropped, and a particle that leaves through a z face is deleted after it has deposited.
+    It is written with the periodic functions above, unchanged, on arrays that carry ``ZPAD`` extra planes at either
+    end: the extra planes are forced back to zero after every operation that writes them, and they are wide enough
+    (4 >= the reach of every stencil) that the periodic seam between them is never felt."""
+
+    ZPAD = 4
 
     def __init__(self, nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, dt, order, nspecies, gather_variant=0,
-                 smooth_passes=0):
-        self.g = make_grid(nx, ny, nz, dx, dy, dz, xmin, ymin, zmin)
+                 smooth_passes=0, open_z=False):
+        self.open_z = bool(open_z)
+        self.nz_phys = int(nz)
+        self.pad = self.ZPAD if self.open_z else 0
+        self.g = make_grid(nx, ny, nz + 2 * self.pad, dx, dy, dz, xmin, ymin, zmin - self.pad * dz)
         if gather_variant not in (0, 1) or smooth_passes < 0:
             raise ValueError("gather_variant must be 0 or 1, smooth_passes >= 0")
+        if self.open_z and smooth_passes:
+            raise ValueError("smoothing is periodic: not with open_z")
         self.gather_variant, self.smooth_passes = int(gather_variant), int(smooth_passes)   # NEXT-3 options
         if order not in (1, 2, 3):
             raise ValueError("order must be 1, 2 or 3")
         if not (0.0 < dt <= courant_dt(self.g)):
             raise ValueError("dt outside (0, Courant limit]")
         self.dt, self.order = float(dt), int(order)
-        self.ncell = nx * ny * nz
-        self.E = [np.zeros(self.ncell) for _ in range(3)]
-        self.B = [np.zeros(self.ncell) for _ in range(3)]
-        self.J = [np.zeros(self.ncell) for _ in range(3)]
+        self.nx, self.ny = int(nx), int(ny)
+        self.ncell = nx * ny * nz                          # physical cells
+        self.ncell_all = nx * ny * (nz + 2 * self.pad)
+        self.E = [np.zeros(self.ncell_all) for _ in range(3)]
+        self.B = [np.zeros(self.ncell_all) for _ in range(3)]
+        self.J = [np.zeros(self.ncell_all) for _ in range(3)]
         self.species: list[_Species | None] = [None] * nspecies
         self.cell_offset: list[np.ndarray | None] = [None] * nspecies
+        self.plane_sources = []                            # (component index 0..2 of J, plane k, values) for the next step
+        self.deleted = 0
+
+    # ---- open-z helpers ------------------------------------------------------------------------------------
+    def _phys(self, a):
+        """View of the physical planes of a padded flat array."""
+        nz_all = self.nz_phys + 2 * self.pad
+        return a.reshape(nz_all, self.ny, self.nx)[self.pad:self.pad + self.nz_phys]
+
+    def _zero_pads(self, arrays):
+        if not self.open_z:
+            return
+        nz_all = self.nz_phys + 2 * self.pad
+        for a in arrays:
+            v = a.reshape(nz_all, self.ny, self.nx)
+            v[:self.pad] = 0.0
+            v[self.pad + self.nz_phys:] = 0.0
+
+    @property
+    def zmin(self):
+        return self.g.zmin + self.pad * self.g.dz
+
+    def _delete_outside_z(self):
+        lo, hi = self.zmin, self.zmin + self.nz_phys * self.g.dz
+        for sp in self.species:
+            if sp is None or sp.x.size == 0:
+                continue
+            keep = (sp.z >= lo) & (sp.z < hi)
+            if not keep.all():
+                self.deleted += int((~keep).sum())
+                for name in ("x", "y", "z", "ux", "uy", "uz", "w", "id"):
+                    setattr(sp, name, np.ascontiguousarray(getattr(sp, name)[keep]))
 
     def set_fields(self, Ex=None, Ey=None, Ez=None, Bx=None, By=None, Bz=None):
         for dst, src in zip(self.E + self.B, (Ex, Ey, Ez, Bx, By, Bz)):
-            dst[:] = 0.0 if src is None else np.asarray(src, dtype=np.float64).reshape(-1)
+            dst[:] = 0.0
+            if src is not None:
+                self._phys(dst)[...] = np.asarray(src, dtype=np.float64).reshape(self.nz_phys, self.ny, self.nx)
 
-    def load_particles(self, s, q, m, x, y, z, ux, uy, uz, w):
+    def load_particles(self, s, q, m, x, y, z, ux, uy, uz, w, id_base=0):
         sp = _Species()
         sp.q, sp.m = float(q), float(m)
         for name, a in zip(("x", "y", "z", "ux", "uy", "uz", "w"), (x, y, z, ux, uy, uz, w)):
             setattr(sp, name, np.array(a, dtype=np.float64, copy=True).reshape(-1))
-        sp.id = np.arange(sp.x.size, dtype=np.uint64)
+        sp.id = np.arange(sp.x.size, dtype=np.uint64) + np.uint64(id_base)
         self.species[s] = sp
         self.cell_offset[s] = None
+
+    def append_particles(self, s, x, y, z, ux, uy, uz, w, ids):
+        """NEXT-2: fresh plasma entering a moving window (the caller draws it)."""
+        sp = self.species[s]
+        for name, a in zip(("x", "y", "z", "ux", "uy", "uz", "w"), (x, y, z, ux, uy, uz, w)):
+            setattr(sp, name, np.concatenate([getattr(sp, name), np.asarray(a, dtype=np.float64).reshape(-1)]))
+        sp.id = np.concatenate([sp.id, np.asarray(ids, dtype=np.uint64).reshape(-1)])
+        self.cell_offset[s] = None
+
+    def add_plane_source(self, comp, k, values):
+        """NEXT-2 antenna: J_comp[:, :, k] += values in the NEXT step, after deposition and before the E push
+        (comp = 0, 1, 2 for Jx, Jy, Jz; values = ny x nx array, x fastest)."""
+        self.plane_sources.append((int(comp), int(k), np.asarray(values, dtype=np.float64).reshape(self.ny, self.nx).copy()))
+
+    def shift_window(self, ncells=1):
+        """NEXT-2 moving window: the box moves up by ncells cells along z.  Field index k now names what was
+        k + ncells, the top ncells planes are new (zero), particles below the new zmin are deleted."""
+        if not self.open_z:
+            raise ValueError("a moving window needs open_z")
+        n = int(ncells)
+        for a in self.E + self.B + self.J:
+            v = self._phys(a)
+            v[:self.nz_phys - n] = v[n:].copy()
+            v[self.nz_phys - n:] = 0.0
+        self.g.zmin = self.g.zmin + n * self.g.dz
+        self._delete_outside_z()
+        self.cell_offset = [None] * len(self.species)
 
     def step(self, nsteps=1):
         g, dt, n = self.g, self.dt, self.order
@@ -251,37 +328,51 @@ class OracleSim:
                 boris(sp.q, sp.m, dt, sp.ux, sp.uy, sp.uz, F[:3], F[3:])          # step 2
                 x1, y1, z1 = move(dt, sp.x, sp.y, sp.z, sp.ux, sp.uy, sp.uz)      # step 3
                 deposit_esirkepov(g, n, sp.q, dt, sp.w, (sp.x, sp.y, sp.z), (x1, y1, z1), self.J)  # 4
-                wrap(g, x1, y1, z1)                                               # step 5
+                if self.open_z:                    # no wrap along z: leavers are deleted below
+                    zkeep = z1.copy()
+                    wrap(g, x1, y1, z1)
+                    z1 = zkeep
+                else:
+                    wrap(g, x1, y1, z1)                                           # step 5
                 sp.x, sp.y, sp.z = x1, y1, z1
+            if self.open_z:
+                self._zero_pads(self.J)            # current deposited outside the box is dropped
+                self._delete_outside_z()
+            for comp, k, vals in self.plane_sources:                              # NEXT-2 antenna
+                self._phys(self.J[comp])[k] += vals
+            self.plane_sources = []
             for a in self.J:                       # NEXT-3: optional binomial smoothing of J
                 if self.smooth_passes:
                     smooth_binomial(g, self.smooth_passes, a)
             yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 6
+            self._zero_pads(self.B)
             yee_push_E(g, dt, self.E, self.B, self.J)                             # step 7
+            self._zero_pads(self.E)
             yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 8
+            self._zero_pads(self.B)
 
     def sort(self):
         for s, sp in enumerate(self.species):
             if sp is None:
                 continue
             key = cell_keys(self.g, sp.x, sp.y, sp.z)
-            perm, off = counting_sort(self.ncell, key)
+            perm, off = counting_sort(self.ncell_all, key)
             for name in ("x", "y", "z", "ux", "uy", "uz", "w", "id"):
                 setattr(sp, name, np.ascontiguousarray(getattr(sp, name)[perm]))
             self.cell_offset[s] = off
 
     def get_fields(self):
-        return {k: v.copy() for k, v in zip(("Ex", "Ey", "Ez", "Bx", "By", "Bz", "Jx", "Jy", "Jz"),
-                                            self.E + self.B + self.J)}
+        return {k: np.ascontiguousarray(self._phys(v)).reshape(-1).copy()
+                for k, v in zip(("Ex", "Ey", "Ez", "Bx", "By", "Bz", "Jx", "Jy", "Jz"), self.E + self.B + self.J)}
 
     def get_particles(self, s):
         sp = self.species[s]
         return {k: getattr(sp, k).copy() for k in ("x", "y", "z", "ux", "uy", "uz", "w", "id")}
 
     def deposit_rho(self, s=-1):
-        rho = np.zeros(self.ncell)
+        rho = np.zeros(self.ncell_all)
         for i, sp in enumerate(self.species):
             if sp is None or (s >= 0 and i != s):
                 continue
             deposit_rho(self.g, self.order, sp.q, sp.w, sp.x, sp.y, sp.z, rho)
-        return rho
+        return np.ascontiguousarray(self._phys(rho)).reshape(-1).copy()
