@@ -272,6 +272,13 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    (NEXT-1, below): particles are not wrapped along d, J guard
  *                    layers along d are not folded, and pic_step is replaced by
  *                    pic_step_stage plus the halo calls.  Default 0.
+ *   "absorb_mask"    bit d set = both faces normal to dimension d are OPEN ENDS
+ *                    (NEXT-2): every field value beyond them is zero at all times,
+ *                    current deposited beyond them is dropped, and a particle that
+ *                    leaves through them is deleted at the end of the particle
+ *                    stage (which then synchronises).  Implies the same bits of
+ *                    "open_mask"; pic_step stays available when every open
+ *                    dimension is absorbing.  Oracle: OracleSim(open_z=True).
  *   "id_base"        ids given by the next pic_load_particles start at this
  *                    value (default 0), so that bricks can hand out disjoint ids.
  * Unknown name: PIC_EINVAL.
@@ -315,6 +322,21 @@ int pic_set_option(pic_ctx*, const char* name, long long value);
  *   seam of the whole domain, else 0).  PIC_ENOMEM if they do not fit np_max.
  */
 int pic_step_stage(pic_ctx*, int stage);
+
+/*
+ * ---- NEXT-2: moving window and antenna -----------
+ * pic_shift_window: the box moves up by `ncells` cells along z (needs
+ *   "absorb_mask" bit 2): field index k now names what was k + ncells, the top
+ *   ncells planes are new and zero, zmin grows by ncells*dz, particles below the
+ *   new zmin are deleted (*deleted = how many, may be NULL), every species counts
+ *   as unsorted.  Fresh plasma for the new planes is the caller's to append with
+ *   pic_import_arrivals.  Synchronises.
+ * pic_add_plane: F[:, :, k] += values for one component (0..8 = Ex Ey Ez Bx By Bz
+ *   Jx Jy Jz), values = nx*ny doubles, x fastest (host or device).  An antenna is
+ *   pic_step_stage(0), pic_add_plane(6.., k, J_source), pic_step_stage(1..3).
+ */
+int pic_shift_window(pic_ctx*, int ncells, long long* deleted /*host, may be NULL*/);
+int pic_add_plane(pic_ctx*, int component, int k, const double* values, int src_on_device);
 long long pic_halo_doubles(pic_ctx*, int dim);
 int pic_export_halo(pic_ctx*, int group, int dim, int side, double* buf_dev);
 int pic_import_halo(pic_ctx*, int group, int dim, int side, const double* buf_dev);

@@ -24,7 +24,8 @@ SYMBOLS = ("pic_query_arena", "pic_init_grid", "pic_set_fields", "pic_load_parti
            "pic_sort", "pic_get_fields", "pic_get_particles", "pic_deposit_rho", "pic_get_cell_offsets",
            "pic_get_counters", "pic_get_stage_ms", "pic_set_option", "pic_sync", "pic_last_error",
            "pic_destroy", "pic_version", "pic_step_stage", "pic_halo_doubles", "pic_export_halo",
-           "pic_import_halo", "pic_export_leavers", "pic_import_arrivals", "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
+           "pic_import_halo", "pic_export_leavers", "pic_import_arrivals", "pic_shift_window", "pic_add_plane",
+           "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
 
 
 class PicError(RuntimeError):
@@ -75,6 +76,8 @@ def load_library(path: str | None = None):
     L.pic_import_halo.argtypes = [vp, i, i, i, vp]
     L.pic_export_leavers.argtypes = [vp, i, i, i, vp, ll, C.POINTER(ll)]
     L.pic_import_arrivals.argtypes = [vp, i, vp, ll, d, d, d]
+    L.pic_shift_window.argtypes = [vp, i, C.POINTER(ll)]
+    L.pic_add_plane.argtypes = [vp, i, i, vp, i]
     L.pic_probe_dfma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_dmma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
@@ -316,6 +319,33 @@ class Sim:
         self._check(self._L.pic_import_arrivals(self._ctx, species, C.c_void_p(buf.data_ptr()) if count else None,
                                                 int(count), float(shift[0]), float(shift[1]), float(shift[2])),
                     "pic_import_arrivals")
+
+    # -- NEXT-2: moving window, plane source, fresh plasma ---------------------------------------
+    def shift_window(self, ncells=1):
+        """Returns the number of particles the window left behind (deleted)."""
+        n = C.c_longlong(0)
+        self._check(self._L.pic_shift_window(self._ctx, int(ncells), C.byref(n)), "pic_shift_window")
+        return int(n.value)
+
+    def add_plane(self, name, k, values):
+        """F[:, :, k] += values (ny x nx, x fastest; numpy on the host or a torch.cuda tensor)."""
+        dev = _on_device([values])
+        self._check(self._L.pic_add_plane(self._ctx, self.FIELD_NAMES.index(name), int(k),
+                                          _ptr(values, np.float64, dev), int(dev)), "pic_add_plane")
+
+    def append_particles(self, species, x, y, z, ux, uy, uz, w, ids):
+        """Appends particles given as host arrays (marshalled into the 8-double records of pic_import_arrivals)."""
+        t = self._torch
+        n = len(x)
+        if n == 0:
+            return
+        rec = np.empty((n, 8))
+        for k, a in enumerate((x, y, z, ux, uy, uz, w)):
+            rec[:, k] = a
+        rec[:, 7] = np.asarray(ids, dtype=np.uint64).view(np.float64)
+        buf = t.from_numpy(rec.reshape(-1)).to(self.device)
+        self.import_arrivals(species, buf, n)
+        self.sync()
 
     def set_option(self, name, value):
         self._check(self._L.pic_set_option(self._ctx, name.encode(), int(value)), "pic_set_option")

@@ -42,6 +42,28 @@ __global__ void halo_kernel(Grid g, PlaneGeom pg, double* F, int dim, int first_
     else F[o] = buf[b];
 }
 
+// every layer first_layer .. first_layer + NG - 1 along dim := value (full padded extent of the other two dimensions)
+__global__ void halo_fill_kernel(PlaneGeom pg, double* F, int first_layer, double value) {
+    const int u = (int)(blockIdx.x * blockDim.x + threadIdx.x), v = (int)blockIdx.y, l = (int)blockIdx.z;
+    if (u >= pg.n1) return;
+    F[pg.s0 * (long long)(first_layer + l + NG) + pg.s1 * u + pg.s2 * v] = value;
+}
+
+// moving window: F[k] := F[k + n] along z over the whole padded array, zero where k + n runs off the top.  One thread
+// per (x, y) column walks z upwards, so every read happens before the write that would overwrite it.
+__global__ void shift_z_kernel(Grid g, double* F, int n) {
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x), j = (int)blockIdx.y;
+    if (i >= g.px) return;
+    double* col = F + i + g.sy * j;
+    for (int k = 0; k < g.pz; ++k) col[g.sz * k] = (k + n < g.pz) ? col[g.sz * (k + n)] : 0.0;
+}
+
+// F[interior plane k] += values (guard-free nx x ny, x fastest)
+__global__ void add_plane_kernel(Grid g, double* F, int k, const double* __restrict__ values) {
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x), j = (int)blockIdx.y;
+    if (i < g.nx) F[g.idx(i, j, k)] += values[i + (long long)g.nx * j];
+}
+
 __global__ void split_leavers_kernel(Grid g, Particles src, Particles dst, long long n, int dim, int side, double* out,
                                      long long capacity, unsigned long long* counters) {
     const long long ip = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -114,6 +136,22 @@ void launch_halo_unpack(const Grid& g, double* F, int dim, int first_layer, cons
     dim3 bs(128, 1, 1), nb((pg.n1 + 127) / 128, pg.n2, NG);
     if (add) halo_kernel<false, true><<<nb, bs, 0, st>>>(g, pg, F, dim, first_layer, const_cast<double*>(buf));
     else halo_kernel<false, false><<<nb, bs, 0, st>>>(g, pg, F, dim, first_layer, const_cast<double*>(buf));
+}
+
+void launch_halo_fill(const Grid& g, double* F, int dim, int first_layer, double value, cudaStream_t st) {
+    const PlaneGeom pg = plane_geom(g, dim);
+    dim3 bs(128, 1, 1), nb((pg.n1 + 127) / 128, pg.n2, NG);
+    halo_fill_kernel<<<nb, bs, 0, st>>>(pg, F, first_layer, value);
+}
+
+void launch_shift_z(const Grid& g, double* F, int ncells, cudaStream_t st) {
+    dim3 bs(128, 1, 1), nb((g.px + 127) / 128, g.py, 1);
+    shift_z_kernel<<<nb, bs, 0, st>>>(g, F, ncells);
+}
+
+void launch_add_plane(const Grid& g, double* F, int k, const double* values_dev, cudaStream_t st) {
+    dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, 1);
+    add_plane_kernel<<<nb, bs, 0, st>>>(g, F, k, values_dev);
 }
 
 void launch_split_leavers(const Grid& g, const Particles& src, const Particles& dst, long long n, int dim, int side,

@@ -71,6 +71,8 @@ struct pic_ctx {
     int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1, fuse_keys = 1;
     int gather_variant = 0, smooth_passes = 0;      // NEXT-3 options
     unsigned long long id_base = 0;                 // ids given at load start here (bricks: unique across contexts)
+    int absorb_mask = 0;                            // NEXT-2: dimensions whose faces are open ends (zero exterior, particles deleted)
+    unsigned long long deleted = 0;                 // particles deleted at absorbing faces / by the moving window
     YeeMaps yee_maps{};
     int device = 0;                     // ordinal of the device the arena lives on; made current by every call
     int yee_tma_ok = 0;                 // tensor maps built: the TMA-staged Yee kernels are available
@@ -286,6 +288,8 @@ void materialize(pic_ctx* c, Species& S) {
 
 extern "C" {
 
+static void zero_absorbing_guards(pic_ctx* c, int group);
+
 const char* pic_version(void) { return "pic_b200 0.1 (sm_100a)"; }
 
 int pic_query_arena(int nx, int ny, int nz, int order, int nspecies, const long long* np_max, size_t* bytes) {
@@ -398,6 +402,10 @@ int pic_set_fields(pic_ctx* c, const double* Ex, const double* Ey, const double*
         int rc = copy_in(c, src[k], dst[k], src_on_device);
         if (rc != PIC_OK) return rc;
     }
+    if (c->absorb_mask) {
+        zero_absorbing_guards(c, 0);
+        zero_absorbing_guards(c, 1);
+    }
     return PIC_OK;
 }
 
@@ -436,6 +444,57 @@ int pic_load_particles(pic_ctx* c, int species, double q, double m, long long n,
         return fail(c, PIC_EINVAL, "species %d: a particle is outside the box or non-finite", species);
     }
     S.loaded = true;
+    return PIC_OK;
+}
+
+// ---- NEXT-2: absorbing faces (zero exterior), used by the step, pic_set_fields and pic_shift_window -----
+// guard layers of a group of three components := 0 along every absorbing dimension
+static void zero_absorbing_guards(pic_ctx* c, int group) {
+    double* F[3][3] = {{c->f.Ex, c->f.Ey, c->f.Ez}, {c->f.Bx, c->f.By, c->f.Bz}, {c->f.Jx, c->f.Jy, c->f.Jz}};
+    const int n[3] = {c->g.nx, c->g.ny, c->g.nz};
+    for (int d = 0; d < 3; ++d)
+        if ((c->absorb_mask >> d) & 1)
+            for (int k = 0; k < 3; ++k) {
+                launch_halo_fill(c->g, F[group][k], d, -NG, 0.0, c->stream);
+                launch_halo_fill(c->g, F[group][k], d, n[d], 0.0, c->stream);
+                c->launches += 2;
+            }
+}
+
+// particles of one species beyond face (dim, side) are removed (container compacted).  Synchronises.
+static int discard_leavers(pic_ctx* c, Species& S, int dim, int side, long long* count) {
+    *count = 0;
+    if (!S.loaded || S.n == 0) return PIC_OK;
+    materialize(c, S);
+    unsigned long long* counters = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(c->status) + 128);
+    CU(c, cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), c->stream));
+    launch_split_leavers(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, dim, side, nullptr, 0, counters, c->stream);
+    c->launches += 1;
+    unsigned long long h[2];
+    CU(c, cudaMemcpyAsync(h, counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (h[0] + h[1] != (unsigned long long)S.n) return fail(c, PIC_ECUDA, "leaver split lost particles");
+    *count = (long long)h[0];
+    if (h[0] > 0) {
+        S.cur ^= 1;
+        S.n = (long long)h[1];
+        S.sorted = false;
+        S.keys_valid = false;
+        S.degraded = false;
+        c->deleted += h[0];
+    }
+    return PIC_OK;
+}
+
+static int discard_at_absorbing_faces(pic_ctx* c) {
+    for (int d = 0; d < 3; ++d)
+        if ((c->absorb_mask >> d) & 1)
+            for (int s = 0; s < c->nspecies; ++s)
+                for (int side = 0; side < 2; ++side) {
+                    long long cnt;
+                    int rc = discard_leavers(c, c->sp[s], d, side, &cnt);
+                    if (rc != PIC_OK) return rc;
+                }
     return PIC_OK;
 }
 
@@ -534,17 +593,30 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
             for (int k = 0; k < 3; ++k) c->launches += launch_smooth_binomial(g, J[k], c->tmp, c->smooth_passes, c->stream);
         }
         nvtxRangePop();
+        if (c->absorb_mask) {            // NEXT-2: whoever left through an open end is gone (synchronises)
+            int rc = discard_at_absorbing_faces(c);
+            if (rc != PIC_OK) { nvtxRangePop(); return rc; }
+        }
         }      // mask & 1
         if (timing) cudaEventRecord(ev[3], c->stream);
         // steps 6-8
         nvtxRangePushA("yee");
-        if (mask & 2) { launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream); c->launches += 1; }
+        if (mask & 2) {
+            launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
+            c->launches += 1;
+            if (c->absorb_mask) zero_absorbing_guards(c, 1);
+        }
         if (timing) cudaEventRecord(ev[4], c->stream);
-        if (mask & 4) { launch_push_E(g, c->f, g.dt, tma_E, c->stream); c->launches += 1; }
+        if (mask & 4) {
+            launch_push_E(g, c->f, g.dt, tma_E, c->stream);
+            c->launches += 1;
+            if (c->absorb_mask) zero_absorbing_guards(c, 0);
+        }
         if (timing) cudaEventRecord(ev[5], c->stream);
         if (mask & 8) {
             launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
             c->launches += 1;
+            if (c->absorb_mask) zero_absorbing_guards(c, 1);
             c->steps += 1;
         }
         nvtxRangePop();
@@ -558,7 +630,9 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
 
 int pic_step(pic_ctx* c, int nsteps) {
     ENTER(c);
-    if (c->g.open_mask) return fail(c, PIC_ESTATE, "a brick (open_mask != 0) is stepped with pic_step_stage and the halo calls");
+    if (c->g.open_mask & ~c->absorb_mask)
+        return fail(c, PIC_ESTATE, "a brick (open_mask != 0) is stepped with pic_step_stage and the halo calls");
+    if (c->smooth_passes > 0 && c->g.open_mask) return fail(c, PIC_ESTATE, "smooth_passes is not available with open faces");
     return step_impl(c, nsteps, 15);
 }
 
@@ -566,6 +640,11 @@ int pic_step_stage(pic_ctx* c, int stage) {
     ENTER(c);
     if (stage < 0 || stage > 3) return fail(c, PIC_EINVAL, "stage must be 0 .. 3");
     if (c->smooth_passes > 0 && c->g.open_mask) return fail(c, PIC_ESTATE, "smooth_passes is not available on a brick");
+    if (stage == 0 && c->nspecies > 0) {
+        bool any = false;
+        for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
+        if (!any) return fail(c, PIC_ESTATE, "pic_step_stage before any pic_load_particles");
+    }
     return step_impl(c, 1, 1 << stage);
 }
 
@@ -664,6 +743,57 @@ int pic_import_arrivals(pic_ctx* c, int species, const double* buf_dev, long lon
     S.sorted = false;
     S.keys_valid = false;
     CU(c, cudaGetLastError());
+    return PIC_OK;
+}
+
+// ---- NEXT-2: moving window and plane source ----------------------------------------------------------------
+int pic_shift_window(pic_ctx* c, int ncells, long long* deleted) {
+    ENTER(c);
+    if (!(c->absorb_mask & 4)) return fail(c, PIC_ESTATE, "a moving window needs open ends along z (absorb_mask bit 2)");
+    if (ncells < 0 || ncells > c->g.nz) return fail(c, PIC_EINVAL, "ncells must be 0 .. nz");
+    if (deleted) *deleted = 0;
+    if (ncells == 0) return PIC_OK;
+    double* F[9] = {c->f.Ex, c->f.Ey, c->f.Ez, c->f.Bx, c->f.By, c->f.Bz, c->f.Jx, c->f.Jy, c->f.Jz};
+    for (int k = 0; k < 9; ++k) launch_shift_z(c->g, F[k], ncells, c->stream);
+    c->launches += 9;
+    // the planes that slid into the lower guard layers are outside the box now
+    zero_absorbing_guards(c, 0);
+    zero_absorbing_guards(c, 1);
+    zero_absorbing_guards(c, 2);
+    Grid& g = c->g;
+    g.zmin += ncells * g.dz;           // the same expression the oracle uses (its zmin + n dz)
+    g.zmax = g.zmin + g.Lz;
+    long long total = 0;
+    for (int s = 0; s < c->nspecies; ++s) {
+        Species& S = c->sp[s];
+        if (!S.loaded) continue;
+        long long cnt = 0;
+        int rc = discard_leavers(c, S, 2, 0, &cnt);
+        if (rc != PIC_OK) return rc;
+        total += cnt;
+        S.sorted = false;              // every cell index changed
+        S.keys_valid = false;
+        S.perm_pending = false;
+    }
+    if (deleted) *deleted = total;
+    CU(c, cudaGetLastError());
+    return PIC_OK;
+}
+
+int pic_add_plane(pic_ctx* c, int component, int k, const double* values, int src_on_device) {
+    ENTER(c);
+    if (component < 0 || component > 8 || k < 0 || k >= c->g.nz || !values)
+        return fail(c, PIC_EINVAL, "bad component, plane or buffer");
+    double* F[9] = {c->f.Ex, c->f.Ey, c->f.Ez, c->f.Bx, c->f.By, c->f.Bz, c->f.Jx, c->f.Jy, c->f.Jz};
+    const double* src = values;
+    if (!src_on_device) {
+        CU(c, cudaMemcpyAsync(c->tmp, values, (size_t)c->g.nx * c->g.ny * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        src = c->tmp;
+    }
+    launch_add_plane(c->g, F[component], k, src, c->stream);
+    c->launches += 1;
+    CU(c, cudaGetLastError());
+    if (!src_on_device) CU(c, cudaStreamSynchronize(c->stream));
     return PIC_OK;
 }
 
@@ -839,6 +969,15 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     else if (!strcmp(name, "open_mask")) {
         if (value < 0 || value > 7) return fail(c, PIC_EINVAL, "open_mask must be 0 .. 7");
         c->g.open_mask = (int)value;
+    } else if (!strcmp(name, "absorb_mask")) {
+        if (value < 0 || value > 7) return fail(c, PIC_EINVAL, "absorb_mask must be 0 .. 7");
+        const int n[3] = {c->g.nx, c->g.ny, c->g.nz};
+        for (int d = 0; d < 3; ++d)
+            if (((value >> d) & 1) && n[d] < NG) return fail(c, PIC_EINVAL, "an open end needs at least %d cells along its dimension", NG);
+        c->g.open_mask = (c->g.open_mask & ~c->absorb_mask) | (int)value;
+        c->absorb_mask = (int)value;
+        zero_absorbing_guards(c, 0);
+        zero_absorbing_guards(c, 1);
     } else if (!strcmp(name, "id_base")) {
         if (value < 0) return fail(c, PIC_EINVAL, "id_base must be >= 0");
         c->id_base = (unsigned long long)value;

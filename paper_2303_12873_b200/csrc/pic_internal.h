@@ -88,6 +88,9 @@ void launch_iota(unsigned long long* id, long long n, unsigned long long base, c
 long long halo_doubles(const Grid& g, int dim);                    // per component and side
 void launch_halo_pack(const Grid& g, const double* F, int dim, int first_layer, double* buf, cudaStream_t st);
 void launch_halo_unpack(const Grid& g, double* F, int dim, int first_layer, const double* buf, bool add, cudaStream_t st);
+void launch_halo_fill(const Grid& g, double* F, int dim, int first_layer, double value, cudaStream_t st);
+void launch_shift_z(const Grid& g, double* F, int ncells, cudaStream_t st);          // moving window (NEXT-2)
+void launch_add_plane(const Grid& g, double* F, int k, const double* values_dev, cudaStream_t st);
 // leavers of face (dim, side) -> out[8 * k .. 8 * k + 7] = x y z ux uy uz w id; everything else -> dst (compacted);
 // counters[0] = leavers, counters[1] = stayers (device, zeroed by the caller)
 void launch_split_leavers(const Grid& g, const Particles& src, const Particles& dst, long long n, int dim, int side,
