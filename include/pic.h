@@ -263,6 +263,12 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    order n-1 along every direction in which the gathered
  *                    component is staggered (
  *                    oracle: ora_gather_variant).  Both particle kernels.
+ *   "deposit_variant" 0 (default) = Esirkepov charge-conserving deposition; 1 =
+ *                    direct deposition (NEXT-3; oracle: ora_deposit_direct): q w v
+ *                    of the move, spread with the order-n shape at the middle
+ *                    of the move at each component's Yee location.  NOT charge
+ *                    conserving.  Runs in the global-atomic kernel only (a sorted
+ *                    species leaves the fused per-tile kernel while it is set).
  *   "smooth_passes"  k >= 0 (default 0, at most 16): after deposition and guard
  *                    fold, each J component is filtered k times by the periodic
  *                    binomial (1/4, 1/2, 1/4) stencil along x, then y, then z

@@ -64,6 +64,7 @@ def lib():
         L.ora_boris.argtypes = [C.c_longlong, C.c_double, C.c_double, C.c_double] + [_dp] * 9
         L.ora_move.argtypes = [C.c_longlong, C.c_double] + [_dp] * 9
         L.ora_deposit_esirkepov.argtypes = [G, C.c_int, C.c_longlong, C.c_double, C.c_double] + [_dp] * 10
+        L.ora_deposit_direct.argtypes = [G, C.c_int, C.c_longlong, C.c_double, C.c_double] + [_dp] * 10
         L.ora_wrap.argtypes = [G, C.c_longlong] + [_dp] * 3
         L.ora_yee_push_B.argtypes = [G, C.c_double] + [_dp] * 6
         L.ora_yee_push_E.argtypes = [G, C.c_double] + [_dp] * 9
@@ -165,6 +166,15 @@ def deposit_esirkepov(g, order, q, dt, w, p0, p1, J):
     _check(rc, "deposit_esirkepov")
 
 
+def deposit_direct(g, order, q, dt, w, p0, p1, J):
+    """NEXT-3: direct deposition; accumulates into J = (Jx,Jy,Jz)."""
+    n = p0[0].size
+    rc = lib().ora_deposit_direct(C.byref(g), order, n, q, dt, _d(_f64(w)),
+                                  *[_d(_f64(a)) for a in p0], *[_d(_f64(a)) for a in p1],
+                                  *[_d(a) for a in J])
+    _check(rc, "deposit_direct")
+
+
 def wrap(g, x, y, z):
     _check(lib().ora_wrap(C.byref(g), x.size, _d(x), _d(y), _d(z)), "wrap")
 
@@ -215,7 +225,10 @@ class OracleSim:
     ZPAD = 4
 
     def __init__(self, nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, dt, order, nspecies, gather_variant=0,
-                 smooth_passes=0, open_z=False):
+                 smooth_passes=0, open_z=False, deposit_variant=0):
+        if deposit_variant not in (0, 1):
+            raise ValueError("deposit_variant must be 0 (Esirkepov) or 1 (direct)")
+        self.deposit_variant = int(deposit_variant)
         self.open_z = bool(open_z)
         self.nz_phys = int(nz)
         self.pad = self.ZPAD if self.open_z else 0
@@ -327,7 +340,10 @@ class OracleSim:
                     F = gather(g, n, sp.x, sp.y, sp.z, self.E, self.B)             # step 1
                 boris(sp.q, sp.m, dt, sp.ux, sp.uy, sp.uz, F[:3], F[3:])          # step 2
                 x1, y1, z1 = move(dt, sp.x, sp.y, sp.z, sp.ux, sp.uy, sp.uz)      # step 3
-                deposit_esirkepov(g, n, sp.q, dt, sp.w, (sp.x, sp.y, sp.z), (x1, y1, z1), self.J)  # 4
+                if self.deposit_variant:
+                    deposit_direct(g, n, sp.q, dt, sp.w, (sp.x, sp.y, sp.z), (x1, y1, z1), self.J)
+                else:
+                    deposit_esirkepov(g, n, sp.q, dt, sp.w, (sp.x, sp.y, sp.z), (x1, y1, z1), self.J)  # 4
                 if self.open_z:                    # no wrap along z: leavers are deleted below
                     zkeep = z1.copy()
                     wrap(g, x1, y1, z1)

@@ -310,6 +310,44 @@ int ora_deposit_esirkepov(const ora_grid* g, int order, long long np,
     return 0;
 }
 
+/* NEXT-3: direct, NOT charge-conserving deposition.  The particle is taken at the middle of its
+ * move, x_h = (x0 + x1)/2, with the velocity of the move v = (x1 - x0)/dt, and its current q w v / dV is spread with
+ * the order-n shape evaluated at each component's own Yee location:
+ *  Jx[i+1/2,j,k] += (q w vx/dV) S(xi_h - i - 1/2) S(eta_h - j)       S(zeta_h - k)
+ *  Jy[i,j+1/2,k] += (q w vy/dV) S(xi_h - i)       S(eta_h - j - 1/2) S(zeta_h - k)
+ *  Jz[i,j,k+1/2] += (q w vz/dV) S(xi_h - i)       S(eta_h - j)       S(zeta_h - k - 1/2)     */
+int ora_deposit_direct(const ora_grid* g, int order, long long np,
+                       double q, double dt, const double* w,
+                       const double* x0, const double* y0, const double* z0,
+                       const double* x1, const double* y1, const double* z1,
+                       double* Jx, double* Jy, double* Jz)
+{
+    if (order < 1 || order > 3) return -1;
+    int h = window_h(order), wn = 2 * h + 2;
+    double inv_dx = 1.0 / g->dx, inv_dy = 1.0 / g->dy, inv_dz = 1.0 / g->dz;
+    double inv_dv = 1.0 / (g->dx * g->dy * g->dz);
+    for (long long p = 0; p < np; ++p) {
+        double xh = 0.5 * (x0[p] + x1[p]), yh = 0.5 * (y0[p] + y1[p]), zh = 0.5 * (z0[p] + z1[p]);
+        double vx = (x1[p] - x0[p]) / dt, vy = (y1[p] - y0[p]) / dt, vz = (z1[p] - z0[p]) / dt;
+        double xi = (xh - g->xmin) * inv_dx, eta = (yh - g->ymin) * inv_dy, zeta = (zh - g->zmin) * inv_dz;
+        long long i0 = (long long)floor(xi), j0 = (long long)floor(eta), k0 = (long long)floor(zeta);
+        double qw = q * w[p] * inv_dv;
+        for (int c = 0; c < wn; ++c)
+            for (int b = 0; b < wn; ++b)
+                for (int a = 0; a < wn; ++a) {
+                    long long i = i0 - h + a, j = j0 - h + b, k = k0 - h + c;
+                    double sxn = ora_shape(order, xi - (double)i), sxs = ora_shape(order, xi - (double)i - 0.5);
+                    double syn = ora_shape(order, eta - (double)j), sys = ora_shape(order, eta - (double)j - 0.5);
+                    double szn = ora_shape(order, zeta - (double)k), szs = ora_shape(order, zeta - (double)k - 0.5);
+                    size_t o = gidx(g, i, j, k);
+                    Jx[o] += qw * vx * sxs * syn * szn;
+                    Jy[o] += qw * vy * sxn * sys * szn;
+                    Jz[o] += qw * vz * sxn * syn * szs;
+                }
+    }
+    return 0;
+}
+
 /* one wrap suffices since |move| < 1 cell. */
 static double wrap1(double v, double lo, double hi, double L)
 {

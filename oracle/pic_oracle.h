@@ -100,6 +100,14 @@ int ora_deposit_esirkepov(const ora_grid* g, int order, long long np,
                           const double* x1, const double* y1, const double* z1,
                           double* Jx, double* Jy, double* Jz);
 
+/* NEXT-3: direct (not charge-conserving) deposition, ACCUMULATED into Jx,Jy,Jz: q w v S(x_half - node)/dV with
+ * x_half = (x0 + x1)/2, v = (x1 - x0)/dt, order-n shapes at each component's Yee location. */
+int ora_deposit_direct(const ora_grid* g, int order, long long np,
+                       double q, double dt, const double* w,
+                       const double* x0, const double* y0, const double* z0,
+                       const double* x1, const double* y1, const double* z1,
+                       double* Jx, double* Jy, double* Jz);
+
 /* Step 5: periodic wrap of positions into [xmin, xmax), in place. */
 int ora_wrap(const ora_grid* g, long long np, double* x, double* y, double* z);
 

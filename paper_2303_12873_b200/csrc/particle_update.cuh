@@ -155,9 +155,42 @@ __device__ __forceinline__ void deposit_global(const Grid& g, const Fields& f, d
     deposit_esirkepov<N>(g, xi0, et0, ze0, xi1, et1, ze1, qw, bad, add);
 }
 
+// Direct, not charge-conserving deposition (pic_set_option "deposit_variant" = 1): the particle at
+// the middle of its move with the velocity of the move, order-N shapes at each component's Yee location, one
+// global fp64 atomic per non-zero point.
+template <int N>
+__device__ __forceinline__ void deposit_direct_global(const Grid& g, const Fields& f, double x0, double y0, double z0,
+                                                      double x1, double y1, double z1, double qw) {
+    const double xh = 0.5 * (x0 + x1), yh = 0.5 * (y0 + y1), zh = 0.5 * (z0 + z1);
+    const double inv_dt = 1.0 / g.dt;
+    const double xi = (xh - g.xmin) * g.inv_dx, et = (yh - g.ymin) * g.inv_dy, ze = (zh - g.zmin) * g.inv_dz;
+    double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[N + 1], wys[N + 1], wzs[N + 1];
+    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn), fzn = shape_weights<N>(ze, wzn);
+    const int fxs = shape_weights<N>(xi - 0.5, wxs), fys = shape_weights<N>(et - 0.5, wys),
+              fzs = shape_weights<N>(ze - 0.5, wzs);
+    const double c = qw * (g.inv_dx * g.inv_dy * g.inv_dz);
+    const double cx = c * ((x1 - x0) * inv_dt), cy = c * ((y1 - y0) * inv_dt), cz = c * ((z1 - z0) * inv_dt);
+    double* jx = f.Jx + g.idx(fxs, fyn, fzn);
+    double* jy = f.Jy + g.idx(fxn, fys, fzn);
+    double* jz = f.Jz + g.idx(fxn, fyn, fzs);
+#pragma unroll
+    for (int cc = 0; cc <= N; ++cc)
+#pragma unroll
+        for (int b = 0; b <= N; ++b)
+#pragma unroll
+            for (int a = 0; a <= N; ++a) {
+                const long long o = a + b * g.sy + cc * g.sz;
+                const double vx = cx * wxs[a] * wyn[b] * wzn[cc], vy = cy * wxn[a] * wys[b] * wzn[cc],
+                             vz = cz * wxn[a] * wyn[b] * wzs[cc];
+                if (vx != 0.0) atomicAdd(jx + o, vx);
+                if (vy != 0.0) atomicAdd(jy + o, vy);
+                if (vz != 0.0) atomicAdd(jz + o, vz);
+            }
+}
+
 // Device function used by both particle paths: the whole update of one
-// particle against the GLOBAL field arrays.
-template <int N, int GV>
+// particle against the GLOBAL field arrays.  DV = 0: Esirkepov deposition; 1: direct deposition.
+template <int N, int GV, int DV = 0>
 __device__ __forceinline__ void update_particle_global(const Grid& g, const Fields& f, const Particles& p,
                                                        long long ip, double q, double h, DevStatus* status) {
     const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
@@ -178,7 +211,12 @@ __device__ __forceinline__ void update_particle_global(const Grid& g, const Fiel
     // step 4: deposit from (x^n, x~^{n+1})
     const double xi1 = (x1 - g.xmin) * g.inv_dx, et1 = (y1 - g.ymin) * g.inv_dy, ze1 = (z1 - g.zmin) * g.inv_dz;
     bool bad = !(isfinite(x1) && isfinite(y1) && isfinite(z1));
-    if (!bad && q != 0.0) deposit_global<N>(g, f, xi, et, ze, xi1, et1, ze1, q * w, bad);
+    if constexpr (DV == 1) {
+        bad = bad || !(fabs(xi1 - xi) < 1.0) || !(fabs(et1 - et) < 1.0) || !(fabs(ze1 - ze) < 1.0);
+        if (!bad && q != 0.0) deposit_direct_global<N>(g, f, x, y, z, x1, y1, z1, q * w);
+    } else {
+        if (!bad && q != 0.0) deposit_global<N>(g, f, xi, et, ze, xi1, et1, ze1, q * w, bad);
+    }
     if (bad) status->ephys = 1;
     // step 5: wrap and store
     p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx, g.open_mask & 1);

@@ -69,7 +69,7 @@ struct pic_ctx {
     unsigned long long launches = 0, steps = 0, sorts = 0;
     // options
     int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1, fuse_keys = 1;
-    int gather_variant = 0, smooth_passes = 0;      // NEXT-3 options
+    int gather_variant = 0, smooth_passes = 0, deposit_variant = 0;      // NEXT-3 options
     unsigned long long id_base = 0;                 // ids given at load start here (bricks: unique across contexts)
     int absorb_mask = 0;                            // NEXT-2: dimensions whose faces are open ends (zero exterior, particles deleted)
     unsigned long long deleted = 0;                 // particles deleted at absorbing faces / by the moving window
@@ -245,7 +245,7 @@ bool take_events(pic_ctx* c, int n, size_t* first) {
 }
 
 bool use_tile_path(const pic_ctx* c, const Species& s) {
-    if (c->force_path == 1) return false;
+    if (c->force_path == 1 || c->deposit_variant != 0) return false;     // direct deposition lives in the global kernel only
     if (c->force_path == 2) return s.sorted;
     return s.sorted && !s.degraded;
 }
@@ -569,8 +569,8 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
                     if (S.sorted && S.degraded) c->fallbacks += 1;
                     materialize(c, S);
                     S.keys_valid = false;
-                    launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->gather_variant, c->status,
-                                            c->stream);
+                    launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->gather_variant,
+                                            c->deposit_variant, c->status, c->stream);
                     c->launches += 1;
                 }
                 S.steps_since_sort += 1;
@@ -984,6 +984,10 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     } else if (!strcmp(name, "gather_variant")) {
         if (value < 0 || value > 1) return fail(c, PIC_EINVAL, "gather_variant must be 0 or 1");
         c->gather_variant = (int)value;
+    } else if (!strcmp(name, "deposit_variant")) {
+        if (value < 0 || value > 1) return fail(c, PIC_EINVAL, "deposit_variant must be 0 or 1");
+        if (value && c->force_path == 2) return fail(c, PIC_ESTATE, "direct deposition runs in the global-atomic kernel: not with force_path = 2");
+        c->deposit_variant = (int)value;
     } else if (!strcmp(name, "smooth_passes")) {
         if (value < 0 || value > 16) return fail(c, PIC_EINVAL, "smooth_passes must be 0 .. 16");
         c->smooth_passes = (int)value;

@@ -72,8 +72,10 @@ int launch_smooth_binomial(const Grid& g, double* F, double* tmp, int npass, cud
 // ---- particles_global.cu --------------------------------------------------
 // gather + Boris + move + Esirkepov with global fp64 atomics + wrap; any particle order.
 // gather_variant: 0 = order n in every direction, 1 = order n-1 along a component's staggered directions
+// deposit_variant: 0 = Esirkepov (charge-conserving), 1 = direct deposition at the middle of the move
 void launch_particles_global(const Grid& g, const Fields& f, const Particles& p, long long n, double q,
-                             double m, int order, int gather_variant, DevStatus* status, cudaStream_t st);
+                             double m, int order, int gather_variant, int deposit_variant, DevStatus* status,
+                             cudaStream_t st);
 void launch_deposit_rho(const Grid& g, const Particles& p, long long n, double q, int order, double* rho_pad,
                         cudaStream_t st);
 void launch_fold_guards(const Grid& g, double* F, cudaStream_t st);       // sum periodic images into the interior

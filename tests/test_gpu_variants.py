@@ -28,9 +28,9 @@ def _rand_fields(wl, seed, e_amp=1e9):
     return f
 
 
-def _pair(ora, Sim, wl, gather_variant=0, smooth_passes=0, sort_first=False, force_path=0):
+def _pair(ora, Sim, wl, gather_variant=0, smooth_passes=0, sort_first=False, force_path=0, deposit_variant=0):
     o = ora.OracleSim(*wl.grid_args(), wl.dt, wl.order, len(wl.species), gather_variant=gather_variant,
-                      smooth_passes=smooth_passes)
+                      smooth_passes=smooth_passes, deposit_variant=deposit_variant)
     g = Sim.from_workload(wl)
     if wl.fields:
         o.set_fields(**wl.fields)
@@ -38,6 +38,7 @@ def _pair(ora, Sim, wl, gather_variant=0, smooth_passes=0, sort_first=False, for
         o.load_particles(s, sp.q, sp.m, *sp.arrays())
     g.set_option("gather_variant", gather_variant)
     g.set_option("smooth_passes", smooth_passes)
+    g.set_option("deposit_variant", deposit_variant)
     if force_path:
         g.set_option("force_path", force_path)
     if sort_first:
@@ -108,11 +109,28 @@ def test_binomial_smoothing_of_J(ora, Sim, passes):
         g.close()
 
 
+@pytest.mark.parametrize("order", [1, 2, 3])
+def test_direct_deposition(ora, Sim, order):
+    """deposit_variant = 1 against ora_deposit_direct: 1 step and 10 steps, sorted or not (a sorted species leaves the
+    fused kernel while the option is set: every update is counted as 'global'), with the energy-conserving gather too."""
+    wl = W.uniform_plasma(11, 9, 10, ppc=5, u_th=0.2, order=order, seed=360 + order, protons=True, dy=0.4e-6)
+    wl.fields = _rand_fields(wl, 43, e_amp=3e8)
+    o, g = _pair(ora, Sim, wl, deposit_variant=1, gather_variant=order % 2, sort_first=True)
+    o.step(1); g.step(1)
+    check_step_parity(o, g, wl, "direct deposition order %d" % order)
+    o.step(9); g.step(9)
+    assert field_l2_error(o.get_fields(), g.get_fields()) <= TOL_FIELD_L2_10STEP
+    c = g.counters()
+    assert c["global"] == 10 * wl.nparticles and c["fast"] + c["slow"] == 0
+    g.close()
+
+
 def test_option_validation(Sim):
     from paper_2303_12873_b200.binding import PicError
     wl = W.uniform_plasma(8, 8, 8, ppc=1, u_th=0.0, order=1, seed=1)
     g = Sim.from_workload(wl)
-    for name, bad in (("gather_variant", 2), ("gather_variant", -1), ("smooth_passes", -1), ("smooth_passes", 17)):
+    for name, bad in (("gather_variant", 2), ("gather_variant", -1), ("smooth_passes", -1), ("smooth_passes", 17),
+                      ("deposit_variant", 2)):
         with pytest.raises(PicError):
             g.set_option(name, bad)
     g.close()

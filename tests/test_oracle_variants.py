@@ -280,3 +280,67 @@ def test_cycle_with_variant_keeps_gauss_and_conserves_energy_better(ora):
         assert np.abs(res).max() <= 1e-9 * np.abs(rho0).max() / EPS0
         drift[variant] = abs(energy(sim) - e0) / e0
     assert drift[1] < drift[0], drift
+
+
+# ---------------------------------------------------------------- direct deposition ---
+@pytest.mark.parametrize("n", ORDERS)
+def test_direct_deposition_moments_impulse_and_zero_move(ora, n):
+    """ora_deposit_direct: total current = sum q w v exactly (partition of unity at each staggering); its first moment
+    along the staggered axis puts the current at the mid-point of the move (B-splines reproduce linear functions);
+    one particle = product of shapes at the mid-point (checked against ora_shape at every grid point); no move, no
+    current; linear in q w; and, unlike Esirkepov, it does NOT satisfy discrete continuity."""
+    g = _grid(ora, 10, 9, 8); rng = np.random.default_rng(20 + n)
+    nc = g.nx * g.ny * g.nz
+    dt, q = 1.3e-16, -1.602176634e-19
+    npart = 30
+    x0, y0, z0 = _rand_particles(g, rng, npart, margin=3.0)
+    d = (rng.random((3, npart)) - 0.5) * 1.6
+    x1, y1, z1 = x0 + d[0] * g.dx, y0 + d[1] * g.dy, z0 + d[2] * g.dz
+    w = rng.random(npart) * 1e4 + 1.0
+    J = [np.zeros(nc) for _ in range(3)]
+    ora.deposit_direct(g, n, q, dt, w, (x0, y0, z0), (x1, y1, z1), J)
+    dv = g.dx * g.dy * g.dz
+    for c, (a0, a1) in enumerate(((x0, x1), (y0, y1), (z0, z1))):
+        tot = np.sum(q * w * (a1 - a0) / dt)
+        assert abs(J[c].sum() * dv - tot) <= 2e-14 * np.sum(np.abs(q * w * (a1 - a0) / dt))
+    # first moment of Jx along x: sum Jx[i+1/2,..] (i + 1/2) dV = sum q w vx xi_half
+    I = np.arange(g.nx)
+    jx = J[0].reshape(g.nz, g.ny, g.nx)
+    lhs = np.sum(jx.sum(axis=(0, 1)) * (I + 0.5)) * dv
+    xi_h = (0.5 * (x0 + x1) - g.xmin) / g.dx
+    rhs = np.sum(q * w * (x1 - x0) / dt * xi_h)
+    assert abs(lhs - rhs) <= 1e-13 * np.sum(np.abs(q * w * (x1 - x0) / dt * xi_h))
+    # one particle, every grid point
+    J1 = [np.zeros(nc) for _ in range(3)]
+    ora.deposit_direct(g, n, q, dt, w[:1], (x0[:1], y0[:1], z0[:1]), (x1[:1], y1[:1], z1[:1]), J1)
+    xi = (0.5 * (x0[0] + x1[0]) - g.xmin) / g.dx; et = (0.5 * (y0[0] + y1[0]) - g.ymin) / g.dy
+    ze = (0.5 * (z0[0] + z1[0]) - g.zmin) / g.dz
+    v = ((x1[0] - x0[0]) / dt, (y1[0] - y0[0]) / dt, (z1[0] - z0[0]) / dt)
+    for c in range(3):
+        ox, oy, oz = STAG[c]
+        ref = np.zeros((g.nz, g.ny, g.nx))
+        for k in range(g.nz):
+            for j in range(g.ny):
+                for i in range(g.nx):
+                    ref[k, j, i] = ora.shape(n, xi - i - ox) * ora.shape(n, et - j - oy) * ora.shape(n, ze - k - oz)
+        ref *= q * w[0] * v[c] / dv
+        np.testing.assert_allclose(J1[c].reshape(g.nz, g.ny, g.nx), ref, rtol=0, atol=1e-13 * np.abs(ref).max())   # xi is (x - xmin) * (1/dx) in the oracle
+    # no move, no current; linear in the weight
+    J0 = [np.zeros(nc) for _ in range(3)]
+    ora.deposit_direct(g, n, q, dt, w, (x0, y0, z0), (x0, y0, z0), J0)
+    assert not any(a.any() for a in J0)
+    J2 = [np.zeros(nc) for _ in range(3)]
+    ora.deposit_direct(g, n, q, dt, 2.0 * w, (x0, y0, z0), (x1, y1, z1), J2)
+    for a, b in zip(J, J2):
+        np.testing.assert_allclose(b, 2.0 * a, rtol=4e-16)
+    # continuity is violated (that is what "direct" gives up), Esirkepov on the same moves satisfies it
+    def residual(Jc):
+        rho0 = np.zeros(nc); rho1 = np.zeros(nc)
+        ora.deposit_rho(g, n, q, w, x0, y0, z0, rho0); ora.deposit_rho(g, n, q, w, x1, y1, z1, rho1)
+        sh = (g.nz, g.ny, g.nx)
+        jx_, jy_, jz_ = (a.reshape(sh) for a in Jc)
+        div = ((jx_ - np.roll(jx_, 1, 2)) / g.dx + (jy_ - np.roll(jy_, 1, 1)) / g.dy + (jz_ - np.roll(jz_, 1, 0)) / g.dz)
+        return np.abs((rho1 - rho0).reshape(sh) / dt + div).max() / (np.abs(rho0).max() / dt)
+    Je = [np.zeros(nc) for _ in range(3)]
+    ora.deposit_esirkepov(g, n, q, dt, w, (x0, y0, z0), (x1, y1, z1), Je)
+    assert residual(Je) < 1e-13 and residual(J) > 1e-4
