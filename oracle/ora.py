@@ -61,6 +61,8 @@ def lib():
         L.ora_shape0.argtypes = [C.c_double]
         L.ora_gather_variant.argtypes = [G, C.c_int, C.c_int, C.c_longlong] + [_dp] * 15
         L.ora_smooth_binomial.argtypes = [G, C.c_int, _dp]
+        L.ora_gather_f32.argtypes = [G, C.c_int, C.c_int, C.c_longlong] + [_dp] * 15
+        L.ora_boris_f32.argtypes = [C.c_longlong, C.c_double, C.c_double, C.c_double] + [_dp] * 9
         L.ora_boris.argtypes = [C.c_longlong, C.c_double, C.c_double, C.c_double] + [_dp] * 9
         L.ora_move.argtypes = [C.c_longlong, C.c_double] + [_dp] * 9
         L.ora_deposit_esirkepov.argtypes = [G, C.c_int, C.c_longlong, C.c_double, C.c_double] + [_dp] * 10
@@ -135,6 +137,24 @@ def gather_variant(g: OraGrid, order: int, variant: int, x, y, z, E, B):
     _check(lib().ora_gather_variant(C.byref(g), order, variant, n, _d(x), _d(y), _d(z), *[_d(a) for a in F],
                                     *[_d(a) for a in out]), "gather_variant")
     return tuple(out)
+
+
+def gather_f32(g: OraGrid, order: int, variant: int, x, y, z, E, B):
+    """NEXT-4: the gather in single precision (shape and field values rounded to float); returns doubles."""
+    x, y, z = _f64(x), _f64(y), _f64(z)
+    n = x.size
+    F = [_f64(a) for a in (*E, *B)]
+    out = [np.empty(n) for _ in range(6)]
+    _check(lib().ora_gather_f32(C.byref(g), order, variant, n, _d(x), _d(y), _d(z), *[_d(a) for a in F],
+                                *[_d(a) for a in out]), "gather_f32")
+    return tuple(out)
+
+
+def boris_f32(q, m, dt, ux, uy, uz, Ep, Bp):
+    """NEXT-4: the Boris push in single precision, in place on doubles that hold float values."""
+    n = ux.size
+    _check(lib().ora_boris_f32(n, q, m, dt, _d(ux), _d(uy), _d(uz), *[_d(_f64(a)) for a in (*Ep, *Bp)]),
+           "boris_f32")
 
 
 def smooth_binomial(g: OraGrid, npass: int, F: np.ndarray):
@@ -225,10 +245,12 @@ class OracleSim:
     ZPAD = 4
 
     def __init__(self, nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, dt, order, nspecies, gather_variant=0,
-                 smooth_passes=0, open_z=False, deposit_variant=0):
+                 smooth_passes=0, open_z=False, deposit_variant=0, precision=0):
         if deposit_variant not in (0, 1):
             raise ValueError("deposit_variant must be 0 (Esirkepov) or 1 (direct)")
-        self.deposit_variant = int(deposit_variant)
+        if precision not in (0, 1):
+            raise ValueError("precision must be 0 (fp64) or 1 (fp32 fields and momenta, fp64 positions)")
+        self.deposit_variant, self.precision = int(deposit_variant), int(precision)
         self.open_z = bool(open_z)
         self.nz_phys = int(nz)
         self.pad = self.ZPAD if self.open_z else 0
@@ -334,11 +356,15 @@ class OracleSim:
             for sp in self.species:
                 if sp is None or sp.x.size == 0:
                     continue
-                if self.gather_variant:
-                    F = gather_variant(g, n, self.gather_variant, sp.x, sp.y, sp.z, self.E, self.B)
+                if self.precision:                 # NEXT-4: gather and push in fp32, the rest in fp64
+                    F = gather_f32(g, n, self.gather_variant, sp.x, sp.y, sp.z, self.E, self.B)
+                    boris_f32(sp.q, sp.m, dt, sp.ux, sp.uy, sp.uz, F[:3], F[3:])
                 else:
-                    F = gather(g, n, sp.x, sp.y, sp.z, self.E, self.B)             # step 1
-                boris(sp.q, sp.m, dt, sp.ux, sp.uy, sp.uz, F[:3], F[3:])          # step 2
+                    if self.gather_variant:
+                        F = gather_variant(g, n, self.gather_variant, sp.x, sp.y, sp.z, self.E, self.B)
+                    else:
+                        F = gather(g, n, sp.x, sp.y, sp.z, self.E, self.B)         # step 1
+                    boris(sp.q, sp.m, dt, sp.ux, sp.uy, sp.uz, F[:3], F[3:])      # step 2
                 x1, y1, z1 = move(dt, sp.x, sp.y, sp.z, sp.ux, sp.uy, sp.uz)      # step 3
                 if self.deposit_variant:
                     deposit_direct(g, n, sp.q, dt, sp.w, (sp.x, sp.y, sp.z), (x1, y1, z1), self.J)

@@ -193,6 +193,93 @@ int ora_smooth_binomial(const ora_grid* g, int npass, double* F)
     return 0;
 }
 
+/* ---- NEXT-4: mixed precision -- fp32 fields and momenta, fp64 positions ----------------
+ * The gather and the Boris push run in IEEE single precision; everything that touches a position (shape
+ * arguments, the move, the deposition) stays in double.
+ *  gather: the shape values are evaluated in double (they are functions of the fp64 position) and rounded to
+ *   float; the field values are rounded to float; products and the sum are float, in the same loop order as
+ *   ora_gather:  F_p = sum_k sum_j sum_i  fl(fl(fl(sx*sy)*sz) * F).
+ *  Boris: the formulas of ora_boris with every variable and constant a float (h, 1/c^2 rounded once from
+ *   double); momenta come in and go out as doubles that hold float values. */
+static float gather_one_f32(const ora_grid* g, int n, int n1, int n2, int n3, double xi, double eta, double zeta,
+                            double ox, double oy, double oz, const double* F)
+{
+    int h = window_h(n), wn = 2 * h + 2;
+    long long i0 = (long long)floor(xi), j0 = (long long)floor(eta), k0 = (long long)floor(zeta);
+    float sum = 0.0f;
+    for (int c = 0; c < wn; ++c) {
+        long long k = k0 - h + c;
+        float sz = (float)shape_any(n3, zeta - (double)k - oz);
+        for (int b = 0; b < wn; ++b) {
+            long long j = j0 - h + b;
+            float sy = (float)shape_any(n2, eta - (double)j - oy);
+            for (int a = 0; a < wn; ++a) {
+                long long i = i0 - h + a;
+                float sx = (float)shape_any(n1, xi - (double)i - ox);
+                float t = sx * sy;
+                t = t * sz;
+                t = t * (float)F[gidx(g, i, j, k)];
+                sum = sum + t;
+            }
+        }
+    }
+    return sum;
+}
+
+int ora_gather_f32(const ora_grid* g, int order, int variant, long long np,
+                   const double* x, const double* y, const double* z,
+                   const double* Ex, const double* Ey, const double* Ez,
+                   const double* Bx, const double* By, const double* Bz,
+                   double* Exp, double* Eyp, double* Ezp,
+                   double* Bxp, double* Byp, double* Bzp)
+{
+    if (order < 1 || order > 3 || variant < 0 || variant > 1) return -1;
+    int n = order, m = variant ? order - 1 : order;
+    double inv_dx = 1.0 / g->dx, inv_dy = 1.0 / g->dy, inv_dz = 1.0 / g->dz;
+    for (long long p = 0; p < np; ++p) {
+        double xi = (x[p] - g->xmin) * inv_dx;
+        double eta = (y[p] - g->ymin) * inv_dy;
+        double zeta = (z[p] - g->zmin) * inv_dz;
+        Exp[p] = (double)gather_one_f32(g, n, m, n, n, xi, eta, zeta, 0.5, 0.0, 0.0, Ex);
+        Eyp[p] = (double)gather_one_f32(g, n, n, m, n, xi, eta, zeta, 0.0, 0.5, 0.0, Ey);
+        Ezp[p] = (double)gather_one_f32(g, n, n, n, m, xi, eta, zeta, 0.0, 0.0, 0.5, Ez);
+        Bxp[p] = (double)gather_one_f32(g, n, n, m, m, xi, eta, zeta, 0.0, 0.5, 0.5, Bx);
+        Byp[p] = (double)gather_one_f32(g, n, m, n, m, xi, eta, zeta, 0.5, 0.0, 0.5, By);
+        Bzp[p] = (double)gather_one_f32(g, n, m, m, n, xi, eta, zeta, 0.5, 0.5, 0.0, Bz);
+    }
+    return 0;
+}
+
+int ora_boris_f32(long long np, double q, double m, double dt,
+                  double* ux, double* uy, double* uz,
+                  const double* Exp, const double* Eyp, const double* Ezp,
+                  const double* Bxp, const double* Byp, const double* Bzp)
+{
+    float h = (float)(q * dt / (2.0 * m));
+    float inv_c2 = (float)(1.0 / (ORA_C * ORA_C));
+    for (long long p = 0; p < np; ++p) {
+        float ex = (float)Exp[p], ey = (float)Eyp[p], ez = (float)Ezp[p];
+        float bx = (float)Bxp[p], by = (float)Byp[p], bz = (float)Bzp[p];
+        float umx = (float)ux[p] + h * ex;
+        float umy = (float)uy[p] + h * ey;
+        float umz = (float)uz[p] + h * ez;
+        float gam = sqrtf(1.0f + (umx * umx + umy * umy + umz * umz) * inv_c2);
+        float tx = h * bx / gam, ty = h * by / gam, tz = h * bz / gam;
+        float t2 = tx * tx + ty * ty + tz * tz;
+        float sx = 2.0f * tx / (1.0f + t2), sy = 2.0f * ty / (1.0f + t2), sz = 2.0f * tz / (1.0f + t2);
+        float upx = umx + (umy * tz - umz * ty);
+        float upy = umy + (umz * tx - umx * tz);
+        float upz = umz + (umx * ty - umy * tx);
+        float uqx = umx + (upy * sz - upz * sy);
+        float uqy = umy + (upz * sx - upx * sz);
+        float uqz = umz + (upx * sy - upy * sx);
+        ux[p] = (double)(uqx + h * ex);
+        uy[p] = (double)(uqy + h * ey);
+        uz[p] = (double)(uqz + h * ez);
+    }
+    return 0;
+}
+
 /* Boris (1970), relativistic form:
  *  h = q dt/(2m); u- = u + h E; gamma- = sqrt(1+|u-|^2/c^2); t = h B/gamma-;
  *  s = 2t/(1+|t|^2); u' = u- + u- x t; u+ = u- + u' x s; u_new = u+ + h E. */

@@ -79,6 +79,20 @@ int ora_gather_variant(const ora_grid* g, int order, int variant, long long np,
 /* Binomial (1-2-1) smoothing of one component in place, periodic; one pass = x, then y, then z. */
 int ora_smooth_binomial(const ora_grid* g, int npass, double* F);
 
+/* NEXT-4: mixed precision.  ora_gather_f32 = the gather (either variant) with shape values and
+ * field values rounded to float and float products / sums; ora_boris_f32 = ora_boris in float arithmetic.
+ * Momenta and gathered fields travel as doubles holding float values.  Positions are never touched by them. */
+int ora_gather_f32(const ora_grid* g, int order, int variant, long long np,
+                   const double* x, const double* y, const double* z,
+                   const double* Ex, const double* Ey, const double* Ez,
+                   const double* Bx, const double* By, const double* Bz,
+                   double* Exp, double* Eyp, double* Ezp,
+                   double* Bxp, double* Byp, double* Bzp);
+int ora_boris_f32(long long np, double q, double m, double dt,
+                  double* ux, double* uy, double* uz,
+                  const double* Exp, const double* Eyp, const double* Ezp,
+                  const double* Bxp, const double* Byp, const double* Bzp);
+
 /* Step 2: relativistic Boris push, u^{n-1/2} -> u^{n+1/2}, in place. */
 int ora_boris(long long np, double q, double m, double dt,
               double* ux, double* uy, double* uz,
