@@ -263,6 +263,14 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    order n-1 along every direction in which the gathered
  *                    component is staggered (
  *                    oracle: ora_gather_variant).  Both particle kernels.
+ *   "precision"      0 (default) = fp64 throughout (the contract of BASELINE.json);
+ *                    1 = mixed precision (NEXT-4; oracle: ora_gather_f32,
+ *                    ora_boris_f32): field values and shape weights are rounded
+ *                    to fp32 for the gather, the gather and the Boris push run
+ *                    in fp32, momenta are stored as doubles holding fp32 values;
+ *                    positions, the move, the deposition and the Yee update
+ *                    stay fp64 (charge conservation is untouched).  Tolerances
+ *                    against the oracle are those of fp32 arithmetic.
  *   "deposit_variant" 0 (default) = Esirkepov charge-conserving deposition; 1 =
  *                    direct deposition (NEXT-3; oracle: ora_deposit_direct): q w v
  *                    of the move, spread with the order-n shape at the middle

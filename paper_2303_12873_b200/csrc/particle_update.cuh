@@ -10,26 +10,29 @@
 namespace pic {
 
 // ---------------------------------------------------------------- gather ----
+__device__ __forceinline__ double fma_t(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float fma_t(float a, float b, float c) { return fmaf(a, b, c); }
+
 // One component: sum over the (NX+1)(NY+1)(NZ+1) support, factored z(y(x)).  The orders may differ per
-// direction (gather variant 1, below).
-template <int NX, int NY, int NZ>
-__device__ __forceinline__ double gather_comp(const double* __restrict__ F, const Grid& g, int fx, int fy, int fz,
-                                              const double (&wx)[NX + 1], const double (&wy)[NY + 1],
-                                              const double (&wz)[NZ + 1]) {
+// direction (gather variant 1, below).  T = arithmetic type: double, or float in the mixed-precision mode
+// (field values and weights rounded to float, float FMAs).
+template <int NX, int NY, int NZ, class T>
+__device__ __forceinline__ T gather_comp(const double* __restrict__ F, const Grid& g, int fx, int fy, int fz,
+                                         const T (&wx)[NX + 1], const T (&wy)[NY + 1], const T (&wz)[NZ + 1]) {
     const double* base = F + g.idx(fx, fy, fz);
-    double acc = 0.0;
+    T acc = T(0);
 #pragma unroll
     for (int c = 0; c <= NZ; ++c) {
-        double accy = 0.0;
+        T accy = T(0);
 #pragma unroll
         for (int b = 0; b <= NY; ++b) {
             const double* row = base + b * g.sy + c * g.sz;
-            double accx = 0.0;
+            T accx = T(0);
 #pragma unroll
-            for (int a = 0; a <= NX; ++a) accx = fma(wx[a], __ldg(row + a), accx);
-            accy = fma(wy[b], accx, accy);
+            for (int a = 0; a <= NX; ++a) accx = fma_t(wx[a], (T)__ldg(row + a), accx);
+            accy = fma_t(wy[b], accx, accy);
         }
-        acc = fma(wz[c], accy, acc);
+        acc = fma_t(wz[c], accy, acc);
     }
     return acc;
 }
@@ -42,21 +45,32 @@ struct GatherOrders {
     static constexpr int NS = GV ? N - 1 : N;      // order along a staggered direction
 };
 
+// shape weights in the arithmetic type of the gather: evaluated in double (they are functions of the fp64
+// position), then rounded
+template <int N, class T>
+__device__ __forceinline__ int shape_weights_t(double xi, T (&w)[N + 1]) {
+    double wd[N + 1];
+    const int f = shape_weights<N>(xi, wd);
+#pragma unroll
+    for (int a = 0; a <= N; ++a) w[a] = (T)wd[a];
+    return f;
+}
+
 // All six components from the padded GLOBAL arrays.
-template <int N, int GV>
+template <int N, int GV, class T>
 __device__ __forceinline__ void gather6_global(const Grid& g, const Fields& f, double xi, double et, double ze,
-                                               double (&eb)[6]) {
+                                               T (&eb)[6]) {
     constexpr int NS = GatherOrders<N, GV>::NS;
-    double wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[NS + 1], wys[NS + 1], wzs[NS + 1];
-    const int fxn = shape_weights<N>(xi, wxn), fyn = shape_weights<N>(et, wyn), fzn = shape_weights<N>(ze, wzn);
-    const int fxs = shape_weights<NS>(xi - 0.5, wxs), fys = shape_weights<NS>(et - 0.5, wys),
-              fzs = shape_weights<NS>(ze - 0.5, wzs);
-    eb[0] = gather_comp<NS, N, N>(f.Ex, g, fxs, fyn, fzn, wxs, wyn, wzn);
-    eb[1] = gather_comp<N, NS, N>(f.Ey, g, fxn, fys, fzn, wxn, wys, wzn);
-    eb[2] = gather_comp<N, N, NS>(f.Ez, g, fxn, fyn, fzs, wxn, wyn, wzs);
-    eb[3] = gather_comp<N, NS, NS>(f.Bx, g, fxn, fys, fzs, wxn, wys, wzs);
-    eb[4] = gather_comp<NS, N, NS>(f.By, g, fxs, fyn, fzs, wxs, wyn, wzs);
-    eb[5] = gather_comp<NS, NS, N>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
+    T wxn[N + 1], wyn[N + 1], wzn[N + 1], wxs[NS + 1], wys[NS + 1], wzs[NS + 1];
+    const int fxn = shape_weights_t<N, T>(xi, wxn), fyn = shape_weights_t<N, T>(et, wyn), fzn = shape_weights_t<N, T>(ze, wzn);
+    const int fxs = shape_weights_t<NS, T>(xi - 0.5, wxs), fys = shape_weights_t<NS, T>(et - 0.5, wys),
+              fzs = shape_weights_t<NS, T>(ze - 0.5, wzs);
+    eb[0] = gather_comp<NS, N, N, T>(f.Ex, g, fxs, fyn, fzn, wxs, wyn, wzn);
+    eb[1] = gather_comp<N, NS, N, T>(f.Ey, g, fxn, fys, fzn, wxn, wys, wzn);
+    eb[2] = gather_comp<N, N, NS, T>(f.Ez, g, fxn, fyn, fzs, wxn, wyn, wzs);
+    eb[3] = gather_comp<N, NS, NS, T>(f.Bx, g, fxn, fys, fzs, wxn, wys, wzs);
+    eb[4] = gather_comp<NS, N, NS, T>(f.By, g, fxs, fyn, fzs, wxs, wyn, wzs);
+    eb[5] = gather_comp<NS, NS, N, T>(f.Bz, g, fxs, fys, fzn, wxs, wys, wzn);
 }
 
 // Esirkepov deposition of one particle through an adder:
@@ -190,7 +204,7 @@ __device__ __forceinline__ void deposit_direct_global(const Grid& g, const Field
 
 // Device function used by both particle paths: the whole update of one
 // particle against the GLOBAL field arrays.  DV = 0: Esirkepov deposition; 1: direct deposition.
-template <int N, int GV, int DV = 0>
+template <int N, int GV, int DV = 0, class T = double>
 __device__ __forceinline__ void update_particle_global(const Grid& g, const Fields& f, const Particles& p,
                                                        long long ip, double q, double h, DevStatus* status) {
     const double x = p.x[ip], y = p.y[ip], z = p.z[ip];
@@ -198,13 +212,15 @@ __device__ __forceinline__ void update_particle_global(const Grid& g, const Fiel
     const double w = p.w[ip];
     // normalised coordinates: a subtraction then a multiplication (R30)
     const double xi = (x - g.xmin) * g.inv_dx, et = (y - g.ymin) * g.inv_dy, ze = (z - g.zmin) * g.inv_dz;
-    // step 1: gather
-    double eb[6];
-    gather6_global<N, GV>(g, f, xi, et, ze, eb);
-    const double ex = eb[0], ey = eb[1], ez = eb[2], bx = eb[3], by = eb[4], bz = eb[5];
-    // step 2: Boris
+    // step 1: gather, step 2: Boris -- in T (float in the mixed-precision mode: momenta are then doubles that hold floats)
+    T eb[6];
+    gather6_global<N, GV, T>(g, f, xi, et, ze, eb);
     const double inv_c2 = 1.0 / (C_LIGHT * C_LIGHT);
-    boris_push(h, inv_c2, ux, uy, uz, ex, ey, ez, bx, by, bz);
+    {
+        T tx = (T)ux, ty = (T)uy, tz = (T)uz;
+        boris_push<T>((T)h, (T)inv_c2, tx, ty, tz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
+        ux = (double)tx; uy = (double)ty; uz = (double)tz;
+    }
     // step 3: move (unwrapped)
     const double dtg = dt_over_gamma(g.dt, inv_c2, ux, uy, uz);
     const double x1 = x + dtg * ux, y1 = y + dtg * uy, z1 = z + dtg * uz;

@@ -12,35 +12,43 @@
 
 namespace pic {
 
-template <int N, int GV, int DV>
+template <int N, int GV, int DV, class T>
 __global__ void __launch_bounds__(128) particles_global_kernel(Grid g, Fields f, Particles p, long long n, double q,
                                                                double h, DevStatus* status) {
     long long ip = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (ip < n) update_particle_global<N, GV, DV>(g, f, p, ip, q, h, status);
+    if (ip < n) update_particle_global<N, GV, DV, T>(g, f, p, ip, q, h, status);
     if (ip == 0) atomicAdd(&status->n_global, (unsigned long long)n);
 }
 
-template <int GV, int DV>
+template <int GV, int DV, class T>
 static void launch_global_gv(const Grid& g, const Fields& f, const Particles& p, long long n, double q, double h,
                              int order, DevStatus* status, cudaStream_t st) {
     const int bs = 128;
     const unsigned nb = (unsigned)((n + bs - 1) / bs);
-    if (order == 1) particles_global_kernel<1, GV, DV><<<nb, bs, 0, st>>>(g, f, p, n, q, h, status);
-    else if (order == 2) particles_global_kernel<2, GV, DV><<<nb, bs, 0, st>>>(g, f, p, n, q, h, status);
-    else particles_global_kernel<3, GV, DV><<<nb, bs, 0, st>>>(g, f, p, n, q, h, status);
+    if (order == 1) particles_global_kernel<1, GV, DV, T><<<nb, bs, 0, st>>>(g, f, p, n, q, h, status);
+    else if (order == 2) particles_global_kernel<2, GV, DV, T><<<nb, bs, 0, st>>>(g, f, p, n, q, h, status);
+    else particles_global_kernel<3, GV, DV, T><<<nb, bs, 0, st>>>(g, f, p, n, q, h, status);
+}
+
+template <class T>
+static void launch_global_t(const Grid& g, const Fields& f, const Particles& p, long long n, double q, double h,
+                            int order, int gather_variant, int deposit_variant, DevStatus* status, cudaStream_t st) {
+    if (deposit_variant) {
+        if (gather_variant) launch_global_gv<1, 1, T>(g, f, p, n, q, h, order, status, st);
+        else launch_global_gv<0, 1, T>(g, f, p, n, q, h, order, status, st);
+    } else {
+        if (gather_variant) launch_global_gv<1, 0, T>(g, f, p, n, q, h, order, status, st);
+        else launch_global_gv<0, 0, T>(g, f, p, n, q, h, order, status, st);
+    }
 }
 
 void launch_particles_global(const Grid& g, const Fields& f, const Particles& p, long long n, double q, double m,
-                             int order, int gather_variant, int deposit_variant, DevStatus* status, cudaStream_t st) {
+                             int order, int gather_variant, int deposit_variant, int precision, DevStatus* status,
+                             cudaStream_t st) {
     if (n <= 0) return;
     const double h = q * g.dt / (2.0 * m);
-    if (deposit_variant) {
-        if (gather_variant) launch_global_gv<1, 1>(g, f, p, n, q, h, order, status, st);
-        else launch_global_gv<0, 1>(g, f, p, n, q, h, order, status, st);
-    } else {
-        if (gather_variant) launch_global_gv<1, 0>(g, f, p, n, q, h, order, status, st);
-        else launch_global_gv<0, 0>(g, f, p, n, q, h, order, status, st);
-    }
+    if (precision) launch_global_t<float>(g, f, p, n, q, h, order, gather_variant, deposit_variant, status, st);
+    else launch_global_t<double>(g, f, p, n, q, h, order, gather_variant, deposit_variant, status, st);
 }
 
 // ------------------------------------------------------------------- rho ----

@@ -60,8 +60,12 @@ struct FastWin {
 // that has moved since its last pic_sort, 0 right after a sort (every particle is in its listed cell), which
 // shrinks the stencil from 14 x 10 x 10 to 12 x 8 x 8 nodes per component so that TWO blocks fit one SM
 // and one block's prologue (stencil staging: every warp of the block waits) overlaps the other's particles.
-template <int TX_, int TY_, int TZ_, int NP_, int MINB_, int DRIFT_, int RING_, bool UG_>
+template <int TX_, int TY_, int TZ_, int NP_, int MINB_, int DRIFT_, int RING_, bool UG_, class FT_ = double>
 struct TileCfg {
+    // FT = type of the staged field stencil and of the gather / push arithmetic: double, or float in the
+    // mixed-precision mode (pic_set_option "precision" = 1)
+    using FT = FT_;
+    static_assert(!UG_ || sizeof(FT_) == 8, "the cell-anchored gather is written for the fp64 stencil");
     // NP producer warps (phase A) and NP consumer warps (phase B), paired one to one
     static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NP = NP_, NW = 2 * NP_, NT = 32 * NW, MINB = MINB_,
                          DRIFT = DRIFT_;
@@ -82,7 +86,9 @@ struct TileCfg {
     // One component occupies FP words; components that are nodal in x (Ey, Ez, Bx) never read x-slab 0
     // (their lowest node is i-1), so that slab is not stored: their base is shifted back by one slab.
     static constexpr int FP = (EX - 1) * SX + (EZ - 1) * SZ + EY;
-    static constexpr int TOT = 6 * FP - 3 * SX + ((6 * FP - 3 * SX) & 1);     // even: staging stays 16-byte aligned
+    static constexpr int TOT = 6 * FP - 3 * SX + ((6 * FP - 3 * SX) & 1);     // stencil words of type FT, even
+    // the stencil in units of doubles, rounded up to a 16-byte boundary: staging stays 16-byte aligned
+    static constexpr int TOT_D = ((TOT * (int)sizeof(FT) + 15) / 16) * 2;
     __host__ __device__ static constexpr bool trimmed(int k) { return k >= 1 && k <= 3; }
     __host__ __device__ static constexpr int comp_base(int k) {   // word of (x = 0, y = 0, z = 0), virtual for k = 1..3
         return k == 0 ? 0 : (k == 1 ? FP - SX : (k == 2 ? 2 * FP - 2 * SX : (k == 3 ? 3 * FP - 3 * SX
@@ -102,7 +108,7 @@ struct TileCfg {
     static constexpr int STG_W = BODY_W + TAIL_W + CODE_W + (CODE_W & 1) + SLOW_W + PBUF_W + TAB_W;
     static_assert(STG_W % 2 == 0 && BODY_W % 2 == 0, "staging layout: 16-byte alignment");
     static constexpr int NOFF = NROW * (TX + 1);
-    static constexpr size_t SMEM = sizeof(double) * ((size_t)TOT + (size_t)NP * STG_W) + sizeof(int) * (NOFF + 4);
+    static constexpr size_t SMEM = sizeof(double) * ((size_t)TOT_D + (size_t)NP * STG_W) + sizeof(int) * (NOFF + 4);
     static_assert(TX == 8, "phase B maps 8 cells x 4 planes onto a warp");
 };
 
@@ -227,16 +233,15 @@ __device__ __forceinline__ void place_uniform(const double (&w)[N + 1], int shif
 }
 
 // One z-plane of one component from the shared stencil: sum_b wy[b] sum_a wx[a] F[a,b].
-template <int WX, int WY, int PX, int PY, class C>
-__device__ __forceinline__ double gather_plane(const double* __restrict__ base, const double (&wx)[PX],
-                                               const double (&wy)[PY]) {
-    double accy = 0.0;
+template <int WX, int WY, int PX, int PY, class C, class T>
+__device__ __forceinline__ T gather_plane(const T* __restrict__ base, const T (&wx)[PX], const T (&wy)[PY]) {
+    T accy = T(0);
 #pragma unroll
     for (int b = 0; b < WY; ++b) {
-        double accx = 0.0;
+        T accx = T(0);
 #pragma unroll
-        for (int a = 0; a < WX; ++a) accx = fma(wx[a], base[b + C::SX * a], accx);
-        accy = fma(wy[b], accx, accy);
+        for (int a = 0; a < WX; ++a) accx = fma_t(wx[a], base[b + C::SX * a], accx);
+        accy = fma_t(wy[b], accx, accy);
     }
     return accy;
 }
@@ -252,6 +257,7 @@ __device__ __forceinline__ void gather6_cell(const double* __restrict__ Et, int 
                                              const double (&wxs)[UWin<N, GV>::WS], const double (&wys)[UWin<N, GV>::WS],
                                              double (&wzs)[UWin<N, GV>::ZT], double (&eb)[6]) {
     using U = UWin<N, GV>;
+    using FT = double;
     constexpr int WN = U::WN, WS = U::WS, ZT = U::ZT;
     const int o_ex = C::comp_base(0) + tile_word<C>(usx, uny, unz);
     const int o_ey = C::comp_base(1) + tile_word<C>(unx, usy, unz);
@@ -266,14 +272,14 @@ __device__ __forceinline__ void gather6_cell(const double* __restrict__ Et, int 
     for (int c = 0; c < ZT; ++c, pl += C::SZ) {
         const double zn = wzn[0], zs = wzs[0];
         if (WN == ZT || c < WN) {      // components that are nodal in z
-            eb[0] = fma(zn, gather_plane<WS, WN, WS, WN, C>(pl + o_ex, wxs, wyn), eb[0]);
-            eb[1] = fma(zn, gather_plane<WN, WS, WN, WS, C>(pl + o_ey, wxn, wys), eb[1]);
-            eb[5] = fma(zn, gather_plane<WS, WS, WS, WS, C>(pl + o_bz, wxs, wys), eb[5]);
+            eb[0] = fma(zn, gather_plane<WS, WN, WS, WN, C, FT>(pl + o_ex, wxs, wyn), eb[0]);
+            eb[1] = fma(zn, gather_plane<WN, WS, WN, WS, C, FT>(pl + o_ey, wxn, wys), eb[1]);
+            eb[5] = fma(zn, gather_plane<WS, WS, WS, WS, C, FT>(pl + o_bz, wxs, wys), eb[5]);
         }
         if (WS == ZT || c < WS) {      // components that are staggered in z
-            eb[2] = fma(zs, gather_plane<WN, WN, WN, WN, C>(pl + o_ez, wxn, wyn), eb[2]);
-            eb[3] = fma(zs, gather_plane<WN, WS, WN, WS, C>(pl + o_bx, wxn, wys), eb[3]);
-            eb[4] = fma(zs, gather_plane<WS, WN, WS, WN, C>(pl + o_by, wxs, wyn), eb[4]);
+            eb[2] = fma(zs, gather_plane<WN, WN, WN, WN, C, FT>(pl + o_ez, wxn, wyn), eb[2]);
+            eb[3] = fma(zs, gather_plane<WN, WS, WN, WS, C, FT>(pl + o_bx, wxn, wys), eb[3]);
+            eb[4] = fma(zs, gather_plane<WS, WN, WS, WN, C, FT>(pl + o_by, wxs, wyn), eb[4]);
         }
 #pragma unroll
         for (int k = 0; k < ZT - 1; ++k) { wzn[k] = wzn[k + 1]; wzs[k] = wzs[k + 1]; }
@@ -286,11 +292,13 @@ __device__ __forceinline__ void gather6_cell(const double* __restrict__ Et, int 
 // 384 loads at order 3, at 1.8 wavefronts each.  (g*n) / (f*s) = tile slot of the first nodal / staggered node per
 // dimension.  The z weights rotate through arrays padded to ZT = N + 1 entries.
 template <int N, int GV, class C>
-__device__ __forceinline__ void gather6_part(const double* __restrict__ Et, int gxn, int gyn, int gzn, int fxs,
-                                             int fys, int fzs, const double (&wxn)[N + 1], const double (&wyn)[N + 1],
-                                             double (&wzn)[N + 1], const double (&wxs)[GatherOrders<N, GV>::NS + 1],
-                                             const double (&wys)[GatherOrders<N, GV>::NS + 1], double (&wzs)[N + 1],
-                                             double (&eb)[6]) {
+__device__ __forceinline__ void gather6_part(const typename C::FT* __restrict__ Et, int gxn, int gyn, int gzn, int fxs,
+                                             int fys, int fzs, const typename C::FT (&wxn)[N + 1],
+                                             const typename C::FT (&wyn)[N + 1], typename C::FT (&wzn)[N + 1],
+                                             const typename C::FT (&wxs)[GatherOrders<N, GV>::NS + 1],
+                                             const typename C::FT (&wys)[GatherOrders<N, GV>::NS + 1],
+                                             typename C::FT (&wzs)[N + 1], typename C::FT (&eb)[6]) {
+    using FT = typename C::FT;
     constexpr int WN = N + 1, WS = GatherOrders<N, GV>::NS + 1;
     const int o_ex = C::comp_base(0) + tile_word<C>(fxs, gyn, gzn);
     const int o_ey = C::comp_base(1) + tile_word<C>(gxn, fys, gzn);
@@ -299,18 +307,18 @@ __device__ __forceinline__ void gather6_part(const double* __restrict__ Et, int 
     const int o_by = C::comp_base(4) + tile_word<C>(fxs, gyn, fzs);
     const int o_bz = C::comp_base(5) + tile_word<C>(fxs, fys, gzn);
 #pragma unroll
-    for (int k = 0; k < 6; ++k) eb[k] = 0.0;
-    const double* pl = Et;
+    for (int k = 0; k < 6; ++k) eb[k] = FT(0);
+    const FT* pl = Et;
 #pragma unroll 1
     for (int c = 0; c < WN; ++c, pl += C::SZ) {
-        const double zn = wzn[0], zs = wzs[0];
-        eb[0] = fma(zn, gather_plane<WS, WN, WS, WN, C>(pl + o_ex, wxs, wyn), eb[0]);
-        eb[1] = fma(zn, gather_plane<WN, WS, WN, WS, C>(pl + o_ey, wxn, wys), eb[1]);
-        eb[5] = fma(zn, gather_plane<WS, WS, WS, WS, C>(pl + o_bz, wxs, wys), eb[5]);
+        const FT zn = wzn[0], zs = wzs[0];
+        eb[0] = fma_t(zn, gather_plane<WS, WN, WS, WN, C, FT>(pl + o_ex, wxs, wyn), eb[0]);
+        eb[1] = fma_t(zn, gather_plane<WN, WS, WN, WS, C, FT>(pl + o_ey, wxn, wys), eb[1]);
+        eb[5] = fma_t(zn, gather_plane<WS, WS, WS, WS, C, FT>(pl + o_bz, wxs, wys), eb[5]);
         if (WS == WN || c < WS) {
-            eb[2] = fma(zs, gather_plane<WN, WN, WN, WN, C>(pl + o_ez, wxn, wyn), eb[2]);
-            eb[3] = fma(zs, gather_plane<WN, WS, WN, WS, C>(pl + o_bx, wxn, wys), eb[3]);
-            eb[4] = fma(zs, gather_plane<WS, WN, WS, WN, C>(pl + o_by, wxs, wyn), eb[4]);
+            eb[2] = fma_t(zs, gather_plane<WN, WN, WN, WN, C, FT>(pl + o_ez, wxn, wyn), eb[2]);
+            eb[3] = fma_t(zs, gather_plane<WN, WS, WN, WS, C, FT>(pl + o_bx, wxn, wys), eb[3]);
+            eb[4] = fma_t(zs, gather_plane<WS, WN, WS, WN, C, FT>(pl + o_by, wxs, wyn), eb[4]);
         }
 #pragma unroll
         for (int k = 0; k < N; ++k) { wzn[k] = wzn[k + 1]; wzs[k] = wzs[k + 1]; }
@@ -320,10 +328,10 @@ __device__ __forceinline__ void gather6_part(const double* __restrict__ Et, int 
 }
 
 // Gather of all six components from the padded GLOBAL arrays (particle outside the tile's halo).
-template <int N, int GV>
+template <int N, int GV, class T>
 __device__ __noinline__ void gather_global6(const Grid& g, const Fields& f, double xi, double et, double ze,
-                                            double (&eb)[6]) {
-    gather6_global<N, GV>(g, f, xi, et, ze, eb);
+                                            T (&eb)[6]) {
+    gather6_global<N, GV, T>(g, f, xi, et, ze, eb);
 }
 
 // tile-relative cell index with the periodic image nearest to the tile
@@ -758,11 +766,12 @@ __device__ __forceinline__ void tile_consumer(const Grid& g, const Fields& f, co
 template <int N, int GV, class C>
 __device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, const Particles& p, const Particles& po,
                                               const unsigned int* __restrict__ perm, unsigned int* __restrict__ key_out,
-                                              double q, double h, const double* __restrict__ Et, const Staging<C>& S,
+                                              double q, double h, const typename C::FT* __restrict__ Et, const Staging<C>& S,
                                               const int* row_off, int row_first, int t0x, int t0y, int t0z, int lane,
                                               DevStatus* status) {
     constexpr int FW = FastWin<N>::FW, FA = FastWin<N>::FA, DRIFT = C::DRIFT;
     using FR = FastRec<N>;
+    using FT = typename C::FT;
     const int* cp = S.cp;
     double* pbuf = S.pbuf;
     const int T = cp[C::NC];
@@ -832,7 +841,7 @@ __device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, co
                                  ry >= -DRIFT && ry <= C::TY - 1 + DRIFT && t0y + ry <= g.ny - 1 + DRIFT &&
                                  rz >= -DRIFT && rz <= C::TZ - 1 + DRIFT && t0z + rz <= g.nz - 1 + DRIFT;
             fxn = shape_weights<N>(xi, wxn); fyn = shape_weights<N>(et, wyn); fzn = shape_weights<N>(ze, wzn);
-            double eb[6];
+            FT eb[6];
             if (in_tile) {
                 constexpr int NS = GatherOrders<N, GV>::NS;
                 // from global node index to tile slot: slot = node - (t0 - GL) + image shift
@@ -850,19 +859,26 @@ __device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, co
                     gather6_cell<N, GV, C>(Et, ci + U::AN + shx, cj + U::AN + shy, ck + U::AN + shz, ci + U::AS + shx,
                                            cj + U::AS + shy, ck + U::AS + shz, uxn, uyn, uzn, uxs, uys, uzs, eb);
                 } else {
-                    double wxs[NS + 1], wys[NS + 1], ws[NS + 1], wzs[N + 1];
-                    const int fxs = shape_weights<NS>(xi - 0.5, wxs) + shx, fys = shape_weights<NS>(et - 0.5, wys) + shy,
-                              fzs = shape_weights<NS>(ze - 0.5, ws) + shz;
+                    // weights in the gather's arithmetic type (the fp64 nodal ones stay for the deposit record)
+                    FT gxn[N + 1], gyn[N + 1], gzn[N + 1], wxs[NS + 1], wys[NS + 1], ws[NS + 1], wzs[N + 1];
 #pragma unroll
-                    for (int k = 0; k <= N; ++k) wzs[k] = (k <= NS) ? ws[(k <= NS) ? k : 0] : 0.0;
-                    gather6_part<N, GV, C>(Et, fxn + shx, fyn + shy, fzn + shz, fxs, fys, fzs, wxn, wyn, wzn, wxs, wys,
+                    for (int k = 0; k <= N; ++k) { gxn[k] = (FT)wxn[k]; gyn[k] = (FT)wyn[k]; gzn[k] = (FT)wzn[k]; }
+                    const int fxs = shape_weights_t<NS, FT>(xi - 0.5, wxs) + shx, fys = shape_weights_t<NS, FT>(et - 0.5, wys) + shy,
+                              fzs = shape_weights_t<NS, FT>(ze - 0.5, ws) + shz;
+#pragma unroll
+                    for (int k = 0; k <= N; ++k) wzs[k] = (k <= NS) ? ws[(k <= NS) ? k : 0] : FT(0);
+                    gather6_part<N, GV, C>(Et, fxn + shx, fyn + shy, fzn + shz, fxs, fys, fzs, gxn, gyn, gzn, wxs, wys,
                                            wzs, eb);
                 }
             } else {
-                gather_global6<N, GV>(g, f, xi, et, ze, eb);
+                gather_global6<N, GV, FT>(g, f, xi, et, ze, eb);
                 ++n_glob;
             }
-            boris_push(h, inv_c2, ux, uy, uz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
+            {       // Boris in FT (mixed precision: the momenta are doubles that hold floats)
+                FT tx = (FT)ux, ty = (FT)uy, tz = (FT)uz;
+                boris_push<FT>((FT)h, (FT)inv_c2, tx, ty, tz, eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]);
+                ux = (double)tx; uy = (double)ty; uz = (double)tz;
+            }
             const double dtg = dt_over_gamma(g.dt, inv_c2, ux, uy, uz);
             const double x1 = x + dtg * ux, y1 = y + dtg * uy, z1 = z + dtg * uz;
             xi1 = (x1 - g.xmin) * g.inv_dx; et1 = (y1 - g.ymin) * g.inv_dy; ze1 = (z1 - g.zmin) * g.inv_dz;
@@ -962,8 +978,9 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                       unsigned int* __restrict__ key_out, double q, double h,
                       const unsigned int* __restrict__ cell_offset, int ntx, int nty, DevStatus* status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* Et = reinterpret_cast<double*>(smem_raw);            // TOT words: Ex Ey Ez Bx By Bz
-    double* stg_all = Et + C::TOT;                               // NP * STG_W
+    using FT = typename C::FT;
+    FT* Et = reinterpret_cast<FT*>(smem_raw);                    // TOT words of FT: Ex Ey Ez Bx By Bz
+    double* stg_all = reinterpret_cast<double*>(smem_raw) + C::TOT_D;   // NP * STG_W
     int* row_off = reinterpret_cast<int*>(stg_all + C::NP * C::STG_W);   // NROW x (TX+1) container indices
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1013,7 +1030,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
                 const int w = tile_word<C>(e % C::EX, (e / C::EX) % C::EY, e / (C::EX * C::EY));
 #pragma unroll
                 for (int cpt = 0; cpt < 6; ++cpt)
-                    if (!(C::trimmed(cpt) && e % C::EX == 0)) Et[C::comp_base(cpt) + w] = v[it][cpt];
+                    if (!(C::trimmed(cpt) && e % C::EX == 0)) Et[C::comp_base(cpt) + w] = (FT)v[it][cpt];
             }
         }
     }
@@ -1059,8 +1076,11 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
 // CfgDrift: a species that has moved since its last sort (particles up to one cell outside their listed
 // cell still gather from shared memory); one block of 6 + 6 warps per SM, tile 8 x 4 x 6.
 // CfgFresh: right after pic_sort; two blocks of 3 + 3 warps per SM, tile 8 x 4 x 6.
+// *32: the mixed-precision mode (fp32 stencil, gather and push; same tiles and rings).
 using CfgDrift = TileCfg<8, 4, 6, 6, 1, 1, 112, false>;
 using CfgFresh = TileCfg<8, 4, 6, 3, 2, 0, 120, false>;
+using CfgDrift32 = TileCfg<8, 4, 6, 6, 1, 1, 112, false, float>;
+using CfgFresh32 = TileCfg<8, 4, 6, 3, 2, 0, 120, false, float>;
 static_assert(2 * (CfgFresh::SMEM + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
 static_assert(CfgDrift::SMEM <= 227 * 1024, "the drift block must fit one SM");
 
@@ -1093,6 +1113,13 @@ cudaError_t setup_orders() {
     return e;
 }
 
+template <class Cfg>
+cudaError_t setup_cfg() {
+    cudaError_t e = setup_orders<0, Cfg>();
+    if (e == cudaSuccess) e = setup_orders<1, Cfg>();
+    return e;
+}
+
 template <int GV, class Cfg>
 void launch_orders(int order, const Grid& g, const Fields& f, const Particles& p, const Particles& po,
                    const unsigned int* perm, unsigned int* key_out, double q, double h, const unsigned int* cell_offset,
@@ -1102,28 +1129,36 @@ void launch_orders(int order, const Grid& g, const Fields& f, const Particles& p
     else launch_tile<3, GV, Cfg>(g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
 }
 
+template <class Cfg>
+void launch_cfg(int order, int gather_variant, const Grid& g, const Fields& f, const Particles& p, const Particles& po,
+                const unsigned int* perm, unsigned int* key_out, double q, double h, const unsigned int* cell_offset,
+                DevStatus* status, cudaStream_t st) {
+    if (gather_variant) launch_orders<1, Cfg>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+    else launch_orders<0, Cfg>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+}
+
 }  // namespace
 
 int tile_setup() {
-    cudaError_t e = setup_orders<0, CfgDrift>();
-    if (e == cudaSuccess) e = setup_orders<0, CfgFresh>();
-    if (e == cudaSuccess) e = setup_orders<1, CfgDrift>();
-    if (e == cudaSuccess) e = setup_orders<1, CfgFresh>();
+    cudaError_t e = setup_cfg<CfgDrift>();
+    if (e == cudaSuccess) e = setup_cfg<CfgFresh>();
+    if (e == cudaSuccess) e = setup_cfg<CfgDrift32>();
+    if (e == cudaSuccess) e = setup_cfg<CfgFresh32>();
     return (int)e;
 }
 
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& po,
                           const unsigned int* perm, unsigned int* key_out, long long n, double q, double m, int order,
-                          int gather_variant, const unsigned int* cell_offset, bool fresh, DevStatus* status,
-                          cudaStream_t st) {
+                          int gather_variant, int precision, const unsigned int* cell_offset, bool fresh,
+                          DevStatus* status, cudaStream_t st) {
     if (n <= 0) return 0;
     const double h = q * g.dt / (2.0 * m);
-    if (fresh) {
-        if (gather_variant) launch_orders<1, CfgFresh>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
-        else launch_orders<0, CfgFresh>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+    if (precision) {
+        if (fresh) launch_cfg<CfgFresh32>(order, gather_variant, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else launch_cfg<CfgDrift32>(order, gather_variant, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
     } else {
-        if (gather_variant) launch_orders<1, CfgDrift>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
-        else launch_orders<0, CfgDrift>(order, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        if (fresh) launch_cfg<CfgFresh>(order, gather_variant, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
+        else launch_cfg<CfgDrift>(order, gather_variant, g, f, p, po, perm, key_out, q, h, cell_offset, status, st);
     }
     return 1;
 }

@@ -70,6 +70,7 @@ struct pic_ctx {
     // options
     int stage_timing = 0, force_path = 0, yee_tma = 3, tile_fresh = 1, sort_deferred = 1, fuse_keys = 1;
     int gather_variant = 0, smooth_passes = 0, deposit_variant = 0;      // NEXT-3 options
+    int precision = 0;                              // NEXT-4: 1 = gather and Boris push in fp32
     unsigned long long id_base = 0;                 // ids given at load start here (bricks: unique across contexts)
     int absorb_mask = 0;                            // NEXT-2: dimensions whose faces are open ends (zero exterior, particles deleted)
     unsigned long long deleted = 0;                 // particles deleted at absorbing faces / by the moving window
@@ -556,7 +557,7 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
                     const bool keys = c->fuse_keys != 0;
                     c->launches += launch_particles_tile(g, c->f, P, PO, deferred ? S.perm : nullptr,
                                                          keys ? S.key : nullptr, S.n, S.q, S.m, c->order, c->gather_variant,
-                                                         S.cell_offset,
+                                                         c->precision, S.cell_offset,
                                                          S.steps_since_sort == 0 && c->tile_fresh != 0, c->status,
                                                          c->stream);
                     S.keys_valid = keys;
@@ -570,7 +571,7 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
                     materialize(c, S);
                     S.keys_valid = false;
                     launch_particles_global(g, c->f, S.buf[S.cur], S.n, S.q, S.m, c->order, c->gather_variant,
-                                            c->deposit_variant, c->status, c->stream);
+                                            c->deposit_variant, c->precision, c->status, c->stream);
                     c->launches += 1;
                 }
                 S.steps_since_sort += 1;
@@ -984,6 +985,9 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     } else if (!strcmp(name, "gather_variant")) {
         if (value < 0 || value > 1) return fail(c, PIC_EINVAL, "gather_variant must be 0 or 1");
         c->gather_variant = (int)value;
+    } else if (!strcmp(name, "precision")) {
+        if (value < 0 || value > 1) return fail(c, PIC_EINVAL, "precision must be 0 (fp64) or 1 (fp32 fields and momenta)");
+        c->precision = (int)value;
     } else if (!strcmp(name, "deposit_variant")) {
         if (value < 0 || value > 1) return fail(c, PIC_EINVAL, "deposit_variant must be 0 or 1");
         if (value && c->force_path == 2) return fail(c, PIC_ESTATE, "direct deposition runs in the global-atomic kernel: not with force_path = 2");

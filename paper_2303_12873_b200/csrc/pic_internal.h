@@ -73,9 +73,10 @@ int launch_smooth_binomial(const Grid& g, double* F, double* tmp, int npass, cud
 // gather + Boris + move + Esirkepov with global fp64 atomics + wrap; any particle order.
 // gather_variant: 0 = order n in every direction, 1 = order n-1 along a component's staggered directions
 // deposit_variant: 0 = Esirkepov (charge-conserving), 1 = direct deposition at the middle of the move
+// precision: 0 = fp64 throughout, 1 = gather and Boris push in fp32 (NEXT-4), positions and deposition in fp64
 void launch_particles_global(const Grid& g, const Fields& f, const Particles& p, long long n, double q,
-                             double m, int order, int gather_variant, int deposit_variant, DevStatus* status,
-                             cudaStream_t st);
+                             double m, int order, int gather_variant, int deposit_variant, int precision,
+                             DevStatus* status, cudaStream_t st);
 void launch_deposit_rho(const Grid& g, const Particles& p, long long n, double q, int order, double* rho_pad,
                         cudaStream_t st);
 void launch_fold_guards(const Grid& g, double* F, cudaStream_t st);       // sum periodic images into the interior
@@ -129,8 +130,8 @@ struct TileScratch {
 // key_out != nullptr: the kernel also writes the cell key of every particle's new position (for the next pic_sort)
 int launch_particles_tile(const Grid& g, const Fields& f, const Particles& p, const Particles& pout,
                           const unsigned int* perm, unsigned int* key_out, long long n, double q, double m, int order,
-                          int gather_variant, const unsigned int* cell_offset, bool fresh, DevStatus* status,
-                          cudaStream_t st);  // kernels launched
+                          int gather_variant, int precision, const unsigned int* cell_offset, bool fresh,
+                          DevStatus* status, cudaStream_t st);  // kernels launched
 int tile_setup();   // one-time cudaFuncSetAttribute calls; returns cudaError_t as int
 
 }  // namespace pic

@@ -52,17 +52,24 @@ __device__ __forceinline__ int shape_weights(double xi, double (&w)[N + 1]) {
 // instructions of a square root plus a division, and the fused kernel is bound by instruction latency.
 // Both particle kernels use this one formulation, so a particle's trajectory does not depend on
 // which path updated it (a few ulp away from the oracle's sqrt/divide form; the 1-step bound is 1e-12).
-__device__ __forceinline__ void boris_push(double h, double inv_c2, double& ux, double& uy, double& uz, double ex,
-                                           double ey, double ez, double bx, double by, double bz) {
-    const double umx = ux + h * ex, umy = uy + h * ey, umz = uz + h * ez;
-    const double hg = h * rsqrt(1.0 + (umx * umx + umy * umy + umz * umz) * inv_c2);
-    const double tx = hg * bx, ty = hg * by, tz = hg * bz;
-    const double t2 = tx * tx + ty * ty + tz * tz;
-    const double f = 2.0 * __drcp_rn(1.0 + t2);      // = RN(2 / (1 + t2)): the scaling by 2 is exact
-    const double sx = f * tx, sy = f * ty, sz = f * tz;
-    const double upx = umx + (umy * tz - umz * ty);
-    const double upy = umy + (umz * tx - umx * tz);
-    const double upz = umz + (umx * ty - umy * tx);
+__device__ __forceinline__ double rsqrt_t(double x) { return rsqrt(x); }
+__device__ __forceinline__ float rsqrt_t(float x) { return rsqrtf(x); }
+__device__ __forceinline__ double rcp_t(double x) { return __drcp_rn(x); }
+__device__ __forceinline__ float rcp_t(float x) { return __frcp_rn(x); }
+
+// T = double, or float for the mixed-precision mode (pic_set_option "precision" = 1): the
+// same formulas in single precision.
+template <class T>
+__device__ __forceinline__ void boris_push(T h, T inv_c2, T& ux, T& uy, T& uz, T ex, T ey, T ez, T bx, T by, T bz) {
+    const T umx = ux + h * ex, umy = uy + h * ey, umz = uz + h * ez;
+    const T hg = h * rsqrt_t(T(1) + (umx * umx + umy * umy + umz * umz) * inv_c2);
+    const T tx = hg * bx, ty = hg * by, tz = hg * bz;
+    const T t2 = tx * tx + ty * ty + tz * tz;
+    const T f = T(2) * rcp_t(T(1) + t2);      // = RN(2 / (1 + t2)): the scaling by 2 is exact
+    const T sx = f * tx, sy = f * ty, sz = f * tz;
+    const T upx = umx + (umy * tz - umz * ty);
+    const T upy = umy + (umz * tx - umx * tz);
+    const T upz = umz + (umx * ty - umy * tx);
     ux = umx + (upy * sz - upz * sy) + h * ex;
     uy = umy + (upz * sx - upx * sz) + h * ey;
     uz = umz + (upx * sy - upy * sx) + h * ez;
