@@ -31,7 +31,16 @@ __global__ void __launch_bounds__(256) hist_rank_kernel(long long n, const unsig
                                                         unsigned int* __restrict__ rank, unsigned int* count) {
     long long ip = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (ip >= n) return;
-    rank[ip] = atomicAdd(count + key[ip], 1u);
+    // The keys arrive in the order of the last sort, so a warp holds a handful of distinct cells: one atomic per
+    // distinct key and warp instead of one per particle (the kernel is bound by the rate of returned L2 atomics).
+    const unsigned int k = key[ip];
+    const unsigned int active = __activemask();
+    const unsigned int same = __match_any_sync(active, k);
+    const int leader = __ffs(same) - 1, lane = threadIdx.x & 31;
+    unsigned int base = 0;
+    if (lane == leader) base = atomicAdd(count + k, (unsigned int)__popc(same));
+    base = __shfl_sync(same, base, leader);
+    rank[ip] = base + (unsigned int)__popc(same & ((1u << lane) - 1u));
 }
 
 constexpr int SCAN_T = 256, SCAN_V = 8, SCAN_ITEMS = SCAN_T * SCAN_V;
