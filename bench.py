@@ -460,6 +460,48 @@ def run_ours(args):
     return 0
 
 
+def run_bricks(args):
+    """--bricks PX,PY,PZ: the same workload cut into PX x PY x PZ bricks that all live on THIS GPU and exchange halos and
+    particles through the C-ABI brick calls (NEXT-1).  It measures what the decomposition costs on
+    one GPU (pack / unpack / migration kernels, the per-face synchronisations, smaller launches); it is NOT a scaling
+    number.  Prints one JSON line of its own kind ("kind": "bricks_on_one_gpu")."""
+    import torch
+    from paper_2303_12873_b200 import bricks as B
+    from paper_2303_12873_b200 import workloads as W
+    from paper_2303_12873_b200.binding import Sim
+    torch.cuda.set_device(0)
+    procs = tuple(int(v) for v in args.bricks.split(","))
+    kw = {"n": args.n} if args.n is not None else {}
+    wl = W.config(args.config, parity=False, **kw)
+    lay = B.BrickLayout(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, 0.0, 0.0, 0.0, procs)
+    sims, _ = B.make_local_bricks(Sim, lay, wl, slack=1.15)
+    st = B.BrickStepper(lay, sims, B.LocalTransport(range(lay.size)), len(wl.species), leaver_capacity=1 << 21)
+    st.start()
+    for s in sims.values():
+        s.sort()
+    for _ in range(args.warmup):
+        st.step()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        st.step()
+    ev1.record()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    ms = ev0.elapsed_time(ev1) / args.steps
+    n_now = sum(s.get_particles(0)["x"].size for s in sims.values()) if lay.size <= 2 else None
+    print(json.dumps({"kind": "bricks_on_one_gpu", "metric": METRIC, "value": wl.nparticles / (ms * 1e-3), "unit": UNIT,
+                      "ms_per_step": ms, "wall_ms_per_step": 1e3 * wall / args.steps, "steps": args.steps,
+                      "warmup": args.warmup, "n_gpus": 1, "scaling": "none: every brick runs on the same GPU",
+                      "config": {"workload": "configs[%d]" % args.config, "grid": [wl.nx, wl.ny, wl.nz],
+                                 "particles": wl.nparticles, "bricks": list(procs), "brick_cells": list(lay.nl),
+                                 "sort": "every step, per brick"},
+                      "particles_after": n_now}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -474,6 +516,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
                     help="pic_set_option(NAME, VALUE) before the run (experiments: force_path=1, gather_variant=1, ...)")
+    ap.add_argument("--bricks", default=None, metavar="PX,PY,PZ",
+                    help="cost of the brick decomposition on ONE GPU (NEXT-1): every brick a context on this GPU")
     ap.add_argument("--oracle-worker", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--oracle-budget", type=float, default=8.0, help=argparse.SUPPRESS)
     ap.add_argument("--oracle-core", type=int, default=-1, help=argparse.SUPPRESS)
@@ -485,6 +529,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.bricks:
+        return run_bricks(args)
     return run_ours(args)
 
 

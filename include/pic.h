@@ -330,7 +330,10 @@ int pic_set_option(pic_ctx*, const char* name, long long value);
  *   >= max (side 1) along dim are removed from the container and written to
  *   buf (DEVICE, 8 doubles each: x y z ux uy uz w and the id's bit pattern);
  *   *count = how many.  PIC_ENOMEM (container unchanged) if more than
- *   `capacity` leave.  Synchronises.  The species counts as unsorted afterwards.
+ *   `capacity` (or a third of the species' np_max, the size of the library's
+ *   index scratch) leave.  In place: one coordinate of every particle is read,
+ *   the holes are filled from the end of the container.  Synchronises once.  The
+ *   species counts as unsorted afterwards.
  * pic_import_arrivals: appends `count` such records, their positions shifted by
  *   (shift_x, shift_y, shift_z) (the box length when the face is the periodic
  *   seam of the whole domain, else 0).  PIC_ENOMEM if they do not fit np_max.

@@ -64,47 +64,69 @@ __global__ void add_plane_kernel(Grid g, double* F, int k, const double* __restr
     if (i < g.nx) F[g.idx(i, j, k)] += values[i + (long long)g.nx * j];
 }
 
-__global__ void split_leavers_kernel(Grid g, Particles src, Particles dst, long long n, int dim, int side, double* out,
-                                     long long capacity, unsigned long long* counters) {
+// ---- leavers: taken out of the container IN PLACE ------------------------------------------------------------
+// Only a sliver of a brick's particles leaves through a face in one step, so the container is not copied: pass 1
+// reads ONE coordinate of every particle, appends the index of every leaver to a list and its record to the
+// message (8 B per particle instead of 128); the holes the leavers leave below the new end n' = n - L are then
+// filled with the stayers found among the last L places (lists of L entries).  The order of the container
+// changes: the species counts as unsorted afterwards.
+__global__ void find_leavers_kernel(Grid g, Particles p, long long n, int dim, int side, double* out, long long capacity,
+                                    unsigned int* leaver_idx, unsigned long long* counters) {
     const long long ip = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
-    bool leaves = false, valid = ip < n;
-    double v[7] = {0, 0, 0, 0, 0, 0, 0};
-    unsigned long long id = 0;
-    if (valid) {
-        v[0] = src.x[ip]; v[1] = src.y[ip]; v[2] = src.z[ip]; v[3] = src.ux[ip]; v[4] = src.uy[ip]; v[5] = src.uz[ip];
-        v[6] = src.w[ip];
-        id = src.id[ip];
-        const double pos = v[dim];
+    bool leaves = false;
+    if (ip < n) {
+        const double pos = (dim == 0) ? p.x[ip] : ((dim == 1) ? p.y[ip] : p.z[ip]);
         const double lo = (dim == 0) ? g.xmin : ((dim == 1) ? g.ymin : g.zmin);
         const double hi = (dim == 0) ? g.xmax : ((dim == 1) ? g.ymax : g.zmax);
         leaves = side ? (pos >= hi) : (pos < lo);
     }
-    // one atomic per warp and destination; the order inside a warp is kept
     const unsigned active = __activemask();
-    const unsigned m_leave = __ballot_sync(active, valid && leaves), m_stay = __ballot_sync(active, valid && !leaves);
-    unsigned long long base_l = 0, base_s = 0;
-    if (lane == __ffs(active) - 1) {
-        if (m_leave) base_l = atomicAdd(&counters[0], (unsigned long long)__popc(m_leave));
-        if (m_stay) base_s = atomicAdd(&counters[1], (unsigned long long)__popc(m_stay));
-    }
-    base_l = __shfl_sync(active, base_l, __ffs(active) - 1);
-    base_s = __shfl_sync(active, base_s, __ffs(active) - 1);
-    const unsigned below = (1u << lane) - 1u;
-    if (valid && leaves) {
-        const long long k = (long long)base_l + __popc(m_leave & below);
+    const unsigned m = __ballot_sync(active, leaves);
+    if (!m) return;
+    const int leader = __ffs(active) - 1;
+    unsigned long long base = 0;
+    if (lane == leader) base = atomicAdd(&counters[0], (unsigned long long)__popc(m));
+    base = __shfl_sync(active, base, leader);
+    if (leaves) {
+        const long long k = (long long)base + __popc(m & ((1u << lane) - 1u));
         if (k < capacity) {
-            double* r = out + 8 * k;
-#pragma unroll
-            for (int a = 0; a < 7; ++a) r[a] = v[a];
-            r[7] = __longlong_as_double((long long)id);
+            leaver_idx[k] = (unsigned int)ip;
+            if (out) {
+                double* r = out + 8 * k;
+                r[0] = p.x[ip]; r[1] = p.y[ip]; r[2] = p.z[ip]; r[3] = p.ux[ip]; r[4] = p.uy[ip]; r[5] = p.uz[ip];
+                r[6] = p.w[ip];
+                r[7] = __longlong_as_double((long long)p.id[ip]);
+            }
         }
-    } else if (valid) {
-        const long long k = (long long)base_s + __popc(m_stay & below);
-        dst.x[k] = v[0]; dst.y[k] = v[1]; dst.z[k] = v[2]; dst.ux[k] = v[3]; dst.uy[k] = v[4]; dst.uz[k] = v[5];
-        dst.w[k] = v[6];
-        dst.id[k] = id;
     }
+}
+
+// tailflag[j] = 1 if place n' + j holds a leaver
+__global__ void mark_tail_kernel(const unsigned int* leaver_idx, long long L, long long nprime, unsigned int* tailflag) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < L && (long long)leaver_idx[k] >= nprime) tailflag[(long long)leaver_idx[k] - nprime] = 1u;
+}
+
+// fillers = the stayers among the last L places
+__global__ void list_fillers_kernel(const unsigned int* tailflag, long long L, long long nprime, unsigned int* fillers,
+                                    unsigned long long* counters) {
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < L && !tailflag[j]) fillers[atomicAdd(&counters[1], 1ull)] = (unsigned int)(nprime + j);
+}
+
+// every hole below n' receives one filler
+__global__ void fill_holes_kernel(Particles p, const unsigned int* leaver_idx, long long L, long long nprime,
+                                  const unsigned int* fillers, unsigned long long* counters) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= L) return;
+    const long long hole = leaver_idx[k];
+    if (hole >= nprime) return;
+    const long long src = fillers[atomicAdd(&counters[2], 1ull)];
+    p.x[hole] = p.x[src]; p.y[hole] = p.y[src]; p.z[hole] = p.z[src];
+    p.ux[hole] = p.ux[src]; p.uy[hole] = p.uy[src]; p.uz[hole] = p.uz[src];
+    p.w[hole] = p.w[src];
+    p.id[hole] = p.id[src];
 }
 
 __global__ void append_arrivals_kernel(Particles dst, long long at, const double* in, long long count, double sx,
@@ -154,10 +176,22 @@ void launch_add_plane(const Grid& g, double* F, int k, const double* values_dev,
     add_plane_kernel<<<nb, bs, 0, st>>>(g, F, k, values_dev);
 }
 
-void launch_split_leavers(const Grid& g, const Particles& src, const Particles& dst, long long n, int dim, int side,
-                          double* out, long long capacity, unsigned long long* counters, cudaStream_t st) {
+void launch_find_leavers(const Grid& g, const Particles& p, long long n, int dim, int side, double* out,
+                         long long capacity, unsigned int* leaver_idx, unsigned long long* counters, cudaStream_t st) {
     if (n <= 0) return;
-    split_leavers_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g, src, dst, n, dim, side, out, capacity, counters);
+    find_leavers_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g, p, n, dim, side, out, capacity, leaver_idx, counters);
+}
+
+int launch_close_holes(const Particles& p, long long n, long long L, const unsigned int* leaver_idx, unsigned int* tailflag,
+                       unsigned int* fillers, unsigned long long* counters, cudaStream_t st) {
+    if (L <= 0) return 0;
+    const long long nprime = n - L;
+    const unsigned nb = (unsigned)((L + 255) / 256);
+    cudaMemsetAsync(tailflag, 0, (size_t)L * sizeof(unsigned int), st);
+    mark_tail_kernel<<<nb, 256, 0, st>>>(leaver_idx, L, nprime, tailflag);
+    list_fillers_kernel<<<nb, 256, 0, st>>>(tailflag, L, nprime, fillers, counters);
+    fill_holes_kernel<<<nb, 256, 0, st>>>(p, leaver_idx, L, nprime, fillers, counters);
+    return 3;
 }
 
 void launch_append_arrivals(const Particles& dst, long long at, const double* in, long long count, double sx, double sy,

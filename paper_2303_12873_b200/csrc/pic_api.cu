@@ -3,6 +3,8 @@
 // the per-step launch sequence of SURVEY 8(c.1) steps 1-8.
 #include <math.h>
 #include <stdarg.h>
+
+#include <algorithm>
 #include <stdio.h>
 #include <string.h>
 
@@ -462,29 +464,43 @@ static void zero_absorbing_guards(pic_ctx* c, int group) {
             }
 }
 
-// particles of one species beyond face (dim, side) are removed (container compacted).  Synchronises.
-static int discard_leavers(pic_ctx* c, Species& S, int dim, int side, long long* count) {
+// Particles of one species beyond face (dim, side) are taken out of the container in place (bricks.cu); their records go
+// to out (device, 8 doubles each) if given.  More than `capacity` leavers: PIC_ENOMEM, container unchanged.
+// Synchronises once (the count).
+static int take_leavers(pic_ctx* c, Species& S, int dim, int side, double* out, long long capacity, long long* count) {
     *count = 0;
     if (!S.loaded || S.n == 0) return PIC_OK;
     materialize(c, S);
+    // scratch: the sort's rank array holds the leaver list, the tail flags and the filler list (a third each)
+    const long long cap = std::min<long long>(capacity, S.np_max / 3);
+    unsigned int* leaver_idx = c->sort_scratch.rank;
+    unsigned int* tailflag = leaver_idx + S.np_max / 3;
+    unsigned int* fillers = tailflag + S.np_max / 3;
     unsigned long long* counters = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(c->status) + 128);
-    CU(c, cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), c->stream));
-    launch_split_leavers(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, dim, side, nullptr, 0, counters, c->stream);
+    CU(c, cudaMemsetAsync(counters, 0, 3 * sizeof(unsigned long long), c->stream));
+    launch_find_leavers(c->g, S.buf[S.cur], S.n, dim, side, out, cap, leaver_idx, counters, c->stream);
     c->launches += 1;
-    unsigned long long h[2];
-    CU(c, cudaMemcpyAsync(h, counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    unsigned long long L = 0;
+    CU(c, cudaMemcpyAsync(&L, counters, sizeof(L), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
-    if (h[0] + h[1] != (unsigned long long)S.n) return fail(c, PIC_ECUDA, "leaver split lost particles");
-    *count = (long long)h[0];
-    if (h[0] > 0) {
-        S.cur ^= 1;
-        S.n = (long long)h[1];
+    if ((long long)L > cap)
+        return fail(c, PIC_ENOMEM, "%llu particles leave through this face, room for %lld (buffer, or np_max / 3)", L, cap);
+    *count = (long long)L;
+    if (L > 0) {
+        c->launches += launch_close_holes(S.buf[S.cur], S.n, (long long)L, leaver_idx, tailflag, fillers, counters, c->stream);
+        S.n -= (long long)L;
         S.sorted = false;
         S.keys_valid = false;
         S.degraded = false;
-        c->deleted += h[0];
     }
+    CU(c, cudaGetLastError());
     return PIC_OK;
+}
+
+static int discard_leavers(pic_ctx* c, Species& S, int dim, int side, long long* count) {
+    int rc = take_leavers(c, S, dim, side, nullptr, S.np_max / 3, count);
+    if (rc == PIC_OK) c->deleted += (unsigned long long)*count;
+    return rc;
 }
 
 static int discard_at_absorbing_faces(pic_ctx* c) {
@@ -703,29 +719,7 @@ int pic_export_leavers(pic_ctx* c, int species, int dim, int side, double* buf_d
         capacity < 0 || (capacity > 0 && !buf_dev))
         return fail(c, PIC_EINVAL, "bad argument of pic_export_leavers");
     Species& S = c->sp[species];
-    *count = 0;
-    if (!S.loaded || S.n == 0) return PIC_OK;
-    materialize(c, S);
-    // two 64-bit counters in the unused half of the 256-byte status block
-    unsigned long long* counters = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(c->status) + 128);
-    CU(c, cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), c->stream));
-    launch_split_leavers(c->g, S.buf[S.cur], S.buf[S.cur ^ 1], S.n, dim, side, buf_dev, capacity, counters, c->stream);
-    c->launches += 1;
-    unsigned long long h[2];
-    CU(c, cudaMemcpyAsync(h, counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    if ((long long)h[0] > capacity)      // nothing was lost: the source buffer is still the current one
-        return fail(c, PIC_ENOMEM, "%llu particles leave through this face, the buffer holds %lld", h[0], capacity);
-    if (h[0] + h[1] != (unsigned long long)S.n) return fail(c, PIC_ECUDA, "leaver split lost particles");
-    *count = (long long)h[0];
-    if (h[0] > 0) {
-        S.cur ^= 1;
-        S.n = (long long)h[1];
-        S.sorted = false;
-        S.keys_valid = false;
-        S.degraded = false;
-    }
-    return PIC_OK;
+    return take_leavers(c, S, dim, side, buf_dev, capacity, count);
 }
 
 int pic_import_arrivals(pic_ctx* c, int species, const double* buf_dev, long long count, double shift_x, double shift_y,

@@ -94,10 +94,14 @@ void launch_halo_unpack(const Grid& g, double* F, int dim, int first_layer, cons
 void launch_halo_fill(const Grid& g, double* F, int dim, int first_layer, double value, cudaStream_t st);
 void launch_shift_z(const Grid& g, double* F, int ncells, cudaStream_t st);          // moving window (NEXT-2)
 void launch_add_plane(const Grid& g, double* F, int k, const double* values_dev, cudaStream_t st);
-// leavers of face (dim, side) -> out[8 * k .. 8 * k + 7] = x y z ux uy uz w id; everything else -> dst (compacted);
-// counters[0] = leavers, counters[1] = stayers (device, zeroed by the caller)
-void launch_split_leavers(const Grid& g, const Particles& src, const Particles& dst, long long n, int dim, int side,
-                          double* out, long long capacity, unsigned long long* counters, cudaStream_t st);
+// Leavers of face (dim, side), in place: find_leavers appends their indices to leaver_idx (and their 8-double records
+// x y z ux uy uz w id to out, if given) and counts them in counters[0] (device, zeroed by the caller; entries beyond
+// `capacity` are counted but not stored); close_holes then moves the stayers among the last L places into the holes
+// below n - L (tailflag, fillers: scratch of L entries each; counters[1], counters[2] zeroed by the caller).
+void launch_find_leavers(const Grid& g, const Particles& p, long long n, int dim, int side, double* out,
+                         long long capacity, unsigned int* leaver_idx, unsigned long long* counters, cudaStream_t st);
+int launch_close_holes(const Particles& p, long long n, long long L, const unsigned int* leaver_idx, unsigned int* tailflag,
+                       unsigned int* fillers, unsigned long long* counters, cudaStream_t st);
 void launch_append_arrivals(const Particles& dst, long long at, const double* in, long long count, double sx, double sy,
                             double sz, cudaStream_t st);
 
