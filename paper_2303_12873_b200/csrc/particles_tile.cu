@@ -1075,7 +1075,9 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
 
 // CfgDrift: a species that has moved since its last sort (particles up to one cell outside their listed
 // cell still gather from shared memory); one block of 6 + 6 warps per SM, tile 8 x 4 x 6.
-// CfgFresh: right after pic_sort; two blocks of 3 + 3 warps per SM, tile 8 x 4 x 6.
+// CfgFresh: right after pic_sort; two blocks of 3 + 3 warps per SM, tile 8 x 4 x 6.  (Measured and dropped,
+// profiles/r02_tile_kernel.md: one consumer for two producers -- its duty is 56 % -- at 4 + 2 warps per block runs at
+// 34.2 instead of 29.2 ms: decoupling two producers needs rings two rows deep, which shared memory does not have.)
 // *32: the mixed-precision mode (fp32 stencil, gather and push; same tiles and rings).
 using CfgDrift = TileCfg<8, 4, 6, 6, 1, 1, 112, false>;
 using CfgFresh = TileCfg<8, 4, 6, 3, 2, 0, 120, false>;
