@@ -113,12 +113,17 @@ class LocalTransport:
 
 
 class DistTransport:
-    """One brick per rank of a torch.distributed group; neighbour-to-neighbour isend / irecv only."""
+    """One brick per rank of a torch.distributed group; neighbour-to-neighbour isend / irecv only.  With the NCCL backend
+    the device buffers travel as they are (NVLink / NVSwitch peer transfers); with gloo (the CPU test, and two processes
+    sharing one GPU) they are staged through host memory."""
 
-    def __init__(self, dist, rank, device):
+    def __init__(self, dist, rank, device, stage_through_host=None):
         self.dist, self.rank, self.device = dist, int(rank), device
         import torch
         self.torch = torch
+        if stage_through_host is None:
+            stage_through_host = dist.get_backend() != "nccl"
+        self.host = bool(stage_through_host)
 
     @staticmethod
     def _tag(key):
@@ -128,28 +133,37 @@ class DistTransport:
     def exchange(self, sends, recv_like=None):
         """sends: [(src == my rank, dst, key, tensor)]; recv_like: {(src, key): empty tensor to receive into} for the
         messages this rank expects, keyed by the face they arrive at.  Returns {(my rank, key): tensor}."""
-        ops, out = [], {}
+        ops, out, landed = [], {}, []
         for (src, key), buf in (recv_like or {}).items():
             if src == self.rank:
                 continue
-            ops.append(self.dist.P2POp(self.dist.irecv, buf, src, tag=self._tag(key)))
+            tmp = self.torch.empty(buf.shape, dtype=buf.dtype) if (self.host and buf.is_cuda) else buf
+            ops.append(self.dist.P2POp(self.dist.irecv, tmp, src, tag=self._tag(key)))
+            if tmp is not buf:
+                landed.append((tmp, buf))
             out[(self.rank, key)] = buf
         for (src, dst, key, t) in sends:
             assert src == self.rank
             if dst == self.rank:                     # a brick that is its own neighbour (never with procs > 1)
                 out[(dst, key)] = t
                 continue
-            ops.append(self.dist.P2POp(self.dist.isend, t.contiguous(), dst, tag=self._tag(key)))
+            t = t.contiguous()
+            if self.host and t.is_cuda:
+                t = t.cpu()
+            ops.append(self.dist.P2POp(self.dist.isend, t, dst, tag=self._tag(key)))
         if ops:
             for r in self.dist.batch_isend_irecv(ops):
                 r.wait()
+        for tmp, buf in landed:
+            buf.copy_(tmp)
         return out
 
     def exchange_counts(self, sends, expect):
         """sends: [(src, dst, key, n)]; expect: [(src, key)] faces this rank receives on.  Returns {(rank, key): n}."""
         t = self.torch
-        bufs = {(src, key): t.zeros(1, dtype=t.int64, device=self.device) for (src, key) in expect}
-        msgs = [(src, dst, key, t.tensor([int(n)], dtype=t.int64, device=self.device)) for (src, dst, key, n) in sends]
+        dev = "cpu" if self.host else self.device
+        bufs = {(src, key): t.zeros(1, dtype=t.int64, device=dev) for (src, key) in expect}
+        msgs = [(src, dst, key, t.tensor([int(n)], dtype=t.int64, device=dev)) for (src, dst, key, n) in sends]
         got = self.exchange(msgs, bufs)
         return {k: int(v.item()) for k, v in got.items()}
 
