@@ -66,7 +66,7 @@ enum {
 #define PIC_NG 4 /* guard cells per side of every internal field array */
 
 /* Number of entries written by pic_get_counters. */
-#define PIC_NCOUNTERS 8
+#define PIC_NCOUNTERS 9
 
 /* Number of entries written by pic_get_stage_ms. */
 #define PIC_NSTAGES 8
@@ -202,6 +202,7 @@ int pic_get_cell_offsets(pic_ctx*, int species, unsigned int* offsets, int dst_o
  *       then holds a warning
  *   [7] particle launches that ran the global-atomic kernel for a SORTED
  *       species because the drift watch (option "drift_watch") found it stale
+ *   [8] particles deleted at open ends ("absorb_mask") and by pic_shift_window
  */
 int pic_get_counters(pic_ctx*, unsigned long long* counters /*host*/);
 

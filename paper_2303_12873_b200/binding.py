@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpic_b200.so")
 
 PIC_OK, PIC_EINVAL, PIC_ENOMEM, PIC_ECUDA, PIC_ESTATE, PIC_EPHYS = 0, -1, -2, -3, -4, -5
-PIC_NCOUNTERS = 8
+PIC_NCOUNTERS = 9
 PIC_NSTAGES = 8
 _CODE_NAMES = {0: "PIC_OK", -1: "PIC_EINVAL", -2: "PIC_ENOMEM", -3: "PIC_ECUDA", -4: "PIC_ESTATE",
                -5: "PIC_EPHYS"}
@@ -286,7 +286,7 @@ class Sim:
         self._check(self._L.pic_get_counters(self._ctx, arr), "pic_get_counters")
         v = list(arr)
         return {"fast": v[0], "slow": v[1], "global": v[2], "launches": v[3], "steps": v[4], "sorts": v[5],
-                "yee_tma": v[6], "fallbacks": v[7]}
+                "yee_tma": v[6], "fallbacks": v[7], "deleted": v[8]}
 
     # -- NEXT-1: brick calls (device buffers = torch.cuda float64 tensors) -------------------------
     def step_stage(self, stage):

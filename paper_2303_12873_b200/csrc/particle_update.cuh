@@ -233,7 +233,7 @@ __device__ __forceinline__ void update_particle_global(const Grid& g, const Fiel
     } else {
         if (!bad && q != 0.0) deposit_global<N>(g, f, xi, et, ze, xi1, et1, ze1, q * w, bad);
     }
-    if (bad) status->ephys = 1;
+    if (bad) atomicOr(&status->ephys, 1);
     // step 5: wrap and store
     p.x[ip] = wrap1(x1, g.xmin, g.xmax, g.Lx, g.open_mask & 1);
     p.y[ip] = wrap1(y1, g.ymin, g.ymax, g.Ly, g.open_mask & 2);

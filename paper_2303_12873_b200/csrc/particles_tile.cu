@@ -709,6 +709,12 @@ struct Staging {
 };
 
 // ---- consumer warp: phase B and the flush of every row of its producer's stream -------------------------
+// A producer does not wait for ring space for ever: after SPIN_LIMIT polls (seconds; a row takes microseconds) it sets
+// bit 1 of the status flag, which the next synchronising call turns into a sticky PIC_ECUDA, publishes its whole stream
+// as staged so that its consumer drains and leaves, and returns.  The consumer itself only ever waits for its producer,
+// which always publishes the end of its stream (a guard inside the consumer's poll loop cost 4 % of the launch).
+constexpr int SPIN_LIMIT = 1 << 24;
+
 template <int N, class C>
 __device__ __forceinline__ void tile_consumer(const Grid& g, const Fields& f, const Staging<C>& S, const int* row_off,
                                               int row_first, int t0x, int t0y, int t0z, int lane) {
@@ -909,7 +915,14 @@ __device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, co
             if (in_tile) { if (is_slow) ++n_slow; else ++n_fast; }
         }
         // ---- the ring slots of this sub-chunk must have been consumed ------------------------------
-        while (t0 + 32 - ld_acquire(S.flags + 1) > C::RING) __nanosleep(32);
+        for (int spins = 0; t0 + 32 - ld_acquire(S.flags + 1) > C::RING; ++spins) {
+            if (spins > SPIN_LIMIT) {      // give up: flag the error and release the consumer (it drains stale slots)
+                atomicOr(&status->ephys, 2);
+                if (lane == 0) st_release(S.flags, T);
+                return;
+            }
+            __nanosleep(32);
+        }
         if (ip >= 0) {
             double* rec = S.body + body_word<C>(slot);
             if (fast) {
@@ -961,7 +974,7 @@ __device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, co
         c0 = c1; ip0 = ip1; c1 = c2; ip1 = ip2; is1 = is2;
     }
     // ---- flags and counters ----------------------------------------------------------------------
-    if (bad_any) status->ephys = 1;
+    if (bad_any) atomicOr(&status->ephys, 1);
     n_fast = __reduce_add_sync(0xffffffffu, n_fast);
     n_slow = __reduce_add_sync(0xffffffffu, n_slow);
     n_glob = __reduce_add_sync(0xffffffffu, n_glob);
@@ -1075,7 +1088,10 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
 
 // CfgDrift: a species that has moved since its last sort (particles up to one cell outside their listed
 // cell still gather from shared memory); one block of 6 + 6 warps per SM, tile 8 x 4 x 6.
-// CfgFresh: right after pic_sort; two blocks of 3 + 3 warps per SM, tile 8 x 4 x 6.  (Measured and dropped,
+// CfgFresh: right after pic_sort; two blocks of 3 + 3 warps per SM, tile 8 x 4 x 6.  Ring depth: 29.1 ms per launch with
+// 120 slots, 30.1 with 104, 31.2 with 88 (rows of 64 +- 8 records plus the 31 a sub-chunk runs ahead stop fitting and
+// are consumed in two passes); deeper than 120 buys nothing at 8 particles per cell (a 12-double record with the old
+// shapes recomputed by the consumer and 168 slots: 29.4 ms).  (Measured and dropped,
 // profiles/r02_tile_kernel.md: one consumer for two producers -- its duty is 56 % -- at 4 + 2 warps per block runs at
 // 34.2 instead of 29.2 ms: decoupling two producers needs rings two rows deep, which shared memory does not have.)
 // *32: the mixed-precision mode (fp32 stencil, gather and push; same tiles and rings).

@@ -217,6 +217,10 @@ int poll_status(pic_ctx* c) {
     DevStatus h;
     CU(c, cudaMemcpyAsync(&h, c->status, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
+    if (h.ephys & 2) {      // the hand-over between a producer and its consumer warp timed out (particles_tile.cu)
+        c->sticky = PIC_ECUDA;
+        return fail(c, PIC_ECUDA, "internal: the fused particle kernel's producer / consumer hand-over timed out; the state is not valid");
+    }
     if (h.ephys) {
         int zero = 0;
         CU(c, cudaMemcpyAsync(&c->status->ephys, &zero, sizeof(int), cudaMemcpyHostToDevice, c->stream));
@@ -914,6 +918,7 @@ int pic_get_counters(pic_ctx* c, unsigned long long* counters) {
     counters[5] = c->sorts;
     counters[6] = c->yee_tma_ok ? (((c->yee_maps.valid & 2) && c->yee_maps.use_pipe) ? 2ull : 1ull) : 0ull;
     counters[7] = c->fallbacks;
+    counters[8] = c->deleted;
     return PIC_OK;
 }
 
