@@ -19,7 +19,9 @@
  *     F/m are compiled in; charge q [C] and mass m [kg] are per species.
  *   - Field arrays crossing this ABI are GUARD-FREE, nx*ny*nz doubles per
  *     component, index = i + nx*(j + ny*k) (x fastest).  All boundaries are
- *     periodic.  Yee staggering is implied by the component:
+ *     periodic unless options say otherwise ("open_mask": faces shared with
+ *     neighbouring bricks, NEXT-1; "absorb_mask": open ends, NEXT-2; both at
+ *     the end of this header).  Yee staggering is implied by the component:
  *       Ex,Jx (i+1/2,j,k)   Ey,Jy (i,j+1/2,k)   Ez,Jz (i,j,k+1/2)
  *       Bx (i,j+1/2,k+1/2)  By (i+1/2,j,k+1/2)  Bz (i+1/2,j+1/2,k)
  *       rho at nodes (i,j,k); node i sits at xmin + i*dx.
@@ -39,6 +41,15 @@
  *     pic_sort are asynchronous; pic_get_*, pic_deposit_rho, pic_sync and
  *     pic_get_counters synchronise that stream.
  *   - There is no CPU fallback anywhere behind this ABI.
+ *
+ * Beyond the six calls of BASELINE.json:north_star the header declares the
+ * additions SURVEY.md 8(b) proposes (arena query, field input, rho diagnostic,
+ * errors, counters, stage timers, options), the SURVEY.md 8(f) extensions --
+ * NEXT-1 bricks (pic_step_stage, pic_halo_doubles, pic_export_halo,
+ * pic_import_halo, pic_export_leavers, pic_import_arrivals), NEXT-2 open ends,
+ * moving window and plane source (pic_shift_window, pic_add_plane), NEXT-3
+ * gather / deposit variants and smoothing and the NEXT-4 mixed-precision mode
+ * (all through pic_set_option) -- and the machine-rate probes pic_probe_*.
  */
 #ifndef PIC_B200_H
 #define PIC_B200_H
