@@ -163,13 +163,14 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------- oracle legs
-def _oracle_sample(index: int):
-    """The bounded sample of configs[index] the oracle is timed on (last column)."""
+def _oracle_sample(index: int, crop: bool = True):
+    """The bounded sample of configs[index] the oracle is timed on (last column).  crop = False: the
+    size the slow parity tests run (32^3 of config 1, the crops of configs 3 and 4)."""
     from paper_2303_12873_b200 import workloads as W
     # configs 1-2: a 16^3 crop (same ppc, u_th, order, dx, dt) keeps one oracle step under a second
-    wl = W.config(index, parity=True, **({"n": 16} if index in (1, 2) else {}))
-    desc = "%s: %dx%dx%d cells, %d particles, order %d (crop of configs[%d], same ppc/u_th/order/dx/dt)" % (
-        wl.name, wl.nx, wl.ny, wl.nz, wl.nparticles, wl.order, index)
+    wl = W.config(index, parity=True, **({"n": 16} if (crop and index in (1, 2)) else {}))
+    desc = "%s: %dx%dx%d cells, %d particles, order %d (%s of configs[%d], same ppc/u_th/order/dx/dt)" % (
+        wl.name, wl.nx, wl.ny, wl.nz, wl.nparticles, wl.order, "crop" if crop else "parity size", index)
     return wl, desc
 
 
@@ -183,16 +184,18 @@ def _oracle_sim(wl):
     return o
 
 
-def time_oracle(index: int, budget_s: float = 12.0, max_steps: int = 40, core_index: int = -1):
+def time_oracle(index: int, budget_s: float = 12.0, max_steps: int = 40, core_index: int = -1, crop: bool = True,
+                min_steps: int = 2, warm: bool = True):
     """particle-updates/s of the oracle as it stands, single-threaded, pinned to one host core."""
-    wl, desc = _oracle_sample(index)
+    wl, desc = _oracle_sample(index, crop)
     o = _oracle_sim(wl)
     core, before = _pin_to_one_core(core_index)
     try:
-        o.step(1)                                   # warm-up (page in, build tables)
+        if warm:
+            o.step(1)                               # warm-up (page in, build tables)
         t0 = time.perf_counter()
         n = 0
-        while n < max_steps and (n < 2 or time.perf_counter() - t0 < budget_s):
+        while n < max_steps and (n < min_steps or time.perf_counter() - t0 < budget_s):
             o.step(1)
             n += 1
         dt = time.perf_counter() - t0
@@ -433,6 +436,15 @@ def run_ours(args):
                 cpu["config0_full_size"] = time_oracle(0, budget_s=6.0, max_steps=10)
             except Exception as exc:
                 cpu["config0_full_size"] = {"error": str(exc)}
+        # ... and the sizes the slow parity tests step configs 1, 3 and 4 at: one cold step each (a 32^3 order-3 step
+        # takes the oracle several seconds)
+        cpu["parity_sizes"] = {}
+        for k in (1, 3, 4):
+            try:
+                r = time_oracle(k, budget_s=0.0, max_steps=1, crop=False, min_steps=1, warm=False)
+                cpu["parity_sizes"]["configs[%d]" % k] = {"value": r["value"], "unit": UNIT, "sample": r["sample"]}
+            except Exception as exc:
+                cpu["parity_sizes"]["configs[%d]" % k] = {"error": str(exc)}
         try:
             cpu["all_cores"] = time_oracle_all_cores(args.config)
         except Exception as exc:      # a reported baseline, never a reason to lose the bench line

@@ -363,9 +363,17 @@ int pic_step_stage(pic_ctx*, int stage);
  * pic_add_plane: F[:, :, k] += values for one component (0..8 = Ex Ey Ez Bx By Bz
  *   Jx Jy Jz), values = nx*ny doubles, x fastest (host or device).  An antenna is
  *   pic_step_stage(0), pic_add_plane(6.., k, J_source), pic_step_stage(1..3).
+ * pic_set_damping: an absorbing layer of `ncells` planes in front of each open z
+ *   end (needs absorb_mask bit 2, else PIC_ESTATE).  factors[m] (HOST, ncells
+ *   doubles, copied) multiplies every value of B after each B half push and of E
+ *   after the E push on the plane m cells from the face (m = 0 next to it), at
+ *   both ends; the caller chooses the profile, e.g. exp(-a ((n - m)/n)^2).
+ *   ncells = 0 removes the layers.  PIC_EINVAL: ncells not in 0 .. 64, layers
+ *   that overlap (2 ncells > nz), a factor that is not finite.
  */
 int pic_shift_window(pic_ctx*, int ncells, long long* deleted /*host, may be NULL*/);
 int pic_add_plane(pic_ctx*, int component, int k, const double* values, int src_on_device);
+int pic_set_damping(pic_ctx*, int ncells, const double* factors /*host*/);
 long long pic_halo_doubles(pic_ctx*, int dim);
 int pic_export_halo(pic_ctx*, int group, int dim, int side, double* buf_dev);
 int pic_import_halo(pic_ctx*, int group, int dim, int side, const double* buf_dev);

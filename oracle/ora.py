@@ -275,6 +275,7 @@ class OracleSim:
         self.cell_offset: list[np.ndarray | None] = [None] * nspecies
         self.plane_sources = []                            # (component index 0..2 of J, plane k, values) for the next step
         self.deleted = 0
+        self.damp = None                                   # NEXT-2: damping factors of the layers next to the open ends
 
     # ---- open-z helpers ------------------------------------------------------------------------------------
     def _phys(self, a):
@@ -334,6 +335,26 @@ class OracleSim:
         (comp = 0, 1, 2 for Jx, Jy, Jz; values = ny x nx array, x fastest)."""
         self.plane_sources.append((int(comp), int(k), np.asarray(values, dtype=np.float64).reshape(self.ny, self.nx).copy()))
 
+    def set_damping(self, factors):
+        """NEXT-2: an absorbing layer in front of each open z end.  factors[m], m = 0 .. len-1, multiplies every value
+        of B (after each B half push) and of E (after the E push) on the plane m cells away from the face (m = 0: the
+        plane next to it), at both ends.  The caller supplies the profile (e.g. exp(-a ((n - m)/n)^2))."""
+        if not self.open_z:
+            raise ValueError("damping layers sit in front of open ends: needs open_z")
+        f = np.asarray(factors, dtype=np.float64).reshape(-1)
+        if 2 * f.size > self.nz_phys:
+            raise ValueError("the two layers overlap")
+        self.damp = f.copy() if f.size else None
+
+    def _apply_damping(self, arrays):
+        if self.damp is None:
+            return
+        for a in arrays:
+            v = self._phys(a)
+            for m, fm in enumerate(self.damp):
+                v[m] *= fm
+                v[self.nz_phys - 1 - m] *= fm
+
     def shift_window(self, ncells=1):
         """NEXT-2 moving window: the box moves up by ncells cells along z.  Field index k now names what was
         k + ncells, the top ncells planes are new (zero), particles below the new zmin are deleted."""
@@ -388,10 +409,13 @@ class OracleSim:
                     smooth_binomial(g, self.smooth_passes, a)
             yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 6
             self._zero_pads(self.B)
+            self._apply_damping(self.B)
             yee_push_E(g, dt, self.E, self.B, self.J)                             # step 7
             self._zero_pads(self.E)
+            self._apply_damping(self.E)
             yee_push_B(g, 0.5 * dt, self.E, self.B)                               # step 8
             self._zero_pads(self.B)
+            self._apply_damping(self.B)
 
     def sort(self):
         for s, sp in enumerate(self.species):

@@ -25,6 +25,7 @@ SYMBOLS = ("pic_query_arena", "pic_init_grid", "pic_set_fields", "pic_load_parti
            "pic_get_counters", "pic_get_stage_ms", "pic_set_option", "pic_sync", "pic_last_error",
            "pic_destroy", "pic_version", "pic_step_stage", "pic_halo_doubles", "pic_export_halo",
            "pic_import_halo", "pic_export_leavers", "pic_import_arrivals", "pic_shift_window", "pic_add_plane",
+           "pic_set_damping",
            "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
 
 
@@ -78,6 +79,7 @@ def load_library(path: str | None = None):
     L.pic_import_arrivals.argtypes = [vp, i, vp, ll, d, d, d]
     L.pic_shift_window.argtypes = [vp, i, C.POINTER(ll)]
     L.pic_add_plane.argtypes = [vp, i, i, vp, i]
+    L.pic_set_damping.argtypes = [vp, i, C.POINTER(d)]
     L.pic_probe_dfma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_dmma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
@@ -332,6 +334,12 @@ class Sim:
         dev = _on_device([values])
         self._check(self._L.pic_add_plane(self._ctx, self.FIELD_NAMES.index(name), int(k),
                                           _ptr(values, np.float64, dev), int(dev)), "pic_add_plane")
+
+    def set_damping(self, factors):
+        """Absorbing layers in front of the open z ends: factors[m] scales E and B on the plane m cells from a face."""
+        f = np.ascontiguousarray(factors, dtype=np.float64).reshape(-1)
+        self._check(self._L.pic_set_damping(self._ctx, int(f.size), f.ctypes.data_as(C.POINTER(C.c_double))),
+                    "pic_set_damping")
 
     def append_particles(self, species, x, y, z, ux, uy, uz, w, ids):
         """Appends particles given as host arrays (marshalled into the 8-double records of pic_import_arrivals)."""

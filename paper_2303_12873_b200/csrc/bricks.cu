@@ -64,6 +64,19 @@ __global__ void add_plane_kernel(Grid g, double* F, int k, const double* __restr
     if (i < g.nx) F[g.idx(i, j, k)] += values[i + (long long)g.nx * j];
 }
 
+// damping layers in front of the two open z ends: plane m cells from a face (m = 0 next to it) *= t.f[m], over the
+// whole padded x-y extent (the x / y guard cells hold periodic images of the same plane), three components at once
+__global__ void damp_z_kernel(Grid g, double* F0, double* F1, double* F2, DampTable t) {
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x), j = (int)blockIdx.y;
+    if (i >= g.px) return;
+    const int m = (int)blockIdx.z >> 1, k = (blockIdx.z & 1) ? g.nz - 1 - m : m;
+    const long long at = i + g.sy * j + g.sz * (long long)(k + NG);
+    const double fm = t.f[m];
+    F0[at] *= fm;
+    F1[at] *= fm;
+    F2[at] *= fm;
+}
+
 // ---- leavers: taken out of the container IN PLACE ------------------------------------------------------------
 // Only a sliver of a brick's particles leaves through a face in one step, so the container is not copied: pass 1
 // reads ONE coordinate of every particle, appends the index of every leaver to a list and its record to the
@@ -174,6 +187,11 @@ void launch_shift_z(const Grid& g, double* F, int ncells, cudaStream_t st) {
 void launch_add_plane(const Grid& g, double* F, int k, const double* values_dev, cudaStream_t st) {
     dim3 bs(128, 1, 1), nb((g.nx + 127) / 128, g.ny, 1);
     add_plane_kernel<<<nb, bs, 0, st>>>(g, F, k, values_dev);
+}
+
+void launch_damp_z(const Grid& g, double* F0, double* F1, double* F2, const DampTable& t, cudaStream_t st) {
+    dim3 bs(128, 1, 1), nb((g.px + 127) / 128, g.py, 2 * t.n);
+    damp_z_kernel<<<nb, bs, 0, st>>>(g, F0, F1, F2, t);
 }
 
 void launch_find_leavers(const Grid& g, const Particles& p, long long n, int dim, int side, double* out,

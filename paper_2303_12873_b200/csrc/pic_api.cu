@@ -2,6 +2,7 @@
 // arena carving, call-order state machine, copies across the boundary, and
 // the per-step launch sequence of SURVEY 8(c.1) steps 1-8.
 #include <math.h>
+#include <cmath>
 #include <stdarg.h>
 
 #include <algorithm>
@@ -74,6 +75,7 @@ struct pic_ctx {
     int gather_variant = 0, smooth_passes = 0, deposit_variant = 0;      // NEXT-3 options
     int precision = 0;                              // NEXT-4: 1 = gather and Boris push in fp32
     unsigned long long id_base = 0;                 // ids given at load start here (bricks: unique across contexts)
+    DampTable damp;                                 // NEXT-2: damping layers in front of the open z ends (pic_set_damping)
     int absorb_mask = 0;                            // NEXT-2: dimensions whose faces are open ends (zero exterior, particles deleted)
     unsigned long long deleted = 0;                 // particles deleted at absorbing faces / by the moving window
     YeeMaps yee_maps{};
@@ -468,6 +470,14 @@ static void zero_absorbing_guards(pic_ctx* c, int group) {
             }
 }
 
+// damping layers of E (group 0) or B (group 1) after their push
+static void damp_layers(pic_ctx* c, int group) {
+    if (c->damp.n == 0) return;
+    if (group == 0) launch_damp_z(c->g, c->f.Ex, c->f.Ey, c->f.Ez, c->damp, c->stream);
+    else launch_damp_z(c->g, c->f.Bx, c->f.By, c->f.Bz, c->damp, c->stream);
+    c->launches += 1;
+}
+
 // Particles of one species beyond face (dim, side) are taken out of the container in place (bricks.cu); their records go
 // to out (device, 8 doubles each) if given.  More than `capacity` leavers: PIC_ENOMEM, container unchanged.
 // Synchronises once (the count).
@@ -626,18 +636,21 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
             launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
             c->launches += 1;
             if (c->absorb_mask) zero_absorbing_guards(c, 1);
+            damp_layers(c, 1);
         }
         if (timing) cudaEventRecord(ev[4], c->stream);
         if (mask & 4) {
             launch_push_E(g, c->f, g.dt, tma_E, c->stream);
             c->launches += 1;
             if (c->absorb_mask) zero_absorbing_guards(c, 0);
+            damp_layers(c, 0);
         }
         if (timing) cudaEventRecord(ev[5], c->stream);
         if (mask & 8) {
             launch_push_B(g, c->f, 0.5 * g.dt, tma_B, c->stream);
             c->launches += 1;
             if (c->absorb_mask) zero_absorbing_guards(c, 1);
+            damp_layers(c, 1);
             c->steps += 1;
         }
         nvtxRangePop();
@@ -776,6 +789,20 @@ int pic_shift_window(pic_ctx* c, int ncells, long long* deleted) {
     }
     if (deleted) *deleted = total;
     CU(c, cudaGetLastError());
+    return PIC_OK;
+}
+
+int pic_set_damping(pic_ctx* c, int ncells, const double* factors) {
+    ENTER(c);
+    if (ncells < 0 || ncells > DAMP_MAX || (ncells > 0 && !factors))
+        return fail(c, PIC_EINVAL, "damping layer of 0 .. %d cells, factors given", DAMP_MAX);
+    if (ncells > 0 && !(c->absorb_mask & 4))
+        return fail(c, PIC_ESTATE, "damping layers sit in front of open z ends (absorb_mask bit 2)");
+    if (2 * ncells > c->g.nz) return fail(c, PIC_EINVAL, "the two layers overlap (nz = %d)", c->g.nz);
+    for (int m = 0; m < ncells; ++m)
+        if (!std::isfinite(factors[m])) return fail(c, PIC_EINVAL, "factor %d is not finite", m);
+    c->damp.n = ncells;
+    for (int m = 0; m < ncells; ++m) c->damp.f[m] = factors[m];
     return PIC_OK;
 }
 
@@ -976,6 +1003,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
             if (((value >> d) & 1) && n[d] < NG) return fail(c, PIC_EINVAL, "an open end needs at least %d cells along its dimension", NG);
         c->g.open_mask = (c->g.open_mask & ~c->absorb_mask) | (int)value;
         c->absorb_mask = (int)value;
+        if (!(value & 4)) c->damp.n = 0;            // the layers go with the open z ends
         zero_absorbing_guards(c, 0);
         zero_absorbing_guards(c, 1);
     } else if (!strcmp(name, "id_base")) {

@@ -94,6 +94,12 @@ void launch_halo_unpack(const Grid& g, double* F, int dim, int first_layer, cons
 void launch_halo_fill(const Grid& g, double* F, int dim, int first_layer, double value, cudaStream_t st);
 void launch_shift_z(const Grid& g, double* F, int ncells, cudaStream_t st);          // moving window (NEXT-2)
 void launch_add_plane(const Grid& g, double* F, int k, const double* values_dev, cudaStream_t st);
+constexpr int DAMP_MAX = 64;                       // thickest damping layer (cells); the table travels as a kernel argument
+struct DampTable {
+    int n = 0;
+    double f[DAMP_MAX];
+};
+void launch_damp_z(const Grid& g, double* F0, double* F1, double* F2, const DampTable& t, cudaStream_t st);
 // Leavers of face (dim, side), in place: find_leavers appends their indices to leaver_idx (and their 8-double records
 // x y z ux uy uz w id to out, if given) and counts them in counters[0] (device, zeroed by the caller; entries beyond
 // `capacity` are counted but not stored); close_holes then moves the stayers among the last L places into the holes

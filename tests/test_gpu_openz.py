@@ -169,3 +169,71 @@ def test_open_end_calls_reject_bad_arguments(Sim):
     with pytest.raises(PicError):
         g2.set_option("absorb_mask", 4)            # fewer than NG cells along z
     g2.close()
+
+
+def test_damping_layers_match_the_oracle_and_absorb(ora, Sim):
+    """pic_set_damping against OracleSim.set_damping: random fields and hot plasma for 10 steps (1-step and 10-step
+    tolerances), then a vacuum pulse sent into the upper layer: what comes back is the oracle's small remainder, not the
+    full reflection of the bare open end.  Validation of the arguments too."""
+    from paper_2303_12873_b200.binding import PicError
+    wl = W.uniform_plasma(9, 7, 40, ppc=3, u_th=0.2, order=2, seed=731, dz=0.3e-6)
+    wl.fields = _rand_fields(wl.ncell, 73)
+    nd = 9
+    prof = np.exp(-0.35 * ((nd - np.arange(nd)) / nd) ** 2)
+    o = ora.OracleSim(*wl.grid_args(), wl.dt, wl.order, 1, open_z=True)
+    g = Sim.from_workload(wl)
+    with pytest.raises(PicError):
+        g.set_damping(prof)                        # no open ends yet
+    g.set_option("absorb_mask", 4)
+    with pytest.raises(PicError):
+        g.set_damping(np.ones(21))                 # 2 x 21 > nz
+    with pytest.raises(PicError):
+        g.set_damping(np.array([1.0, np.nan]))
+    g.set_damping(prof)
+    o.set_damping(prof)
+    g.set_fields(**wl.fields); o.set_fields(**wl.fields)
+    sp = wl.species[0]
+    o.load_particles(0, sp.q, sp.m, *sp.arrays())
+    g.sort()
+    o.step(1); g.step(1)
+    for grp, e in group_maxabs_errors(o.get_fields(), g.get_fields()).items():
+        assert e <= TOL_FIELD_1STEP, (grp, e)
+    o.step(9); g.step(9)
+    assert field_l2_error(o.get_fields(), g.get_fields()) <= TOL_FIELD_L2_10STEP
+    g.close()
+
+    # vacuum pulse into the layer (no particles that matter: one cold particle at rest, weight 0)
+    nx, ny, nz = 4, 4, 96
+    wl = W.uniform_plasma(nx, ny, nz, ppc=1, u_th=0.0, order=1, seed=5, dx=1e-6, dy=1e-6, dz=0.25e-6)
+    wl.species[0].w[:] = 0.0
+    k, _, _ = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    env = np.exp(-((k - 40.0) / 6.0) ** 2) * np.cos(2 * np.pi * (k - 40.0) / 12.0)
+    envb = np.exp(-((k + 0.5 - 40.0) / 6.0) ** 2) * np.cos(2 * np.pi * (k + 0.5 - 40.0) / 12.0)
+    zero = np.zeros(wl.ncell)
+    f = {n: zero for n in ("Ex", "Ey", "Ez", "Bx", "By", "Bz")}
+    f["Ex"] = (1e9 * env).reshape(-1); f["By"] = (1e9 / C_LIGHT * envb).reshape(-1)
+    nd = 12
+    prof = np.exp(-0.35 * ((nd - np.arange(nd)) / nd) ** 2)
+    nsteps = int(2 * (nz - 40) * 0.25e-6 / (C_LIGHT * wl.dt)) + 10
+    back = {}
+    for name in ("bare", "layer"):
+        g = Sim.from_workload(wl)
+        g.set_option("absorb_mask", 4)
+        g.set_fields(**f)
+        if name == "layer":
+            g.set_damping(prof)
+        g.step(nsteps)
+        out = g.get_fields()
+        back[name] = sum(np.sum(out[n].reshape(nz, ny, nx)[:nz - nd - 4] ** 2) for n in ("Ex", "Ey", "Ez")) / np.sum(f["Ex"] ** 2)
+        if name == "layer":
+            o = ora.OracleSim(*wl.grid_args(), wl.dt, 1, 1, open_z=True)
+            o.set_fields(**f); o.set_damping(prof)
+            sp = wl.species[0]
+            o.load_particles(0, sp.q, sp.m, *sp.arrays())
+            o.step(nsteps)
+            fo = o.get_fields()
+            ref = max(np.abs(f["Ex"]).max(), 1.0)
+            assert np.abs(fo["Ex"] - out["Ex"]).max() <= 1e-9 * ref
+        g.set_damping([])                           # and the layers can be removed again
+        g.close()
+    assert back["bare"] > 0.4 and back["layer"] < 0.02 * back["bare"], back

@@ -191,3 +191,56 @@ def test_only_charge_that_leaves_goes_missing(ora, order):
     assert sim.get_particles(0)["x"].size == 0 and sim.deleted == n
     sim.step(1)
     assert not any(sim.get_fields()[c].any() for c in ("Jx", "Jy", "Jz"))
+
+
+def test_damping_layer_absorbs_what_the_bare_open_end_reflects(ora):
+    """A plane pulse sent at the upper end: the bare open end (zero exterior) reflects all of its energy, a 12-cell
+    damping layer with a smooth profile sends back less than 2 %; factors of 1 change nothing; one step multiplies the
+    layer's planes by exactly the given factors."""
+    nx, ny, nz = 4, 4, 96
+    dz = 0.25e-6
+    k, _, _ = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    env = np.exp(-((k - 40.0) / 6.0) ** 2) * np.cos(2 * np.pi * (k - 40.0) / 12.0)
+    envb = np.exp(-((k + 0.5 - 40.0) / 6.0) ** 2) * np.cos(2 * np.pi * (k + 0.5 - 40.0) / 12.0)
+    fields = {"Ex": (1e9 * env).reshape(-1), "By": (1e9 / C_LIGHT * envb).reshape(-1)}      # travels towards +z
+
+    def energy(sim, lo, hi):
+        f = sim.get_fields()
+        e = sum(np.sum(f[n].reshape(nz, ny, nx)[lo:hi] ** 2) for n in ("Ex", "Ey", "Ez"))
+        b = sum(np.sum(f[n].reshape(nz, ny, nx)[lo:hi] ** 2) for n in ("Bx", "By", "Bz"))
+        return EPS0 * (e + C_LIGHT ** 2 * b)
+
+    nd = 12
+    prof = np.exp(-0.35 * ((nd - np.arange(nd)) / nd) ** 2)
+    back = {}
+    for name, factors in (("bare", None), ("ones", np.ones(nd)), ("layer", prof)):
+        sim, dt = _sim(ora, nz, True, nx=nx, ny=ny)
+        sim.set_fields(**fields)
+        if factors is not None:
+            sim.set_damping(factors)
+        e0 = energy(sim, 0, nz)
+        nsteps = int(2 * (nz - 40) * dz / (C_LIGHT * dt)) + 10          # to the end and back to the middle
+        sim.step(nsteps)
+        back[name] = energy(sim, 0, nz - nd - 4) / e0
+    assert back["bare"] > 0.9 and abs(back["bare"] - back["ones"]) < 1e-12
+    assert back["layer"] < 0.02, back
+    # where it acts: factors of zero leave exactly zero on the layer's planes at both ends, and one step changes nothing
+    # further than its stencils reach (3 pushes, one plane each)
+    rng = np.random.default_rng(6)
+    f = {n: rng.standard_normal(nx * ny * nz) * (1e9 if n[0] == "E" else 3.0) for n in ("Ex", "Ey", "Ez", "Bx", "By", "Bz")}
+    a, _ = _sim(ora, nz, True, nx=nx, ny=ny)
+    b, _ = _sim(ora, nz, True, nx=nx, ny=ny)
+    a.set_fields(**f)
+    b.set_fields(**f)
+    b.set_damping(np.zeros(2))
+    a.step(1)
+    b.step(1)
+    fa, fb = a.get_fields(), b.get_fields()
+    for n in ("Ex", "Ey", "Ez", "Bx", "By", "Bz"):
+        va, vb = fa[n].reshape(nz, ny, nx), fb[n].reshape(nz, ny, nx)
+        assert np.array_equal(va[5:nz - 5], vb[5:nz - 5]), n
+        assert not vb[:2].any() and not vb[nz - 2:].any(), n
+        assert va[:2].any(), n
+    assert any(not np.array_equal(fa[n].reshape(nz, ny, nx)[2:5], fb[n].reshape(nz, ny, nx)[2:5]) for n in ("Ex", "Ey", "Bx", "By"))
+    with pytest.raises(ValueError):
+        b.set_damping(np.ones(nz))
