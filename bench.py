@@ -280,6 +280,8 @@ def run_ours(args):
     kw = {}
     if args.n is not None:
         kw["n"] = args.n
+    if args.ppc is not None:
+        kw["ppc"] = args.ppc
     wl = W.config(args.config, parity=False, **kw)
     wl = R.make_replica(wl, rank)   # replicas differ only by a cyclic shift of the particle momenta
     sort_every = wl.sort_every if wl.sort_every > 0 else 0
@@ -345,7 +347,7 @@ def run_ours(args):
     fp64_per_particle = FP64_INSTR_PER_PARTICLE.get(wl.order, FP64_INSTR_PER_PARTICLE[3])
     fp64_alg = fp64_per_particle * np_launch
     fp64_ach = fp64_alg / (ms_launch * 1e-3) / 1e12
-    full_size = args.n is None
+    full_size = args.n is None and args.ppc is None
     mc = _measured_counters("configs[%d]" % args.config) if full_size else None
     roofline = {"bound": "alu", "kernel": kname, "achieved": fp64_ach, "peak": fp64_peak,
                 "peak_kind": "derived: 148 SMs x 64 fp64 lanes/clk x 1965 MHz (DESIGN.md 5.1; DFMA probe: 62.5 lanes/clk/SM)",
@@ -460,6 +462,7 @@ def run_ours(args):
             "config": {"workload": "configs[%d]" % args.config, "name": wl.name,
                        "grid": [wl.nx, wl.ny, wl.nz], "particles": npart, "species": len(wl.species),
                        "order": wl.order, "sort_every": sort_every, "replicas": world, "options": options,
+                       **({"ppc_override": args.ppc} if args.ppc is not None else {}),
                        "l2": "inputs larger than L2 (%.1f GB of particles + fields per step)" % (
                            (BYTES_PER_PARTICLE * npart + 9 * 8 * ncell) / 1e9),
                        "generation_s": round(t_gen, 1)},
@@ -523,6 +526,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: 256^3 x 8 ppc)")
     ap.add_argument("--n", "--cube", dest="n", type=int, default=None,
                     help="override the cube edge of configs 0-2 (debugging; under torchrun use --cube: --n is ambiguous there)")
+    ap.add_argument("--ppc", type=int, default=None,
+                    help="particles per cell of configs 0-2 (default: the 8 the configs name; experiments only)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--sort-every", type=int, default=None, help="override the workload's sort cadence (steps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -233,18 +233,19 @@ def config(index: int, parity: bool = False, **kw) -> Workload:
     """BASELINE.json configs[index] at full size, or (parity=True) at the size
     the oracle finishes in seconds (last column)."""
     seed = SEED0 + index
+    ppc = kw.pop("ppc", 8) if index <= 2 else None      # configs 0-2 name 8 particles per cell; experiments may override
     if index == 0:
         n = kw.pop("n", 32)
-        return uniform_plasma(n, n, n, 8, 0.01, 1, seed, nsteps=10, sort_every=0, name="config0", **kw)
+        return uniform_plasma(n, n, n, ppc, 0.01, 1, seed, nsteps=10, sort_every=0, name="config0", **kw)
     if index == 1:
         n = kw.pop("n", 32 if parity else 128)
-        return uniform_plasma(n, n, n, 8, 0.01, 3, seed, nsteps=100, sort_every=4, protons=True,
+        return uniform_plasma(n, n, n, ppc, 0.01, 3, seed, nsteps=100, sort_every=4, protons=True,
                               name="config1", **kw)
     if index == 2:
         n = kw.pop("n", 32 if parity else 256)
         # the config names no sort cadence; at u_th = 0.05 c about 7 % of the particles change cell per
         # step, so sorting every step keeps the fused kernel's per-cell fast path at ~93 % (R25)
-        return uniform_plasma(n, n, n, 8, 0.05, 3, seed, nsteps=10 if parity else 50, sort_every=1,
+        return uniform_plasma(n, n, n, ppc, 0.05, 3, seed, nsteps=10 if parity else 50, sort_every=1,
                               name="config2", **kw)
     if index == 3:
         if parity:
