@@ -27,6 +27,9 @@ SYMBOLS = ("pic_query_arena", "pic_init_grid", "pic_set_fields", "pic_load_parti
            "pic_import_halo", "pic_export_leavers", "pic_import_arrivals", "pic_shift_window", "pic_add_plane",
            "pic_set_damping",
            "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
+# include/pic_noalloc.h
+NOALLOC_SYMBOLS = ("pic_cell_offsets_noalloc", "pic_noalloc_last_error")
+NOALLOC_MAX_CELLS = 2048 * 16384 - 1
 
 
 class PicError(RuntimeError):
@@ -84,6 +87,10 @@ def load_library(path: str | None = None):
     L.pic_probe_dmma.argtypes = [i, i, C.POINTER(d)]
     L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
     L.pic_probe_red.argtypes = [i, ll, ll, i, C.POINTER(d)]
+    L.pic_cell_offsets_noalloc.argtypes = [i, i, i, d, d, d, d, d, d, ll, vp, vp, vp, vp, vp]
+    L.pic_cell_offsets_noalloc.restype = i
+    L.pic_noalloc_last_error.argtypes = []
+    L.pic_noalloc_last_error.restype = C.c_char_p
     for name in SYMBOLS:
         if name not in ("pic_version", "pic_last_error"):
             getattr(L, name).restype = i
@@ -100,6 +107,31 @@ def query_arena(nx, ny, nz, order, np_max) -> int:
     if rc != PIC_OK:
         raise PicError(rc, "pic_query_arena")
     return int(out.value)
+
+
+def cell_offsets_noalloc(nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, x, y, z, offsets, stream=None):
+    """pic_cell_offsets_noalloc (include/pic_noalloc.h): for callers that may not allocate device memory (a
+    hook inside another code's loop whose pool owns the GPU, a latency-critical step, an out-of-memory
+    path), the counting sort's cell-offset table from caller buffers only.  x, y, z: torch.cuda float64
+    tensors of n entries; offsets: a torch.cuda int32/uint32 tensor of nx*ny*nz + 1 entries that the caller
+    owns and this call overwrites.  Queued on `stream` (default: torch's current stream of that device);
+    the library's 64 KiB built-in scratch is shared, so do not overlap two calls on one GPU."""
+    import torch
+    L = load_library()
+    n = int(x.numel())
+    for a in (x, y, z):
+        assert a.is_cuda and a.is_contiguous() and a.dtype == torch.float64 and a.numel() == n
+    assert offsets.is_cuda and offsets.is_contiguous() and offsets.element_size() == 4
+    assert offsets.numel() >= nx * ny * nz + 1
+    with torch.cuda.device(offsets.device):
+        st = stream if stream is not None else torch.cuda.current_stream(offsets.device)
+        rc = L.pic_cell_offsets_noalloc(nx, ny, nz, dx, dy, dz, xmin, ymin, zmin, n,
+                                        C.c_void_p(x.data_ptr()) if n else None,
+                                        C.c_void_p(y.data_ptr()) if n else None,
+                                        C.c_void_p(z.data_ptr()) if n else None,
+                                        C.c_void_p(offsets.data_ptr()), C.c_void_p(st.cuda_stream))
+    if rc != PIC_OK:
+        raise PicError(rc, "pic_cell_offsets_noalloc", (L.pic_noalloc_last_error() or b"").decode())
 
 
 def _is_torch(a) -> bool:

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpic_b200.so")
-SOURCES = ["pic_api.cu", "yee.cu", "particles_global.cu", "particles_tile.cu", "sort.cu", "peaks.cu", "bricks.cu"]
+SOURCES = ["pic_api.cu", "yee.cu", "particles_global.cu", "particles_tile.cu", "sort.cu", "peaks.cu", "bricks.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 
