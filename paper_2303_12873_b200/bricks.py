@@ -126,19 +126,26 @@ class DistTransport:
         self.host = bool(stage_through_host)
 
     @staticmethod
-    def _tag(key):
+    def _face_order(key):
         dim, side = key
         return 2 * dim + side
 
     def exchange(self, sends, recv_like=None):
         """sends: [(src == my rank, dst, key, tensor)]; recv_like: {(src, key): empty tensor to receive into} for the
-        messages this rank expects, keyed by the face they arrive at.  Returns {(my rank, key): tensor}."""
-        ops, out, landed = [], {}, []
+        messages this rank expects, keyed by the face they arrive at.  Returns {(my rank, key): tensor}.
+
+        Messages are matched by ORDER, never by tag: the NCCL backend ignores P2P tags and pairs the sends and
+        receives between two ranks in the order they were issued.  With two bricks along a dimension both faces of a
+        brick talk to the same peer, so both sides must agree on the order without talking: every message is named by
+        the face (dim, side) it ARRIVES at -- the sender's `key` and the receiver's `key` are that same face -- and both
+        the sends to a peer and the receives from it are issued in increasing (peer, 2 dim + side).  All tags are 0,
+        so the gloo test exercises exactly the matching NCCL does."""
+        recvs, out, landed, posts = [], {}, [], []
         for (src, key), buf in (recv_like or {}).items():
             if src == self.rank:
                 continue
             tmp = self.torch.empty(buf.shape, dtype=buf.dtype) if (self.host and buf.is_cuda) else buf
-            ops.append(self.dist.P2POp(self.dist.irecv, tmp, src, tag=self._tag(key)))
+            recvs.append((src, self._face_order(key), tmp))
             if tmp is not buf:
                 landed.append((tmp, buf))
             out[(self.rank, key)] = buf
@@ -150,7 +157,11 @@ class DistTransport:
             t = t.contiguous()
             if self.host and t.is_cuda:
                 t = t.cpu()
-            ops.append(self.dist.P2POp(self.dist.isend, t, dst, tag=self._tag(key)))
+            posts.append((dst, self._face_order(key), t))
+        recvs.sort(key=lambda m: m[:2])
+        posts.sort(key=lambda m: m[:2])
+        ops = [self.dist.P2POp(self.dist.irecv, t, src, tag=0) for (src, _, t) in recvs]
+        ops += [self.dist.P2POp(self.dist.isend, t, dst, tag=0) for (dst, _, t) in posts]
         if ops:
             for r in self.dist.batch_isend_irecv(ops):
                 r.wait()

@@ -54,6 +54,53 @@ def test_local_transport_hands_buffers_over():
     assert t.exchange_counts([(0, 1, (2, 1), 7)]) == {(1, (2, 1)): 7}
 
 
+class _FakeDist:
+    """Records the order in which DistTransport issues its point-to-point operations."""
+    isend, irecv = "isend", "irecv"
+
+    class P2POp:
+        def __init__(self, op, tensor, peer, tag=0):
+            self.op, self.tensor, self.peer, self.tag = op, tensor, peer, tag
+
+    def __init__(self):
+        self.issued = []
+
+    def get_backend(self):
+        return "nccl"
+
+    def batch_isend_irecv(self, ops):
+        self.issued = list(ops)
+        return []
+
+
+def test_dist_transport_orders_messages_by_arrival_face_not_by_tag():
+    """The NCCL backend ignores tags and pairs the messages between two ranks in issue order.  With two
+    bricks along a dimension both faces talk to the same peer: the k-th send of rank 0 to rank 1 must be the k-th
+    receive rank 1 posts from rank 0, whatever order the schedule listed them in, and no tag may be relied on."""
+    import torch
+    lay = B.BrickLayout(16, 8, 8, 1.0, 1.0, 1.0, 0.0, 0.0, 0.0, (2, 2, 1))
+    # ranks 0 and 1 are each other's neighbour through BOTH x faces; 0's y neighbour (both faces) is rank 2
+    plans = {}
+    for rank in (0, 1):
+        fd = _FakeDist()
+        tr = B.DistTransport(fd, rank, "cpu")
+        sends, expect = [], {}
+        for d in ((1, 0) if rank == 0 else (0, 1)):          # the two ranks walk dimensions and faces in different orders
+            for side in ((0, 1) if rank == 0 else (1, 0)):
+                nb = lay.neighbour(rank, d, side)
+                arrives_at = (d, 1 - side)                     # face of the neighbour this message lands on
+                # every tensor carries the name of the face it arrives at, as a number
+                sends.append((rank, nb, arrives_at, torch.full((1,), 10.0 * d + (1 - side), dtype=torch.float64)))
+                expect[(nb, (d, side))] = torch.full((1,), 10.0 * d + side, dtype=torch.float64)
+        tr.exchange(sends, expect)
+        assert all(op.tag == 0 for op in fd.issued)
+        plans[rank] = fd.issued
+    for a, b in ((0, 1), (1, 0)):
+        sent = [float(op.tensor[0]) for op in plans[a] if op.op == "isend" and op.peer == b]
+        posted = [float(op.tensor[0]) for op in plans[b] if op.op == "irecv" and op.peer == a]
+        assert len(sent) == 2 and sent == posted, (a, b, sent, posted)   # k-th send meets the k-th receive: same face
+
+
 _WORKER = textwrap.dedent("""
     import os, sys
     sys.path.insert(0, %r)
