@@ -302,12 +302,16 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    (NEXT-2): every field value beyond them is zero at all times,
  *                    current deposited beyond them is dropped, and a particle that
  *                    leaves through them is deleted at the end of the particle
- *                    stage (which then synchronises).  Implies the same bits of
- *                    "open_mask"; pic_step stays available when every open
- *                    dimension is absorbing.  Oracle: OracleSim(open_z=True).
+ *                    stage (which then synchronises; any number of them: the
+ *                    deletion works in batches of np_max / 3).  Implies the same
+ *                    bits of "open_mask", in whichever order the two options are
+ *                    set (a later "open_mask" keeps them); pic_step stays
+ *                    available when every open dimension is absorbing.  Oracle:
+ *                    OracleSim(open_z=True).
  *   "id_base"        ids given by the next pic_load_particles start at this
  *                    value (default 0), so that bricks can hand out disjoint ids.
- * Unknown name: PIC_EINVAL.
+ * Unknown name: PIC_EINVAL.  Like every call that takes a context it makes the
+ * context's device current and returns the sticky error, if one is pending.
  */
 int pic_set_option(pic_ctx*, const char* name, long long value);
 
@@ -357,8 +361,9 @@ int pic_step_stage(pic_ctx*, int stage);
  * pic_shift_window: the box moves up by `ncells` cells along z (needs
  *   "absorb_mask" bit 2): field index k now names what was k + ncells, the top
  *   ncells planes are new and zero, zmin grows by ncells*dz, particles below the
- *   new zmin are deleted (*deleted = how many, may be NULL), every species counts
- *   as unsorted.  Fresh plasma for the new planes is the caller's to append with
+ *   new zmin are deleted (*deleted = how many, may be NULL; no limit on the
+ *   number -- unlike pic_export_leavers the deletion works in batches of
+ *   np_max / 3), every species counts as unsorted.  Fresh plasma for the new planes is the caller's to append with
  *   pic_import_arrivals.  Synchronises.
  * pic_add_plane: F[:, :, k] += values for one component (0..8 = Ex Ey Ez Bx By Bz
  *   Jx Jy Jz), values = nx*ny doubles, x fastest (host or device).  An antenna is

@@ -86,6 +86,7 @@ struct pic_ctx {
     DevStatus* watch = nullptr;         // [MAX_SPECIES + 1]
     cudaEvent_t watch_ev = nullptr;
     bool watch_armed = false;
+    unsigned long long watch_sorts = 0;    // c->sorts when the snapshot was armed: a pic_sort since then voids it
     bool watch_tile[MAX_SPECIES] = {false};
     int drift_watch = 1;
     unsigned long long fallbacks = 0;   // particle launches that took the global kernel because of the watch
@@ -267,6 +268,7 @@ void poll_watch(pic_ctx* c) {
         return;
     }
     c->watch_armed = false;
+    if (c->watch_sorts != c->sorts) return;    // taken before the last pic_sort: says nothing about the new order
     for (int s = 0; s < c->nspecies; ++s) {
         Species& S = c->sp[s];
         if (!c->watch_tile[s] || S.n == 0 || S.steps_since_sort == 0) continue;   // sorted since: nothing to conclude
@@ -479,10 +481,13 @@ static void damp_layers(pic_ctx* c, int group) {
 }
 
 // Particles of one species beyond face (dim, side) are taken out of the container in place (bricks.cu); their records go
-// to out (device, 8 doubles each) if given.  More than `capacity` leavers: PIC_ENOMEM, container unchanged.
-// Synchronises once (the count).
-static int take_leavers(pic_ctx* c, Species& S, int dim, int side, double* out, long long capacity, long long* count) {
+// to out (device, 8 doubles each) if given.  More than `capacity` leavers: PIC_ENOMEM, container unchanged -- unless
+// `remaining` is given: then the first `capacity` of them (in list order) are taken out and *remaining = how many are
+// still in the container (discard_leavers comes back for them).  Synchronises once (the count).
+static int take_leavers(pic_ctx* c, Species& S, int dim, int side, double* out, long long capacity, long long* count,
+                        long long* remaining = nullptr) {
     *count = 0;
+    if (remaining) *remaining = 0;
     if (!S.loaded || S.n == 0) return PIC_OK;
     materialize(c, S);
     // scratch: the sort's rank array holds the leaver list, the tail flags and the filler list (a third each)
@@ -497,8 +502,12 @@ static int take_leavers(pic_ctx* c, Species& S, int dim, int side, double* out, 
     unsigned long long L = 0;
     CU(c, cudaMemcpyAsync(&L, counters, sizeof(L), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
-    if ((long long)L > cap)
-        return fail(c, PIC_ENOMEM, "%llu particles leave through this face, room for %lld (buffer, or np_max / 3)", L, cap);
+    if ((long long)L > cap) {
+        if (!remaining || cap == 0)
+            return fail(c, PIC_ENOMEM, "%llu particles leave through this face, room for %lld (buffer, or np_max / 3)", L, cap);
+        *remaining = (long long)L - cap;     // entries 0 .. cap-1 of the list are complete: take those out now
+        L = (unsigned long long)cap;
+    }
     *count = (long long)L;
     if (L > 0) {
         c->launches += launch_close_holes(S.buf[S.cur], S.n, (long long)L, leaver_idx, tailflag, fillers, counters, c->stream);
@@ -511,10 +520,19 @@ static int take_leavers(pic_ctx* c, Species& S, int dim, int side, double* out, 
     return PIC_OK;
 }
 
+// Deletes every particle beyond face (dim, side), in batches of np_max / 3 (the size of the index scratch), so that
+// a caller of pic_shift_window or of a step with absorbing faces never meets that limit half way through.
 static int discard_leavers(pic_ctx* c, Species& S, int dim, int side, long long* count) {
-    int rc = take_leavers(c, S, dim, side, nullptr, S.np_max / 3, count);
-    if (rc == PIC_OK) c->deleted += (unsigned long long)*count;
-    return rc;
+    *count = 0;
+    long long left = 0;
+    do {
+        long long got = 0;
+        int rc = take_leavers(c, S, dim, side, nullptr, S.np_max / 3, &got, &left);
+        if (rc != PIC_OK) return rc;
+        *count += got;
+        c->deleted += (unsigned long long)got;
+    } while (left > 0);
+    return PIC_OK;
 }
 
 static int discard_at_absorbing_faces(pic_ctx* c) {
@@ -612,6 +630,7 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
         if (watch) {
             CU(c, cudaEventRecord(c->watch_ev, c->stream));
             c->watch_armed = true;
+            c->watch_sorts = c->sorts;
         }
         nvtxRangePop();
         if (timing) cudaEventRecord(ev[2], c->stream);
@@ -950,7 +969,8 @@ int pic_get_counters(pic_ctx* c, unsigned long long* counters) {
 }
 
 int pic_get_stage_ms(pic_ctx* c, float* ms) {
-    if (!c || !ms) return PIC_EINVAL;
+    ENTER(c);
+    if (!ms) return PIC_EINVAL;
     if (!c->stage_timing) return fail(c, PIC_ESTATE, "stage timing is off");
     CU(c, cudaStreamSynchronize(c->stream));
     for (int k = 0; k < NSTAGE; ++k) ms[k] = 0.f;
@@ -977,7 +997,8 @@ int pic_get_stage_ms(pic_ctx* c, float* ms) {
 }
 
 int pic_set_option(pic_ctx* c, const char* name, long long value) {
-    if (!c || !name) return PIC_EINVAL;
+    ENTER(c);
+    if (!name) return PIC_EINVAL;
     if (!strcmp(name, "stage_timing")) {
         if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail(c, PIC_ECUDA, "cudaStreamSynchronize");
         c->stage_timing = value != 0;
@@ -995,7 +1016,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     else if (!strcmp(name, "drift_watch")) c->drift_watch = value != 0;
     else if (!strcmp(name, "open_mask")) {
         if (value < 0 || value > 7) return fail(c, PIC_EINVAL, "open_mask must be 0 .. 7");
-        c->g.open_mask = (int)value;
+        c->g.open_mask = (int)value | c->absorb_mask;     // an absorbing face stays open whatever the brick layout says
     } else if (!strcmp(name, "absorb_mask")) {
         if (value < 0 || value > 7) return fail(c, PIC_EINVAL, "absorb_mask must be 0 .. 7");
         const int n[3] = {c->g.nx, c->g.ny, c->g.nz};
@@ -1006,6 +1027,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
         if (!(value & 4)) c->damp.n = 0;            // the layers go with the open z ends
         zero_absorbing_guards(c, 0);
         zero_absorbing_guards(c, 1);
+        CU(c, cudaGetLastError());
     } else if (!strcmp(name, "id_base")) {
         if (value < 0) return fail(c, PIC_EINVAL, "id_base must be >= 0");
         c->id_base = (unsigned long long)value;
@@ -1028,7 +1050,7 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
 }
 
 int pic_sync(pic_ctx* c) {
-    if (!c) return PIC_EINVAL;
+    ENTER(c);
     return sync_and_check(c);
 }
 

@@ -237,3 +237,51 @@ def test_damping_layers_match_the_oracle_and_absorb(ora, Sim):
         g.set_damping([])                           # and the layers can be removed again
         g.close()
     assert back["bare"] > 0.4 and back["layer"] < 0.02 * back["bare"], back
+
+
+def test_window_shift_deletes_more_than_a_third_of_the_container(Sim):
+    """The index scratch behind the deletion holds np_max / 3 entries; a shift that drops more than that used to
+    fail with PIC_ENOMEM after the fields and the box had already moved.  It now deletes in batches."""
+    nx, ny, nz, d = 8, 8, 16, 0.5e-6
+    rng = np.random.default_rng(77)
+    n = 3001
+    x, y, z = rng.random(n) * nx * d, rng.random(n) * ny * d, rng.random(n) * nz * d
+    zero = np.zeros(n)
+    g = Sim(nx, ny, nz, d, d, d, 0.0, 0.0, 0.0, W.courant_dt(d, d, d), 1, [n])      # np_max = n: batches of 1,000
+    g.set_option("absorb_mask", 4)
+    g.load_particles(0, -W.Q_E, W.M_E, x, y, z, zero, zero, zero, np.ones(n))
+    survivors = np.nonzero(z >= 0.0 + 11 * d)[0]
+    assert n - survivors.size > 2 * (n // 3)                        # needs three batches
+    assert g.shift_window(11) == n - survivors.size
+    p = g.get_particles(0)
+    assert np.array_equal(np.sort(p["id"]), survivors.astype(np.uint64))
+    order = np.argsort(p["id"])
+    assert np.array_equal(p["z"][order], z[survivors]) and np.array_equal(p["x"][order], x[survivors])
+    assert g.counters()["deleted"] == n - survivors.size
+    # and the same through a step: everything flies out of the top face at once
+    g2 = Sim(nx, ny, nz, d, d, d, 0.0, 0.0, 0.0, W.courant_dt(d, d, d), 1, [n])
+    g2.set_option("absorb_mask", 4)
+    ztop = (nz - 1e-3 * rng.random(n)) * d
+    g2.load_particles(0, -W.Q_E, W.M_E, x, y, ztop, zero, zero, np.full(n, 5.0 * C_LIGHT), np.ones(n))
+    g2.step(1)
+    assert g2.num_particles(0) == 0 and g2.counters()["deleted"] == n
+
+
+@pytest.mark.parametrize("absorb_first", [True, False])
+def test_absorbing_face_stays_open_whatever_order_the_masks_are_set_in(Sim, absorb_first):
+    """pic.h: absorb_mask implies the same bits of open_mask.  Setting open_mask afterwards (BrickStepper always does)
+    used to drop them: particles were wrapped through a face whose guards are zeroed."""
+    nx, ny, nz, d = 8, 8, 8, 0.5e-6
+    g = Sim(nx, ny, nz, d, d, d, 0.0, 0.0, 0.0, W.courant_dt(d, d, d), 1, [4])
+    if absorb_first:
+        g.set_option("absorb_mask", 4)
+        g.set_option("open_mask", 0)
+    else:
+        g.set_option("open_mask", 0)
+        g.set_option("absorb_mask", 4)
+    one = np.ones(1)
+    # one particle a thousandth of a cell below the top z face, moving up at 0.98 c: it must leave, not wrap
+    g.load_particles(0, -W.Q_E, W.M_E, 4.2 * d * one, 3.3 * d * one, (nz - 1e-3) * d * one, 0 * one, 0 * one,
+                     5.0 * C_LIGHT * one, one)
+    g.step(1)
+    assert g.num_particles(0) == 0 and g.counters()["deleted"] == 1
