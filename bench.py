@@ -56,20 +56,46 @@ YEE_BYTES_PER_CELL = 240.0
 # fp64-pipe roofline of the fused kernel.  ALGORITHMIC fp64-pipe instructions per particle
 # (an FMA counts once): order 3 = gather 6 x (64 + 16 + 4) = 504 FMA + nine shape-weight sets ~108
 # + push and move ~130 + Esirkepov ~465 + ~20; orders 1 and 2 likewise.  What the committed kernel EXECUTES
-# (ncu sm__inst_executed_pipe_fp64, thread level) is reported beside it from profiles/measured_counters.json.
+# (ncu, thread level: DFMA + DADD + DMUL) is reported beside it, parsed from the committed ncu export of that order
+# (profiles/r03_ncu_order<N>.raw.csv): 288 / 883 / 1,204 at orders 1 / 2 / 3 (profiles/r03_orders.md).
 FP64_INSTR_PER_PARTICLE = {1: 380.0, 2: 710.0, 3: 1230.0}
 FP64_LANES_PER_SM = 64
 N_SM = 148
 SM_MAX_MHZ = 1965.0
 
 
-def _measured_counters(workload_key):
-    """ncu counters of one launch of the dominant kernel at this workload, from the committed capture summary
-    profiles/measured_counters.json (written by hand from `ncu --set full`; names the capture it came from).
-    None when there is no capture of this workload: the bench then reports traffic = null."""
+def _measured_counters(config_index, order):
+    """ncu counters of ONE launch of the dominant kernel, parsed from the committed `ncu --page raw --csv` export of a
+    `ncu --set full` capture (profiles/r03_ncu_order<N>.raw.csv; the command that made it is in profiles/r03_orders.md).
+    Only configs[2] at full size has captures, one per shape order.  Nothing is copied by hand: the numbers are read
+    from the export, whose name and sha256 go into the bench line.  None when there is no capture of this workload:
+    the bench then reports traffic = null."""
+    if config_index != 2:
+        return None
+    path = os.path.join(ROOT, "profiles", "r03_ncu_order%d.raw.csv" % order)
     try:
-        with open(os.path.join(ROOT, "profiles", "measured_counters.json")) as fh:
-            return json.load(fh).get(workload_key)
+        import csv
+        import hashlib
+        with open(path, "rb") as fh:
+            sha = hashlib.sha256(fh.read()).hexdigest()
+        with open(path, newline="") as fh:
+            rows = list(csv.reader(fh))
+        d = dict(zip(rows[0], rows[2]))
+
+        def num(k):
+            return float(d[k].replace(",", ""))
+        units = dict(zip(rows[0], rows[1]))
+        scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+        dram = sum(num(k) * scale[units[k]] for k in ("dram__bytes_read.sum", "dram__bytes_write.sum"))
+        npart = 134217728.0
+        cycles = num("sm__cycles_elapsed.max")
+        fp64 = sum(num("smsp__sass_thread_inst_executed_op_%s_pred_on.sum.per_cycle_elapsed" % op)
+                   for op in ("dfma", "dadd", "dmul")) * cycles / npart
+        lsu = num("SM_A.TriageCompute.l1tex__data_pipe_lsu_wavefronts.avg") * N_SM / npart
+        return {"source": "profiles/%s (ncu --set full, one launch, 256^3 x 8 ppc; profiles/r03_orders.md)" % os.path.basename(path),
+                "sha256": sha, "kernel": d.get("Kernel Name"), "dram_bytes_per_launch": dram,
+                "executed_fp64_instr_per_particle": round(fp64, 1), "lsu_wavefronts_per_particle": round(lsu, 2),
+                "gpu_time_ms_under_ncu": num("gpu__time_duration.sum")}
     except Exception:
         return None
 
@@ -355,13 +381,14 @@ def run_ours(args):
     fp64_per_particle = FP64_INSTR_PER_PARTICLE.get(wl.order, FP64_INSTR_PER_PARTICLE[3])
     fp64_alg = fp64_per_particle * np_launch
     fp64_ach = fp64_alg / (ms_launch * 1e-3) / 1e12
-    full_size = args.n is None and args.ppc is None and args.order is None
-    mc = _measured_counters("configs[%d]" % args.config) if full_size else None
+    full_size = args.n is None and args.ppc is None
+    mc = _measured_counters(args.config, wl.order) if full_size else None
     roofline = {"bound": "alu", "kernel": kname, "achieved": fp64_ach, "peak": fp64_peak,
                 "peak_kind": "derived: 148 SMs x 64 fp64 lanes/clk x 1965 MHz (DESIGN.md 5.1; DFMA probe: 62.5 lanes/clk/SM)",
                 "unit": "T fp64-instr/s", "frac": fp64_ach / fp64_peak,
                 "traffic": mc.get("dram_bytes_per_launch") if mc else None,
                 "traffic_source": mc.get("source") if mc else None,
+                "traffic_sha256": mc.get("sha256") if mc else None,
                 "ms_per_launch": ms_launch, "algorithmic_fp64_instr_per_particle": fp64_per_particle,
                 "algorithmic_fp64_instr_per_launch": fp64_alg,
                 "executed_fp64_instr_per_particle": mc.get("executed_fp64_instr_per_particle") if mc else None,
