@@ -161,6 +161,14 @@ int pic_step(pic_ctx*, int nsteps);
  * per-tile kernel of the next pic_step, which reads its inputs through the
  * permutation at no extra pass over the data; the observable result is the
  * same.  Asynchronous.
+ * What not sorting costs (one B200, round 2/3 measurements, DESIGN.md section
+ * 6): the fused kernel is fastest on the step right after a sort; sorting every
+ * step costs 1.4 ms at 134 M particles and the step then takes 31.0 ms, while
+ * a species that drifts for four steps runs the slower "drift" instantiation:
+ * configs[1] 8.2 ms per step sorted every 4 steps against 7.0 ms sorted every
+ * step, configs[3] 15.0 against 7.4 ms, configs[4] 50.7 against 33.4 ms.  A
+ * caller that does not need a particular cadence should sort every step, or
+ * set the option "auto_sort" and let pic_step do it.
  */
 int pic_sort(pic_ctx*);
 
@@ -260,6 +268,13 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *                    particle's new cell key, so that the next pic_sort
  *                    skips its pass over the positions; 0 = pic_sort always
  *                    computes the keys itself
+ *   "auto_sort"      k > 0 = pic_step (and stage 0 of pic_step_stage) sorts by
+ *                    itself, exactly as pic_sort would, before any step on which
+ *                    a loaded species is unsorted or has taken k steps since its
+ *                    last sort; 1 keeps every step on the fused kernel's fastest
+ *                    instantiation.  The container order then changes inside
+ *                    pic_step, the values do not (beyond summation order).
+ *                    0 (default) = only the caller sorts.
  *   "drift_watch"    1 (default) = after every fused-kernel launch the library
  *                    reads back (asynchronously, never waiting) how many
  *                    particles left the fast per-cell deposit path; a species

@@ -85,6 +85,7 @@ struct pic_ctx {
     // the last pic_step iteration; evaluated by a later pic_step once the event has completed, never waited on
     DevStatus* watch = nullptr;         // [MAX_SPECIES + 1]
     cudaEvent_t watch_ev = nullptr;
+    int auto_sort = 0;                     // option "auto_sort": pic_step sorts a species every this many steps (0 = never)
     bool watch_armed = false;
     unsigned long long watch_sorts = 0;    // c->sorts when the snapshot was armed: a pic_sort since then voids it
     bool watch_tile[MAX_SPECIES] = {false};
@@ -549,6 +550,8 @@ static int discard_at_absorbing_faces(pic_ctx* c) {
 
 // mask: bit 0 = J := 0, particles, J fold (and smoothing); bit 1 = first B half push; bit 2 = E push;
 // bit 3 = second B half push (ends the step).  pic_step runs all four; pic_step_stage one at a time (bricks).
+static int sort_impl(pic_ctx* c);
+
 static int step_impl(pic_ctx* c, int nsteps, int mask) {
     if (nsteps < 0) return fail(c, PIC_EINVAL, "nsteps < 0");
     bool any = false;
@@ -564,6 +567,19 @@ static int step_impl(pic_ctx* c, int nsteps, int mask) {
     const YeeMaps* tma_B = ((c->yee_tma & 1) && c->yee_tma_ok) ? &c->yee_maps : nullptr;
     const YeeMaps* tma_E = ((c->yee_tma & 2) && c->yee_tma_ok) ? &c->yee_maps : nullptr;
     for (int it = 0; it < nsteps; ++it) {
+        if ((mask & 1) && c->auto_sort > 0) {
+            // option "auto_sort" = k: the library keeps the fused per-tile kernel on its fast path by sorting (deferred:
+            // keys, ranks and the permutation only) whenever a species is unsorted or has taken k steps since its last sort
+            bool due = false;
+            for (int s = 0; s < c->nspecies; ++s) {
+                const Species& S = c->sp[s];
+                due = due || (S.loaded && S.n > 0 && (!S.sorted || S.steps_since_sort >= c->auto_sort));
+            }
+            if (due) {
+                const int rc = sort_impl(c);
+                if (rc != PIC_OK) return rc;
+            }
+        }
         cudaEvent_t* ev = nullptr;
         if (timing) {
             size_t first;
@@ -847,6 +863,11 @@ int pic_sort(pic_ctx* c) {
     bool any = false;
     for (int s = 0; s < c->nspecies; ++s) any = any || c->sp[s].loaded;
     if (!any) return fail(c, PIC_ESTATE, "pic_sort before any pic_load_particles");
+    return sort_impl(c);
+}
+
+// every loaded species; asynchronous (pic_sort, and pic_step itself under the option "auto_sort")
+static int sort_impl(pic_ctx* c) {
     cudaEvent_t* ev = nullptr;
     nvtxRangePushA("pic_sort");
     if (c->stage_timing) {
@@ -1014,6 +1035,10 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
     else if (!strcmp(name, "sort_deferred")) c->sort_deferred = value != 0;
     else if (!strcmp(name, "fuse_keys")) c->fuse_keys = value != 0;
     else if (!strcmp(name, "drift_watch")) c->drift_watch = value != 0;
+    else if (!strcmp(name, "auto_sort")) {
+        if (value < 0 || value > 1000000) return fail(c, PIC_EINVAL, "auto_sort must be 0 (off) or a number of steps");
+        c->auto_sort = (int)value;
+    }
     else if (!strcmp(name, "open_mask")) {
         if (value < 0 || value > 7) return fail(c, PIC_EINVAL, "open_mask must be 0 .. 7");
         c->g.open_mask = (int)value | c->absorb_mask;     // an absorbing face stays open whatever the brick layout says

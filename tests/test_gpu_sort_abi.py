@@ -271,3 +271,30 @@ def test_selfcheck_module_passes():
     from paper_2303_12873_b200 import selfcheck
     selfcheck.run_case(12, 3, "drift", verbose=False)
     selfcheck.run_case(12, 1, "global", verbose=False)
+
+
+def test_auto_sort_keeps_the_fast_path_without_the_caller_sorting(ora):
+    """Option "auto_sort" = 1: pic_step sorts by itself before every step, so a caller that never calls pic_sort still
+    runs the fused per-tile kernel; the physics is the oracle's (which never sorts) within the step tolerances."""
+    from paper_2303_12873_b200 import workloads as W
+    from paper_2303_12873_b200.binding import Sim
+    import parity_util as P
+    wl = W.uniform_plasma(16, 8, 24, ppc=6, u_th=0.05, order=3, seed=11, protons=True, shuffle=True)
+    o, g = P.make_pair(ora, Sim, wl)
+    g.set_option("auto_sort", 1)
+    o.step(1); g.step(1)
+    P.check_step_parity(o, g, wl, "auto_sort step 1")
+    o.step(3); g.step(3)
+    assert P.field_l2_error(o.get_fields(), g.get_fields()) <= P.TOL_FIELD_L2_10STEP
+    c = g.counters()
+    assert c["sorts"] == 4 and c["steps"] == 4
+    assert c["global"] == 0 and c["fast"] > 0.9 * 4 * wl.nparticles      # every launch was the fused kernel
+    off = g.get_cell_offsets(0)
+    assert off[-1] == wl.species[0].n and np.all(np.diff(off.astype(np.int64)) >= 0)
+    # k = 3: sorts before steps 1 and 4 only
+    o2, g2 = P.make_pair(ora, Sim, wl)
+    g2.set_option("auto_sort", 3)
+    g2.step(4)
+    assert g2.counters()["sorts"] == 2
+    with pytest.raises(Exception):
+        g2.set_option("auto_sort", -1)
