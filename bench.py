@@ -415,8 +415,7 @@ def run_ours(args):
     roofline_yee = None
     if yee_ms > 0:
         yee_gbs = YEE_BYTES_PER_CELL * ncell / (yee_ms * 1e-3) / 1e9
-        yee_kernels = {2: "yee_pipe_kernel<B> x2 + yee_pipe_kernel<E> (persistent, TMA ring)",
-                       1: "push_B_tma_kernel x2 + push_E_tma_kernel (one tile per block)"}.get(
+        yee_kernels = {1: "push_B_tma_kernel x2 + push_E_tma_kernel (one tile per block)"}.get(
                            c1.get("yee_tma"), "push_B_kernel x2 + push_E_kernel (plain: the TMA tensor maps could not be built)")
         roofline_yee = {"bound": "hbm", "kernel": yee_kernels, "achieved": yee_gbs,
                         "peak": hbm_peak, "peak_kind": hbm_kind, "unit": "GB/s", "frac": yee_gbs / hbm_peak,

@@ -214,8 +214,7 @@ int pic_get_cell_offsets(pic_ctx*, int species, unsigned int* offsets, int dst_o
  *       particle found outside its tile's halo)
  *   [3] kernels launched by the library
  *   [4] steps completed     [5] sorts completed
- *   [6] 1 = the one-tile-per-block TMA Yee kernels run (default), 2 = the
- *       persistent pipelined TMA kernels (option "yee_pipe" 1), 0 = the tensor maps could not be
+ *   [6] 1 = the TMA-staged Yee kernels run (default), 0 = the tensor maps could not be
  *       built at pic_init_grid and pic_step runs the plain Yee kernels (same
  *       values, about 40 % slower); pic_last_error right after pic_init_grid
  *       then holds a warning
@@ -248,11 +247,6 @@ int pic_get_stage_ms(pic_ctx*, float* ms /*host*/);
  *   "yee_tma"        bit 0 = B push, bit 1 = E push through the TMA-staged
  *                    tile kernels; 3 (default) = both, 0 = plain one-thread-
  *                    per-cell kernels (same arithmetic, bit-identical result)
- *   "yee_pipe"       0 (default) = one block per 32 x 8 x 4 / 32 x 8 x 8 tile; 1 = the
- *                    TMA Yee pushes run as persistent blocks (one per SM) that
- *                    stream 32 x 8 x 4-cell tiles through a shared-memory ring,
- *                    every operand brought in by TMA (measured slower, see
- *                    profiles/r02_yee.md).  Bit-identical results.
  *   "tile_fresh"     1 (default) = a species that has not stepped since its
  *                    last pic_sort runs the small-stencil, two-blocks-per-SM
  *                    variant of the fused per-tile kernel; 0 = always the

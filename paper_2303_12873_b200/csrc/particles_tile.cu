@@ -12,9 +12,7 @@
 // counters (positions staged, positions consumed).  Neither role keeps the
 // other's registers alive: 168 registers and 12 warps per SM instead of 255 and 8.
 // A producer owns RPW consecutive x-rows of the tile; their cells, in order,
-// form its STREAM: cell c occupies the stream positions cp[c] .. cp[c] + n_c - 1
-// (padded to an even length when TileCfg::UG, so that the two lanes of an
-// aligned lane pair always work on particles of the same cell).
+// form its STREAM: cell c occupies the stream positions cp[c] .. cp[c] + n_c - 1.
 //   phase A  (producer) lane <-> stream position, 32 consecutive positions at a time,
 //            ACROSS row boundaries (the lanes stay full: a row of 64 +- 8
 //            particles no longer ends in a nearly empty sub-chunk).  The
@@ -60,16 +58,14 @@ struct FastWin {
 // that has moved since its last pic_sort, 0 right after a sort (every particle is in its listed cell), which
 // shrinks the stencil from 14 x 10 x 10 to 12 x 8 x 8 nodes per component so that TWO blocks fit one SM
 // and one block's prologue (stencil staging: every warp of the block waits) overlaps the other's particles.
-template <int TX_, int TY_, int TZ_, int NP_, int MINB_, int DRIFT_, int RING_, bool UG_, class FT_ = double>
+template <int TX_, int TY_, int TZ_, int NP_, int MINB_, int DRIFT_, int RING_, class FT_ = double>
 struct TileCfg {
     // FT = type of the staged field stencil and of the gather / push arithmetic: double, or float in the
     // mixed-precision mode (pic_set_option "precision" = 1)
     using FT = FT_;
-    static_assert(!UG_ || sizeof(FT_) == 8, "the cell-anchored gather is written for the fp64 stencil");
     // NP producer warps (phase A) and NP consumer warps (phase B), paired one to one
     static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NP = NP_, NW = 2 * NP_, NT = 32 * NW, MINB = MINB_,
                          DRIFT = DRIFT_;
-    static constexpr bool UG = UG_;               // gather on cell-anchored windows (see gather6_cell)
     // The consumer starts on an unfinished row once its producer is within AHEAD records of running out of ring space:
     // 32 (one sub-chunk, i.e. when the producer is about to block) leaves the producers waiting 6 % of their time, 64
     // halves that for a few more partial passes (31.0 instead of 31.9 ms per step; 80: 31.6, 96: 32.1).
@@ -196,46 +192,6 @@ __device__ __forceinline__ void place_new_window(const double (&w)[N + 1], int s
 template <class C>
 __device__ __forceinline__ int tile_word(int x, int y, int z) { return y + C::SZ * z + C::SX * x; }
 
-// ---- gather from the shared stencil on CELL-ANCHORED windows ---------------------------------------
-// The shared-memory return path serves a warp-wide LDS.64 in ONE wavefront instead of two when the two
-// lanes of every aligned lane pair read the same word and the warp reads at most 8 distinct words
-// (profiles/r02_lsu.md).  The stream gives the lanes of a pair particles of the same cell; for them to read
-// the same words, the window a particle gathers from must depend on its CELL only, not on where in the cell
-// it sits.  Per dimension the support of order N starts at one of two nodes for the particles of a cell
-// whenever floor() of the shape's argument can differ from the cell index (order 3 and 1: the staggered
-// windows; order 2: the nodal ones); the gather therefore runs over the union of the two, one node wider,
-// with the weights shifted into place and a zero at the unused end (a zero weight adds exactly 0, so the
-// result is bit-identical to the N+1-point sum).  At order 3 that is 540 loads per particle instead of
-// 384, at one wavefront each instead of 1.8.
-// Gather variant GV = 1 (order N - 1 along the staggered directions, particle_update.cuh): the staggered
-// windows are those of order NS = N - 1 (one node; three nodes with a shift; three nodes).
-template <int N, int GV>
-struct UWin {
-    static constexpr int NS = GatherOrders<N, GV>::NS;
-    static constexpr int WN = (N == 1) ? 2 : 4;            // nodal window: nodes AN .. AN + WN - 1 relative to the cell
-    static constexpr int AN = (N == 1) ? 0 : -1;
-    // staggered window (node m sits at m + 1/2): orders 1 and 3 anchor their support at floor(xi - 1/2), which is the
-    // cell index or one less: NS + 2 nodes; orders 0 and 2 at the cell index itself: NS + 1 nodes
-    static constexpr int WS = (NS == 0) ? 1 : ((NS == 2) ? 3 : NS + 2);
-    static constexpr int AS = (NS == 0) ? 0 : ((NS == 3) ? -2 : -1);
-    static constexpr int ZT = (WN > WS) ? WN : WS;         // trips of the rolled z loop
-};
-
-// N+1 weights whose first node sits `shift` (0 or 1) slots into a window of W >= N+1 slots, padded to P >= W entries
-template <int N, int W, int P>
-__device__ __forceinline__ void place_uniform(const double (&w)[N + 1], int shift, double (&u)[P]) {
-#pragma unroll
-    for (int a = 0; a < P; ++a) {
-        const double v0 = (a <= N) ? w[(a <= N) ? a : 0] : 0.0;
-        if constexpr (W == N + 1) {
-            u[a] = v0;
-        } else {
-            const double v1 = (a >= 1 && a <= N + 1) ? w[(a >= 1 && a <= N + 1) ? a - 1 : 0] : 0.0;
-            u[a] = shift ? v1 : v0;
-        }
-    }
-}
-
 // One z-plane of one component from the shared stencil: sum_b wy[b] sum_a wx[a] F[a,b].
 template <int WX, int WY, int PX, int PY, class C, class T>
 __device__ __forceinline__ T gather_plane(const T* __restrict__ base, const T (&wx)[PX], const T (&wy)[PY]) {
@@ -250,50 +206,9 @@ __device__ __forceinline__ T gather_plane(const T* __restrict__ base, const T (&
     return accy;
 }
 
-// All six components.  (un*) / (us*) = tile slot of the first node of the cell's nodal / staggered window per
-// dimension; wxn .. wzs = the particle's weights placed on those windows.  The z loop is kept ROLLED (the z
-// weights rotate through their register arrays, both padded to ZT entries, and are back in place after ZT
-// trips): the body stays a few hundred instructions instead of a few thousand straight-line ones.
-template <int N, int GV, class C>
-__device__ __forceinline__ void gather6_cell(const double* __restrict__ Et, int unx, int uny, int unz, int usx,
-                                             int usy, int usz, const double (&wxn)[UWin<N, GV>::WN],
-                                             const double (&wyn)[UWin<N, GV>::WN], double (&wzn)[UWin<N, GV>::ZT],
-                                             const double (&wxs)[UWin<N, GV>::WS], const double (&wys)[UWin<N, GV>::WS],
-                                             double (&wzs)[UWin<N, GV>::ZT], double (&eb)[6]) {
-    using U = UWin<N, GV>;
-    using FT = double;
-    constexpr int WN = U::WN, WS = U::WS, ZT = U::ZT;
-    const int o_ex = C::comp_base(0) + tile_word<C>(usx, uny, unz);
-    const int o_ey = C::comp_base(1) + tile_word<C>(unx, usy, unz);
-    const int o_ez = C::comp_base(2) + tile_word<C>(unx, uny, usz);
-    const int o_bx = C::comp_base(3) + tile_word<C>(unx, usy, usz);
-    const int o_by = C::comp_base(4) + tile_word<C>(usx, uny, usz);
-    const int o_bz = C::comp_base(5) + tile_word<C>(usx, usy, unz);
-#pragma unroll
-    for (int k = 0; k < 6; ++k) eb[k] = 0.0;
-    const double* pl = Et;
-#pragma unroll 1
-    for (int c = 0; c < ZT; ++c, pl += C::SZ) {
-        const double zn = wzn[0], zs = wzs[0];
-        if (WN == ZT || c < WN) {      // components that are nodal in z
-            eb[0] = fma(zn, gather_plane<WS, WN, WS, WN, C, FT>(pl + o_ex, wxs, wyn), eb[0]);
-            eb[1] = fma(zn, gather_plane<WN, WS, WN, WS, C, FT>(pl + o_ey, wxn, wys), eb[1]);
-            eb[5] = fma(zn, gather_plane<WS, WS, WS, WS, C, FT>(pl + o_bz, wxs, wys), eb[5]);
-        }
-        if (WS == ZT || c < WS) {      // components that are staggered in z
-            eb[2] = fma(zs, gather_plane<WN, WN, WN, WN, C, FT>(pl + o_ez, wxn, wyn), eb[2]);
-            eb[3] = fma(zs, gather_plane<WN, WS, WN, WS, C, FT>(pl + o_bx, wxn, wys), eb[3]);
-            eb[4] = fma(zs, gather_plane<WS, WN, WS, WN, C, FT>(pl + o_by, wxs, wyn), eb[4]);
-        }
-#pragma unroll
-        for (int k = 0; k < ZT - 1; ++k) { wzn[k] = wzn[k + 1]; wzs[k] = wzs[k + 1]; }
-        wzn[ZT - 1] = zn;
-        wzs[ZT - 1] = zs;
-    }
-}
-
-// The same gather on the particle's OWN windows (N + 1 nodes, NS + 1 along staggered directions; C::UG = false):
-// 384 loads at order 3, at 1.8 wavefronts each.  (g*n) / (f*s) = tile slot of the first nodal / staggered node per
+// All six components on the particle's own windows (N + 1 nodes, NS + 1 along staggered directions): 384 loads at
+// order 3, at 1.8 wavefronts each.  (Cell-anchored windows, 540 loads at one wavefront each, were measured slower
+// in round 2 and removed in round 3: DESIGN.md 5.1, profiles/r02_lsu.md.)  (g*n) / (f*s) = tile slot of the first nodal / staggered node per
 // dimension.  The z weights rotate through arrays padded to ZT = N + 1 entries.
 template <int N, int GV, class C>
 __device__ __forceinline__ void gather6_part(const typename C::FT* __restrict__ Et, int gxn, int gyn, int gzn, int fxs,
@@ -857,18 +772,7 @@ __device__ __forceinline__ void tile_producer(const Grid& g, const Fields& f, co
                 // from global node index to tile slot: slot = node - (t0 - GL) + image shift
                 const int shx = (rx - (ci - t0x)) + C::GL - t0x, shy = (ry - (cj - t0y)) + C::GL - t0y,
                           shz = (rz - (ck - t0z)) + C::GL - t0z;
-                if constexpr (C::UG) {
-                    using U = UWin<N, GV>;
-                    double ws[NS + 1], uxn[U::WN], uyn[U::WN], uzn[U::ZT], uxs[U::WS], uys[U::WS], uzs[U::ZT];
-                    place_uniform<N, U::WN, U::WN>(wxn, fxn - (ci + U::AN), uxn);
-                    place_uniform<N, U::WN, U::WN>(wyn, fyn - (cj + U::AN), uyn);
-                    place_uniform<N, U::WN, U::ZT>(wzn, fzn - (ck + U::AN), uzn);
-                    place_uniform<NS, U::WS, U::WS>(ws, shape_weights<NS>(xi - 0.5, ws) - (ci + U::AS), uxs);
-                    place_uniform<NS, U::WS, U::WS>(ws, shape_weights<NS>(et - 0.5, ws) - (cj + U::AS), uys);
-                    place_uniform<NS, U::WS, U::ZT>(ws, shape_weights<NS>(ze - 0.5, ws) - (ck + U::AS), uzs);
-                    gather6_cell<N, GV, C>(Et, ci + U::AN + shx, cj + U::AN + shy, ck + U::AN + shz, ci + U::AS + shx,
-                                           cj + U::AS + shy, ck + U::AS + shz, uxn, uyn, uzn, uxs, uys, uzs, eb);
-                } else {
+                {
                     // weights in the gather's arithmetic type (the fp64 nodal ones stay for the deposit record)
                     FT gxn[N + 1], gyn[N + 1], gzn[N + 1], wxs[NS + 1], wys[NS + 1], ws[NS + 1], wzs[N + 1];
 #pragma unroll
@@ -1052,7 +956,7 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
         }
     }
 
-    // ---- a producer's stream: its RPW rows, cell by cell, every cell padded to an even length (UG) --------
+    // ---- a producer's stream: its RPW rows, cell by cell ---------------------------------------------------
     const int pair = (warp < C::NP) ? warp : warp - C::NP;
     const Staging<C> S(stg_all + pair * C::STG_W);
     const int row_first = pair * C::RPW;
@@ -1065,7 +969,6 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
             if (c < C::NC) {
                 const int* o = row_off + (row_first + c / C::TX) * (C::TX + 1) + c % C::TX;
                 n = o[1] - o[0];
-                if (C::UG) n = (n + 1) & ~1;
             }
             int incl = n;
 #pragma unroll
@@ -1099,10 +1002,10 @@ particles_tile_kernel(Grid g, Fields f, Particles p, Particles po, const unsigne
 // profiles/r02_tile_kernel.md: one consumer for two producers -- its duty is 56 % -- at 4 + 2 warps per block runs at
 // 34.2 instead of 29.2 ms: decoupling two producers needs rings two rows deep, which shared memory does not have.)
 // *32: the mixed-precision mode (fp32 stencil, gather and push; same tiles and rings).
-using CfgDrift = TileCfg<8, 4, 6, 6, 1, 1, 112, false>;
-using CfgFresh = TileCfg<8, 4, 6, 3, 2, 0, 120, false>;
-using CfgDrift32 = TileCfg<8, 4, 6, 6, 1, 1, 112, false, float>;
-using CfgFresh32 = TileCfg<8, 4, 6, 3, 2, 0, 120, false, float>;
+using CfgDrift = TileCfg<8, 4, 6, 6, 1, 1, 112>;
+using CfgFresh = TileCfg<8, 4, 6, 3, 2, 0, 120>;
+using CfgDrift32 = TileCfg<8, 4, 6, 6, 1, 1, 112, float>;
+using CfgFresh32 = TileCfg<8, 4, 6, 3, 2, 0, 120, float>;
 static_assert(2 * (CfgFresh::SMEM + 1024) <= 228 * 1024, "two fresh-sort blocks must fit one SM");
 static_assert(CfgDrift::SMEM <= 227 * 1024, "the drift block must fit one SM");
 

@@ -983,7 +983,7 @@ int pic_get_counters(pic_ctx* c, unsigned long long* counters) {
     counters[3] = c->launches;
     counters[4] = c->steps;
     counters[5] = c->sorts;
-    counters[6] = c->yee_tma_ok ? (((c->yee_maps.valid & 2) && c->yee_maps.use_pipe) ? 2ull : 1ull) : 0ull;
+    counters[6] = c->yee_tma_ok ? 1ull : 0ull;
     counters[7] = c->fallbacks;
     counters[8] = c->deleted;
     return PIC_OK;
@@ -1030,7 +1030,6 @@ int pic_set_option(pic_ctx* c, const char* name, long long value) {
         if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "force_path must be 0, 1 or 2");
         c->force_path = (int)value;
     } else if (!strcmp(name, "yee_tma")) c->yee_tma = (int)value & 3;
-    else if (!strcmp(name, "yee_pipe")) c->yee_maps.use_pipe = value != 0;
     else if (!strcmp(name, "tile_fresh")) c->tile_fresh = value != 0;
     else if (!strcmp(name, "sort_deferred")) c->sort_deferred = value != 0;
     else if (!strcmp(name, "fuse_keys")) c->fuse_keys = value != 0;

@@ -56,10 +56,8 @@ struct DevStatus {
 // ---- yee.cu ---------------------------------------------------------------
 // Six CUtensorMap objects (Ex Ey Ez Bx By Bz), kept opaque here so that only yee.cu needs <cuda.h>.
 struct YeeMaps {
-    alignas(64) unsigned char map[21 * 128];   // [0..5] one-tile-per-block kernels; [6..20] pipelined kernels
-    int valid;       // bit 0: maps 0..5 built; bit 1: maps 6..20 built and the pipelined kernels configured
-    int use_pipe;    // option "yee_pipe": run the persistent pipelined kernels when they are available
-    int n_sm;
+    alignas(64) unsigned char map[6 * 128];    // Ex Ey Ez Bx By Bz
+    int valid;       // 1: the maps are built and the TMA kernels configured
 };
 int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out);   // 0 = ok; else the plain kernels are used
 // maps == nullptr or !maps->valid: plain one-thread-per-cell kernels; else the TMA-staged tile kernels

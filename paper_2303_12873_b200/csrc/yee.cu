@@ -237,159 +237,12 @@ __global__ void __launch_bounds__(YNT) push_E_tma_kernel(Grid g, Fields f, doubl
     }
 }
 
-// ---- persistent, pipelined variant (option "yee_pipe") ------------------------------------------------------
-// One block per SM walks a contiguous range of work items, item = one (32 x 8 x PTZ)-cell tile, z fastest.  Every
-// operand of an item -- the three curl operands with their one-cell halo AND the components the item updates
-// (and J for the E push) -- is brought into one stage of a shared-memory ring by TMA; thread 0 refills a stage as
-// soon as the block has consumed it, PNST - 1 items ahead, so no warp ever waits on a global load of its own and
-// ~130-190 KB per SM are in flight all the time.  Same expression tree as the plain kernels: bit-identical results.
-// MEASURED (256^3, profiles/r02_yee.md): 2.0 TB/s against 4.7 TB/s for one tile per block -- with every operand on
-// the TMA path the SM's TMA unit delivers only ~10 B/clk for these narrow fp64 boxes (272-byte rows), and a block
-// that owns whole z-columns loses the L2 reuse of the x/y halos (DRAM reads 1.55x algorithmic instead of 1.12x).
-// Kept behind the option as the evidence for that, not as the default.
-namespace {
-
-constexpr int PTZ = 4;                 // z planes per item
-constexpr int PNST_B = 3, PNST_E = 2;  // ring depth (61 KB / 88 KB per stage)
-
-template <bool IS_E> struct PipeGeom {
-    static constexpr int HX = IS_E ? 4 : 2;                         // halo box: 36 or 34 wide (even x corner)
-    static constexpr int HSZ = (YTX + HX) * YBY * (PTZ + 1), HPAD = (HSZ + 15) / 16 * 16;
-    static constexpr int OSZ = YTX * YTY * PTZ;                     // box of a component the item updates / of J
-    static constexpr int NOWN = IS_E ? 6 : 3;
-    static constexpr int NST = IS_E ? PNST_E : PNST_B;
-    static constexpr unsigned TX_BYTES = 8u * (3u * HSZ + (unsigned)NOWN * OSZ);
-};
-
-template <bool IS_E> struct PipeSmem {
-    using G = PipeGeom<IS_E>;
-    alignas(128) double halo[G::NST][3][G::HPAD];
-    alignas(128) double own[G::NST][G::NOWN][G::OSZ];
-    alignas(8) unsigned long long full[G::NST];
-};
-
-struct PipeMaps {
-    CUtensorMap halo[3];    // curl operands (E for the B push, B for the E push), box with halo
-    CUtensorMap own[6];     // updated components, then J (E push only)
-};
-
-}  // namespace
-
-template <bool IS_E>
-__global__ void __launch_bounds__(YNT, 1)
-yee_pipe_kernel(Grid g, Fields f, double cdx, double cdy, double cdz, double dt_eps0, int ntx, int nty, int nzc,
-                const __grid_constant__ PipeMaps maps) {
-    using G = PipeGeom<IS_E>;
-    extern __shared__ __align__(128) unsigned char yee_smem_raw[];
-    PipeSmem<IS_E>& sm = *reinterpret_cast<PipeSmem<IS_E>*>(yee_smem_raw);
-    constexpr int NST = G::NST, HBX = YTX + G::HX;
-    const long long total = (long long)ntx * nty * nzc;
-    const long long per = (total + gridDim.x - 1) / gridDim.x;
-    const long long first = per * blockIdx.x, last = min(total, first + per);
-    if (first >= last) return;
-    const int n_items = (int)(last - first);
-    const int tx = threadIdx.x % YTX, ty = threadIdx.x / YTX;
-
-    auto issue = [&](int it) {       // thread 0: arm the stage's barrier and start the item's nine / six TMA loads
-        const int s = it % NST;
-        const long long item = first + it;
-        const int kz = (int)(item % nzc);
-        const long long col = item / nzc;
-        const int t0x = (int)(col % ntx) * YTX, t0y = (int)(col / ntx) * YTY, t0z = kz * PTZ;
-        const int sh = IS_E ? 1 : 0, shx = IS_E ? 2 : 0;
-        mbar_expect_tx(&sm.full[s], G::TX_BYTES);
-#pragma unroll
-        for (int k = 0; k < 3; ++k)
-            tma_load_box(sm.halo[s][k], &maps.halo[k], &sm.full[s], t0x + NG - shx, t0y + NG - sh, t0z + NG - sh);
-#pragma unroll
-        for (int k = 0; k < G::NOWN; ++k)
-            tma_load_box(sm.own[s][k], &maps.own[k], &sm.full[s], t0x + NG, t0y + NG, t0z + NG);
-    };
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < NST; ++s) mbar_init(&sm.full[s], 1);
-    }
-    __syncthreads();
-    if (threadIdx.x == 0)
-        for (int it = 0; it < NST && it < n_items; ++it) issue(it);
-
-    for (int it = 0; it < n_items; ++it) {
-        const int s = it % NST;
-        const long long item = first + it;
-        const int kz = (int)(item % nzc);
-        const long long col = item / nzc;
-        const int t0x = (int)(col % ntx) * YTX, t0y = (int)(col / ntx) * YTY, t0z = kz * PTZ;
-        const int i = t0x + tx, j = t0y + ty;
-        const bool in_xy = i < g.nx && j < g.ny;
-        mbar_wait(&sm.full[s], (unsigned)((it / NST) & 1));
-        const double* own = &sm.own[s][0][0] + tx + YTX * ty;
-        if constexpr (!IS_E) {
-            const double* Ex = sm.halo[s][0] + tx + HBX * ty;
-            const double* Ey = sm.halo[s][1] + tx + HBX * ty;
-            const double* Ez = sm.halo[s][2] + tx + HBX * ty;
-#pragma unroll
-            for (int c = 0; c < PTZ; ++c) {
-                const int k = t0z + c;
-                if (!(in_xy && k < g.nz)) continue;
-                const int w = HBX * YBY * c, wo = YTX * YTY * c;
-                const double ex = Ex[w], ey = Ey[w], ez = Ez[w];
-                const double nbx = own[wo] - (cdy * (Ez[w + HBX] - ez) - cdz * (Ey[w + HBX * YBY] - ey));
-                const double nby = own[G::OSZ + wo] - (cdz * (Ex[w + HBX * YBY] - ex) - cdx * (Ez[w + 1] - ez));
-                const double nbz = own[2 * G::OSZ + wo] - (cdx * (Ey[w + 1] - ey) - cdy * (Ex[w + HBX] - ex));
-                const long long o = g.idx(i, j, k);
-                f.Bx[o] = nbx;
-                f.By[o] = nby;
-                f.Bz[o] = nbz;
-                if (is_edge(g, i, j, k)) store_images3(g, f.Bx, f.By, f.Bz, i, j, k, nbx, nby, nbz);
-            }
-        } else {
-            const double* Bx = sm.halo[s][0] + (tx + 2) + HBX * (ty + 1) + HBX * YBY;
-            const double* By = sm.halo[s][1] + (tx + 2) + HBX * (ty + 1) + HBX * YBY;
-            const double* Bz = sm.halo[s][2] + (tx + 2) + HBX * (ty + 1) + HBX * YBY;
-#pragma unroll
-            for (int c = 0; c < PTZ; ++c) {
-                const int k = t0z + c;
-                if (!(in_xy && k < g.nz)) continue;
-                const int w = HBX * YBY * c, wo = YTX * YTY * c;
-                const double bx = Bx[w], by = By[w], bz = Bz[w];
-                // same operation order as the plain kernel: (E + curl term) - dt/eps0 J
-                const double nex = (own[wo] + (cdy * (bz - Bz[w - HBX]) - cdz * (by - By[w - HBX * YBY]))) -
-                                   dt_eps0 * own[3 * G::OSZ + wo];
-                const double ney = (own[G::OSZ + wo] + (cdz * (bx - Bx[w - HBX * YBY]) - cdx * (bz - Bz[w - 1]))) -
-                                   dt_eps0 * own[4 * G::OSZ + wo];
-                const double nez = (own[2 * G::OSZ + wo] + (cdx * (by - By[w - 1]) - cdy * (bx - Bx[w - HBX]))) -
-                                   dt_eps0 * own[5 * G::OSZ + wo];
-                const long long o = g.idx(i, j, k);
-                f.Ex[o] = nex;
-                f.Ey[o] = ney;
-                f.Ez[o] = nez;
-                if (is_edge(g, i, j, k)) store_images3(g, f.Ex, f.Ey, f.Ez, i, j, k, nex, ney, nez);
-            }
-        }
-        __syncthreads();                                  // the whole block has read stage s
-        if (threadIdx.x == 0 && it + NST < n_items) issue(it + NST);
-    }
-}
-
-template <bool IS_E>
-static void launch_pipe(const Grid& g, const Fields& f, double cdx, double cdy, double cdz, double dt_eps0,
-                        const YeeMaps* maps, cudaStream_t st) {
-    const int ntx = (g.nx + YTX - 1) / YTX, nty = (g.ny + YTY - 1) / YTY, nzc = (g.nz + PTZ - 1) / PTZ;
-    const long long total = (long long)ntx * nty * nzc;
-    const CUtensorMap* m = reinterpret_cast<const CUtensorMap*>(maps->map);
-    PipeMaps pm;
-    for (int k = 0; k < 3; ++k) pm.halo[k] = m[(IS_E ? 9 : 6) + k];
-    for (int k = 0; k < 3; ++k) pm.own[k] = m[(IS_E ? 12 : 15) + k];          // E push updates E, B push updates B
-    for (int k = 0; k < 3; ++k) pm.own[3 + k] = m[18 + k];                     // J (E push only)
-    const unsigned nb = (unsigned)std::min<long long>(total, maps->n_sm > 0 ? maps->n_sm : 148);
-    yee_pipe_kernel<IS_E><<<nb, YNT, sizeof(PipeSmem<IS_E>), st>>>(g, f, cdx, cdy, cdz, dt_eps0, ntx, nty, nzc, pm);
-}
+// (A persistent variant -- one block per SM streaming items through a TMA ring -- was measured in round 2 at 2.0 TB/s
+// against 4.7 TB/s for one tile per block and removed in round 3; the measurement stays in profiles/r02_yee.md.)
 
 void launch_push_B(const Grid& g, const Fields& f, double dth, const YeeMaps* maps, cudaStream_t st) {
     const double cdx = dth * g.inv_dx, cdy = dth * g.inv_dy, cdz = dth * g.inv_dz;
-    if (maps && (maps->valid & 2) && maps->use_pipe) {
-        launch_pipe<false>(g, f, cdx, cdy, cdz, 0.0, maps, st);
-    } else if (maps && maps->valid) {
+    if (maps && maps->valid) {
         dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ_B - 1) / YTZ_B);
         const CUtensorMap* m = reinterpret_cast<const CUtensorMap*>(maps->map);
         push_B_tma_kernel<YTZ_B><<<nb, YNT, sizeof(YeeSmem<2, YTZ_B>), st>>>(g, f, cdx, cdy, cdz, m[0], m[1], m[2]);
@@ -402,9 +255,7 @@ void launch_push_B(const Grid& g, const Fields& f, double dth, const YeeMaps* ma
 void launch_push_E(const Grid& g, const Fields& f, double dt, const YeeMaps* maps, cudaStream_t st) {
     const double c2dt = C_LIGHT * C_LIGHT * dt;
     const double cdx = c2dt * g.inv_dx, cdy = c2dt * g.inv_dy, cdz = c2dt * g.inv_dz;
-    if (maps && (maps->valid & 2) && maps->use_pipe) {
-        launch_pipe<true>(g, f, cdx, cdy, cdz, dt / EPS0, maps, st);
-    } else if (maps && maps->valid) {
+    if (maps && maps->valid) {
         dim3 nb((g.nx + YTX - 1) / YTX, (g.ny + YTY - 1) / YTY, (g.nz + YTZ_E - 1) / YTZ_E);
         const CUtensorMap* m = reinterpret_cast<const CUtensorMap*>(maps->map);
         push_E_tma_kernel<YTZ_E><<<nb, YNT, sizeof(YeeSmem<4, YTZ_E>), st>>>(g, f, cdx, cdy, cdz, dt / EPS0, m[3], m[4], m[5]);
@@ -417,10 +268,8 @@ void launch_push_E(const Grid& g, const Fields& f, double dt, const YeeMaps* map
 // Tensor maps of the six padded E,B components (rank 3, fp64, no swizzle, zero fill outside the array),
 // box = (YTX + 2) x YBY x (YTZ_B + 1) for E (read by the B push), (YTX + 4) x YBY x (YTZ_E + 1) for B.  The driver entry point is fetched through the runtime (no link-time libcuda).
 int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out) {
-    static_assert(sizeof(CUtensorMap) == 128 && sizeof(out->map) == 21 * 128, "YeeMaps storage");
+    static_assert(sizeof(CUtensorMap) == 128 && sizeof(out->map) == 6 * 128, "YeeMaps storage");
     out->valid = 0;
-    out->use_pipe = 0;      // measured slower than one tile per block (profiles/r02_yee.md): off by default
-    out->n_sm = 0;
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -454,31 +303,6 @@ int make_yee_maps(const Grid& g, const Fields& f, YeeMaps* out) {
         return 3;
     }
     out->valid = 1;
-    // maps of the pipelined kernels: [6..8] E with the B push's halo box, [9..11] B with the E push's halo box,
-    // [12..20] E, B, J with the box of an item (no halo)
-    double* all9[9] = {f.Ex, f.Ey, f.Ez, f.Bx, f.By, f.Bz, f.Jx, f.Jy, f.Jz};
-    for (int k = 0; k < 15; ++k) {
-        double* base = (k < 6) ? comp[k] : all9[k - 6];
-        const cuuint32_t hx = (k < 3) ? 2 : 4;
-        const cuuint32_t box_h[3] = {(cuuint32_t)YTX + hx, YBY, (cuuint32_t)PTZ + 1};
-        const cuuint32_t box_o[3] = {(cuuint32_t)YTX, (cuuint32_t)YTY, (cuuint32_t)PTZ};
-        CUresult r = ((EncodeFn)fn)(&m[6 + k], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides,
-                                    (k < 6) ? box_h : box_o, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return 0;      // the one-tile-per-block TMA kernels remain available
-    }
-    int dev = 0, nsm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-        cudaFuncSetAttribute(yee_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)sizeof(PipeSmem<false>)) != cudaSuccess ||
-        cudaFuncSetAttribute(yee_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)sizeof(PipeSmem<true>)) != cudaSuccess) {
-        cudaGetLastError();
-        return 0;
-    }
-    out->n_sm = nsm;
-    out->valid = 3;
     return 0;
 }
 

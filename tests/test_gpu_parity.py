@@ -196,21 +196,19 @@ def test_yee_vacuum_and_source_exact(ora, Sim):
 
 @pytest.mark.parametrize("dims", [(21, 10, 7), (32, 8, 8), (33, 9, 17), (70, 5, 3), (2, 1, 40), (96, 24, 13)])
 def test_yee_tma_and_plain_kernels_agree(ora, Sim, dims):
-    """The persistent pipelined TMA Yee kernels (default), the one-tile-per-block TMA kernels and the plain
-    one-thread-per-cell kernels evaluate the same expression tree: bit-identical E, B after 4 steps on grids that
-    are smaller than, equal to and ragged against the 32 x 8 x 4 / 32 x 8 x 8 Yee tiles (the last grid gives
-    every persistent block several items, so that ring stages are reused); all within 1e-13 of the oracle
+    """The TMA-staged tile kernels (default) and the plain one-thread-per-cell kernels evaluate the same expression
+    tree: bit-identical E, B after 4 steps on grids that are smaller than, equal to and ragged against the
+    32 x 8 x 4 / 32 x 8 x 8 Yee tiles; all within 1e-13 of the oracle
     (J = 0: one q = 0 particle)."""
     nx, ny, nz = dims
     wl = W.uniform_plasma(nx, ny, nz, ppc=1, u_th=0.0, order=1, seed=2, dx=0.4e-6, dy=0.5e-6, dz=0.3e-6)
     wl.species[0].q = 0.0
     wl.fields = _rand_fields(wl, 7)
     out = []
-    for mode, pipe in ((3, 1), (3, 0), (0, 1), (1, 1), (2, 0)):   # pipelined, per-tile TMA, plain, B only, E only
+    for mode in (3, 0, 1, 2):   # per-tile TMA, plain, B only, E only
         o, g = make_pair(ora, Sim, wl)
         g.set_option("yee_tma", mode)
-        g.set_option("yee_pipe", pipe)
-        assert g.counters()["yee_tma"] == (2 if pipe else 1)
+        assert g.counters()["yee_tma"] == 1
         g.step(4)
         out.append(g.get_fields())
     o.step(4)
