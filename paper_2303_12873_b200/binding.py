@@ -25,8 +25,7 @@ SYMBOLS = ("pic_query_arena", "pic_init_grid", "pic_set_fields", "pic_load_parti
            "pic_get_counters", "pic_get_stage_ms", "pic_set_option", "pic_sync", "pic_last_error",
            "pic_destroy", "pic_version", "pic_step_stage", "pic_halo_doubles", "pic_export_halo",
            "pic_import_halo", "pic_export_leavers", "pic_import_arrivals", "pic_shift_window", "pic_add_plane",
-           "pic_set_damping",
-           "pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
+           "pic_set_damping")
 # include/pic_noalloc.h
 NOALLOC_SYMBOLS = ("pic_cell_offsets_noalloc", "pic_noalloc_last_error")
 NOALLOC_MAX_CELLS = 2048 * 16384 - 1
@@ -83,10 +82,6 @@ def load_library(path: str | None = None):
     L.pic_shift_window.argtypes = [vp, i, C.POINTER(ll)]
     L.pic_add_plane.argtypes = [vp, i, i, vp, i]
     L.pic_set_damping.argtypes = [vp, i, C.POINTER(d)]
-    L.pic_probe_dfma.argtypes = [i, i, C.POINTER(d)]
-    L.pic_probe_dmma.argtypes = [i, i, C.POINTER(d)]
-    L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
-    L.pic_probe_red.argtypes = [i, ll, ll, i, C.POINTER(d)]
     L.pic_cell_offsets_noalloc.argtypes = [i, i, i, d, d, d, d, d, d, ll, vp, vp, vp, vp, vp]
     L.pic_cell_offsets_noalloc.restype = i
     L.pic_noalloc_last_error.argtypes = []

@@ -11,7 +11,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpic_b200.so")
-SOURCES = ["pic_api.cu", "yee.cu", "particles_global.cu", "particles_tile.cu", "sort.cu", "peaks.cu", "bricks.cu", "noalloc.cu"]
+SOURCES = ["pic_api.cu", "yee.cu", "particles_global.cu", "particles_tile.cu", "sort.cu", "bricks.cu", "noalloc.cu"]
+# measurement probes (the only code that calls cudaMalloc): a library of their own, include/pic_probes.h
+PROBE_SOURCES = ["peaks.cu"]
+PROBE_LIB = os.path.join(HERE, "libpic_probes.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 
@@ -33,12 +36,13 @@ def _deps_mtime() -> float:
 
 
 def build_library(force: bool = False, verbose: bool = False) -> str:
-    """Compile every .cu under csrc/ and link the shared library.  Returns its path."""
+    """Compile every .cu under csrc/ and link libpic_b200.so (the product) and libpic_probes.so (measurement probes).
+    Returns the path of the former."""
     os.makedirs(OBJ, exist_ok=True)
     hdr_t = _deps_mtime()
     nvcc = _nvcc()
     jobs = []
-    for src in SOURCES:
+    for src in SOURCES + PROBE_SOURCES:
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr_t):
@@ -64,6 +68,13 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         if r.returncode != 0:
             raise RuntimeError("link failed:\n%s\n%s" % (r.stdout, r.stderr))
         os.replace(tmp, LIB)
+    pobjs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in PROBE_SOURCES]
+    if jobs or force or not os.path.exists(PROBE_LIB):
+        tmp = PROBE_LIB + ".tmp%d" % os.getpid()
+        r = subprocess.run([nvcc, "-shared", "-o", tmp, *pobjs, "-lcudart"], capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("link failed:\n%s\n%s" % (r.stdout, r.stderr))
+        os.replace(tmp, PROBE_LIB)
     return LIB
 
 

@@ -2,14 +2,16 @@
 // DESIGN.md section 5 are quoted against ("Builder must measure
 // first: fp64 FMA peak ..., shared-memory LDS.64 wavefront rate with 1/2/4
 // distinct addresses per warp ..., global fp64 red.add rate at L2").  They
-// sit behind the C ABI (include/pic.h, pic_probe_*) so that one committed
+// sit behind a C ABI of their own (include/pic_probes.h, libpic_probes.so) so that one committed
 // command -- python -m paper_2303_12873_b200.peaks -- prints the table and
 // the same command can be put under ncu for the wavefront counters.
 // Unlike the simulation calls, the probes allocate their few MB of scratch
-// themselves (cudaMalloc on the current device, default stream) and free it.
+// themselves (cudaMalloc on the current device, default stream) and free it:
+// they are built into a separate library so that libpic_b200.so never allocates.
 #include <stdio.h>
 
 #include "pic_internal.h"
+#include "../../include/pic_probes.h"
 
 namespace pic {
 namespace {

@@ -189,10 +189,17 @@ int copy_out(pic_ctx* c, const double* pad, double* dst, int on_device) {
         pack_kernel<<<cell_grid(c->g), 128, 0, c->stream>>>(c->g, pad, dst);
         ++c->launches;
     } else {
-        pack_kernel<<<cell_grid(c->g), 128, 0, c->stream>>>(c->g, pad, c->tmp);
-        ++c->launches;
-        CU(c, cudaMemcpyAsync(dst, c->tmp, bytes, cudaMemcpyDeviceToHost, c->stream));
-        CU(c, cudaStreamSynchronize(c->stream));   // tmp is reused by the next component
+        // one strided DMA copy straight out of the padded array (rows of nx doubles, pitch px): no staging buffer, no
+        // pack kernel and no synchronisation between components -- pic_get_fields waits once, at its end
+        const Grid& g = c->g;
+        cudaMemcpy3DParms p3 = {};
+        p3.srcPtr = make_cudaPitchedPtr(const_cast<double*>(pad) + g.idx(0, 0, 0), (size_t)g.px * sizeof(double),
+                                        (size_t)g.nx * sizeof(double), (size_t)g.py);
+        p3.dstPtr = make_cudaPitchedPtr(dst, (size_t)g.nx * sizeof(double), (size_t)g.nx * sizeof(double), (size_t)g.ny);
+        p3.extent = make_cudaExtent((size_t)g.nx * sizeof(double), (size_t)g.ny, (size_t)g.nz);
+        p3.kind = cudaMemcpyDeviceToHost;
+        CU(c, cudaMemcpy3DAsync(&p3, c->stream));
+        (void)bytes;
     }
     return PIC_OK;
 }

@@ -7,7 +7,7 @@ kernel's [x][z][y] stencil strides, and the global ``red.add.f64`` rate.
     python -m paper_2303_12873_b200.peaks --lds      # only the LDS table (one launch per row: for ncu)
 
 Argument marshalling only; the probes are CUDA kernels behind the C ABI
-(``pic_probe_*`` in include/pic.h, csrc/peaks.cu).
+(``pic_probe_*`` in include/pic_probes.h, csrc/peaks.cu, built into libpic_probes.so).
 """
 from __future__ import annotations
 
@@ -15,7 +15,32 @@ import ctypes as C
 import json
 import sys
 
-from .binding import PIC_OK, PicError, load_library
+import os
+
+from .binding import PIC_OK, PicError
+
+PROBE_SYMBOLS = ("pic_probe_dfma", "pic_probe_dmma", "pic_probe_lds", "pic_probe_red")
+_PROBE_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libpic_probes.so")
+_probe_lib = None
+
+
+def load_library():
+    """dlopen libpic_probes.so (include/pic_probes.h): the probes allocate device memory themselves, so they
+    are kept out of libpic_b200.so.  Raises if it has not been built."""
+    global _probe_lib
+    if _probe_lib is None:
+        if not os.path.exists(_PROBE_LIB_PATH):
+            raise FileNotFoundError("%s is missing: build it with `python -m paper_2303_12873_b200.build`" % _PROBE_LIB_PATH)
+        L = C.CDLL(_PROBE_LIB_PATH)
+        i, d, ll = C.c_int, C.c_double, C.c_longlong
+        L.pic_probe_dfma.argtypes = [i, i, C.POINTER(d)]
+        L.pic_probe_dmma.argtypes = [i, i, C.POINTER(d)]
+        L.pic_probe_lds.argtypes = [i, C.POINTER(i), C.c_uint, i, i, i, C.POINTER(d)]
+        L.pic_probe_red.argtypes = [i, ll, ll, i, C.POINTER(d)]
+        for name in PROBE_SYMBOLS:
+            getattr(L, name).restype = i
+        _probe_lib = L
+    return _probe_lib
 
 # the fresh-sort tile kernel's stencil strides: word(x, y, z) = y + SZ z + SX x
 SZ, SX = 8, 66

@@ -28,6 +28,22 @@ def test_header_symbols_all_exported(lib):
         assert hasattr(lib, name), name
 
 
+def test_probe_library_is_separate_and_the_product_library_never_allocates(lib):
+    """include/pic_probes.h: the machine-rate probes (the only code that calls cudaMalloc) live in libpic_probes.so;
+    libpic_b200.so exports none of them and does not even import cudaMalloc / cudaFree."""
+    import subprocess
+    from paper_2303_12873_b200 import binding, peaks
+    hdr = open(os.path.join(ROOT, "include", "pic_probes.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    assert set(re.findall(r"\b(pic_[a-z_]+)\s*\(", hdr)) == set(peaks.PROBE_SYMBOLS)
+    P = peaks.load_library()
+    for name in peaks.PROBE_SYMBOLS:
+        assert hasattr(P, name) and not hasattr(lib, name), name
+    undefined = subprocess.run(["nm", "-D", "--undefined-only", binding.LIB_PATH], capture_output=True, text=True).stdout
+    for sym in ("cudaMalloc", "cudaFree", "cudaMallocAsync", "cudaMallocManaged"):
+        assert not re.search(r"\b%s\b" % sym, undefined), sym
+
+
 def test_version_and_null_ctx_behaviour(lib):
     assert b"sm_100a" in lib.pic_version()
     assert lib.pic_last_error(None) == b"NULL context"
