@@ -1,7 +1,7 @@
 // particles_tile.cu -- fused gather + Boris push + Esirkepov deposition per
 // cell-sorted tile (BASELINE.json:north_star parts
 // 1-3, "fused per cell-sorted tile").  Kernel v9 of DESIGN.md section 5.1;
-// measurements in profiles/r02_tile_kernel.md (v1-v8: profiles/r01_*).
+// measurements in profiles/r02_tile_kernel.md (v1-v8: profiles/r01_summary.md).
 //
 // One thread block owns a tile of TX x TY x TZ cells; its E,B stencil (+ halo
 // for the shape support and DRIFT cells of drift since the last pic_sort) is

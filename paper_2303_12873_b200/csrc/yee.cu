@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(128) push_E_kernel(Grid g, Fields f, double cd
 namespace {
 
 constexpr int YTX = 32, YTY = 8;                           // cells per block in x, y (one thread each)
-constexpr int YTZ_B = 4, YTZ_E = 8;                        // z planes a thread walks (measured best: 256^3, profiles/r01_v4)                  // cells per block
+constexpr int YTZ_B = 4, YTZ_E = 8;                        // z planes a thread walks (measured best at 256^3: profiles/r02_yee.md)                  // cells per block
 // Staged box: the tile plus one halo cell in y and z and, in x, 2 cells: with 8-byte elements the box corner
 // must sit on an EVEN x coordinate (TMA wants the first byte of a box row 16-byte aligned; an odd coordinate
 // raises "illegal instruction"), so the E push (backward differences) starts 2 cells below the tile, not 1.
